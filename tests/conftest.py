@@ -1,0 +1,63 @@
+import os
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+
+
+class TinyCase:
+    """A tiny random DAO instance (not a phantom): n_beams x rows x cols beamlets, random sparse D."""
+
+    def __init__(self, seed=0, n_vox=60, n_beams=2, rows=2, cols=3, density=0.5):
+        rng = np.random.default_rng(seed)
+        self.n_vox, self.n_beams = n_vox, n_beams
+        self.n_rows = n_beams * rows
+        self.n_bl = self.n_rows * cols
+        self.beam_row_ptr = (np.arange(n_beams + 1) * rows).astype(np.int32)
+        self.row_bl_ptr = (np.arange(self.n_rows + 1) * cols).astype(np.int32)
+        mask = rng.random((n_vox, self.n_bl)) < density
+        mask[np.arange(n_vox), rng.integers(0, self.n_bl, n_vox)] = True     # no empty voxel rows
+        dense = np.where(mask, rng.uniform(0.05, 1.0, (n_vox, self.n_bl)), 0.0).astype(np.float32)
+        self.dense = dense.astype(np.float64)
+        self.row_ptr = np.r_[0, np.cumsum(mask.sum(1))].astype(np.int32)
+        r, c = np.nonzero(mask)
+        self.col_idx = c.astype(np.int32)
+        self.val = dense[r, c].astype(np.float32)
+        self.nnz = int(self.val.size)
+        # structures: 0 = target (first third), 1 = OAR (second third), -1 = rest
+        vs = np.full(n_vox, -1, dtype=np.int32)
+        vs[: n_vox // 3] = 0
+        vs[n_vox // 3: 2 * n_vox // 3] = 1
+        self.vox_struct = rng.permutation(vs).astype(np.int32)
+        self.n_struct = 2
+        self.t_under = np.array([1.0, 0.0], dtype=np.float32)
+        self.w_under = np.array([10.0, 0.0], dtype=np.float32)
+        self.t_over = np.array([1.05, 0.3], dtype=np.float32)
+        self.w_over = np.array([5.0, 2.0], dtype=np.float32)
+        self.prescription = 1.0
+        self.name = f"tiny{seed}"
+
+
+@pytest.fixture(scope="session")
+def tiny():
+    return TinyCase(seed=1)
+
+
+@pytest.fixture(scope="session")
+def cfg0():
+    from paper_1003_5402_b200.inputs import phantom
+    return phantom.make("cfg0", seed=0)
+
+
+@pytest.fixture(scope="session")
+def mini():
+    from paper_1003_5402_b200.inputs import phantom
+    return phantom.make("mini", seed=0)
