@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""bench.py -- seconds per 50-aperture DAO plan on the 9-field prostate phantom (BASELINE.json
+configs[1]), plus the SpMV / SpMV^T HBM roofline fractions, on N GPUs of one node.
+
+A "step" is one whole plan: 50 column-generation iterations of the hot path (intensities -> dose
+SpMV + objective/gradient -> transposed SpMV -> pricing -> aperture column -> master solve) and the
+final dose evaluation, through the C ABI (`dao_run`).  N > 1 runs N independent replicas (the
+path does not shard at these sizes: DESIGN.md "Multi-GPU"), one process per GPU under torchrun.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg1] [--impl reference]
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the fp64 CPU oracle instead (a bounded
+sample of the same workload on the host cores).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "50-aperture DAO plan time"
+N_APERTURES = 50
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        sm = [float(r[1]) for r in self.rows if len(r) >= 9 and r[1].replace(".", "").isdigit()]
+        mx = [float(r[2]) for r in self.rows if len(r) >= 9 and r[2].replace(".", "").isdigit()]
+        reasons = set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) >= 9:
+                for n, v in zip(names, r[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# --------------------------------------------------------------------------------------------
+def algorithmic_bytes(ph, sell_elems=None):
+    """what each kernel class must move per launch (padding / re-reads excluded)."""
+    V, N, nnz, R = ph.n_vox, ph.n_bl, ph.nnz, ph.n_rows
+    return {
+        "spmv": 8 * nnz + 4 * (V + 1) + 4 * N + 4 * V + V + 4 * V,      # + sid + fused g
+        "spmv_t": 8 * nnz + 4 * (N + 1) + 4 * V + 4 * N,
+        "price": 4 * N + 4 * (R + 1) + 12 * R,
+        "column": 8 * nnz + 4 * (V + 1) + 4 * N + 4 * V,
+    }
+
+
+def run_reference(args, rank, world):
+    """The reference arm: the oracle, as it stands, on the host cores; bounded sample."""
+    if rank != 0:
+        return
+    from oracle import dao_oracle as orc
+    from paper_1003_5402_b200.inputs import phantom
+    orc.build()
+    ph = phantom.make(args.config, 0)
+    n_ap = args.ref_apertures
+    times = []
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        orc.run(ph, n_ap)
+        dt = time.perf_counter() - t0
+        if i >= args.warmup:
+            times.append(dt)
+    per_plan = float(np.mean(times)) * N_APERTURES / n_ap
+    cpu = {"value": per_plan, "unit": "s", "cores": 1, "kind": "oracle",
+           "sample": f"first {n_ap} of {N_APERTURES} column-generation iterations of {ph.name}, time scaled by {N_APERTURES}/{n_ap} "
+                     "(later iterations carry larger master problems, so this under-states the full plan)"}
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": per_plan, "unit": "s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(times)),
+        "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(ph, args), "cpu_baseline": cpu,
+        "e2e": {"value": per_plan, "unit": "s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def workload_config(ph, args):
+    return {"workload": f"{args.config}: {ph.name}, seed 0, {ph.n_beams} beams, V={ph.n_vox} voxels, N={ph.n_bl} beamlets, "
+                        f"nnz={ph.nnz}, {ph.n_rows} leaf rows, {N_APERTURES} apertures",
+            "parallelism": f"replicas x{args.gpus}" if args.gpus > 1 else "single GPU",
+            "l2": "inputs larger than L2 (D and D^T are 8*nnz bytes each; no flush needed)"}
+
+
+def pinned_phantom(ph, torch):
+    """Same phantom with its big arrays in pinned host memory (for the e2e leg)."""
+    import copy
+    q = copy.copy(ph)
+    keep = []
+    for name in ("row_ptr", "col_idx", "val", "vox_struct"):
+        t = torch.from_numpy(np.ascontiguousarray(getattr(ph, name))).pin_memory()
+        keep.append(t)
+        setattr(q, name, t.numpy())
+    q._pinned = keep
+    return q
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="cfg1")
+    ap.add_argument("--impl", default="dao", choices=["dao", "reference"])
+    ap.add_argument("--ref-apertures", type=int, default=3, help="apertures per step of the reference arm / cpu_baseline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1003_5402_b200 import build, dao
+    from paper_1003_5402_b200.inputs import phantom
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    build.build()
+    ph = phantom.make(args.config, 0)
+    peak, peak_src = load_peaks()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    d = dao.Dao(ph, k_max=N_APERTURES)
+    dims = d.dims()
+    infos = []
+    for _ in range(args.warmup):
+        d.reset()
+        d.run(N_APERTURES)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        d.reset()
+        infos.append(d.run(N_APERTURES))
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    elapsed = ev0.elapsed_time(ev1) * 1e-3
+    if world > 1:
+        t = torch.tensor([elapsed], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        elapsed = float(t.item())
+    sec_per_plan = elapsed / (args.steps * world)          # whole job: N replicas produce N plans per step
+    last = infos[-1]
+    n_it = sum(i.n_iterations for i in infos)
+
+    # ---- per-kernel-class device time (CUDA events on the launching stream, inside dao_run) ----
+    ab = algorithmic_bytes(ph)
+    classes = {"intensity": "seconds_intensity", "spmv": "seconds_spmv", "spmv_t": "seconds_spmv_t",
+               "price": "seconds_price", "column": "seconds_column", "master": "seconds_master"}
+    tot = {k: sum(getattr(i, f) for i in infos) for k, f in classes.items()}
+    tsum = sum(tot.values())
+    kernels = {}
+    for k in classes:
+        avg = tot[k] / max(1, n_it)
+        kernels[k] = {"avg_us": 1e6 * avg, "share": tot[k] / tsum if tsum > 0 else None}
+        if k in ab and avg > 0:
+            gbs = ab[k] / avg * 1e-9
+            kernels[k].update({"alg_bytes": ab[k], "GBps": gbs, "frac_of_hbm_peak": gbs / peak})
+    # master: bytes the projected-gradient loop must move: 2 passes over the dense block per iteration
+    pg_total = sum(i.n_pg_iter_total for i in infos)
+    hist = d.get_vector(dao.VEC_HISTORY)[:last.n_apertures]
+    master_bytes_plan = float(sum(int(h["n_pg_iter"]) * (2 * 4 * ph.n_vox * int(h["k"]) + 3 * 17 * ph.n_vox) for h in hist))
+    kernels["master"].update({"pg_iterations_per_plan": pg_total / args.steps, "alg_bytes_per_plan": master_bytes_plan,
+                              "GBps": master_bytes_plan * args.steps / tot["master"] * 1e-9 if tot["master"] > 0 else None,
+                              "note": "dense block A (4*V*K bytes <= L2) is L2-resident: GB/s is not an HBM figure"})
+    plan_bytes = N_APERTURES * (ab["spmv"] + ab["spmv_t"] + ab["price"] + ab["column"]) + master_bytes_plan
+    spmv = kernels["spmv"]
+    roofline = {"kernel": "k_spmv_sell (dose SpMV + fused objective/gradient)", "bound": "hbm",
+                "achieved": spmv.get("GBps"), "peak": peak, "unit": "GB/s", "frac": spmv.get("frac_of_hbm_peak"),
+                "traffic": None, "peak_source": peak_src, "alg_bytes_per_launch": ab["spmv"],
+                "avg_launch_us": spmv["avg_us"], "share_of_step": spmv["share"],
+                "dominant_by_time": max(kernels, key=lambda k: kernels[k]["share"] or 0),
+                "sell_padding": dims.sell_elems / max(1, ph.nnz)}
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(traffic_file):
+        try:
+            roofline["traffic"] = json.load(open(traffic_file)).get("k_spmv_sell")
+        except Exception:
+            pass
+
+    # ---- e2e: host (pinned) buffers -> dao_create -> dao_run -> dao_get_plan, wall clock ----
+    e2e = None
+    if args.e2e_steps > 0:
+        php = pinned_phantom(ph, torch)
+        h2d = int(php.row_ptr.nbytes + php.col_idx.nbytes + php.val.nbytes + php.vox_struct.nbytes)
+        d2h = 0
+        ts = []
+        for i in range(args.e2e_steps + 1):
+            barrier()
+            t0 = time.perf_counter()
+            with dao.Dao(php, k_max=N_APERTURES) as d2:
+                inf = d2.run(N_APERTURES)
+                plan = d2.get_plan()
+                d2h = int(plan.beams.nbytes + plan.intensity.nbytes + plan.ap_row_ptr.nbytes + plan.left.nbytes +
+                          plan.right.nbytes + (inf.n_iterations + 3) * 128)
+            torch.cuda.synchronize()
+            if i > 0:
+                ts.append(time.perf_counter() - t0)
+        e = float(np.mean(ts))
+        if world > 1:
+            t = torch.tensor([e], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e = float(t.item())
+        e2e = {"value": e / world, "unit": "s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "includes": "dao_create from pinned host CSR (H2D + sliced-ELL + transpose build), dao_run(50), dao_get_plan"}
+
+    # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0, N = 1 only ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import dao_oracle as orc
+        orc.build()
+        n_ap = args.ref_apertures
+        t0 = time.perf_counter()
+        orc.run(ph, n_ap)
+        dt = time.perf_counter() - t0
+        cpu = {"value": dt * N_APERTURES / n_ap, "unit": "s", "cores": 1, "kind": "oracle",
+               "sample": f"first {n_ap} of {N_APERTURES} column-generation iterations ({dt:.1f} s), scaled by {N_APERTURES}/{n_ap}; "
+                         "later iterations carry larger master problems, so the full plan takes longer"}
+
+    if rank == 0:
+        launches_per_plan = sum(i.n_iterations for i in infos) / args.steps * 10 + 2
+        out = {"metric": METRIC, "value": sec_per_plan, "unit": "s", "n_gpus": world, "steps": args.steps,
+               "warmup": args.warmup, "ms_per_step": 1e3 * elapsed / args.steps, "higher_is_better": False,
+               "scaling": "weak", "vs_baseline": None, "dtype": "f64", "storage_dtype": "f32/int32", "data": "synthetic",
+               "config": workload_config(ph, args), "clocks": clocks, "e2e": e2e,
+               "gpu_launches": int(launches_per_plan * args.steps), "roofline": roofline, "cpu_baseline": cpu,
+               "kernels": kernels,
+               "plan": {"objective": last.objective, "apertures": last.n_apertures, "cg_iterations_per_s": n_it / elapsed,
+                        "pg_iterations": int(last.n_pg_iter_total), "converged": int(last.converged),
+                        "bytes_moved_roofline_s": plan_bytes / (peak * 1e9),
+                        "frac_of_bytes_moved_roofline": plan_bytes / (peak * 1e9) / (elapsed / args.steps),
+                        "master_tol": d.opt.master_tol, "master_max_iter": d.opt.master_max_iter,
+                        "master_method": d.opt.master_method},
+               "paper_context": "0.7-2.5 s per 50-aperture plan on a Tesla C1060 for ~20x smaller clinical cases (PAPER.md:202)"}
+        print(json.dumps(out))
+    d.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

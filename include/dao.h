@@ -1,0 +1,265 @@
+/*
+ * dao.h -- C ABI of the B200-native hot path of column-generation direct aperture optimisation
+ * (DAO) after Men, Jia & Jiang, arXiv 1003.5402.  Citations are PAPER.md:<line> (+ equation).
+ *
+ * The library computes, entirely in hand-written CUDA kernels for sm_100a:
+ *   1. beamlet intensities   x_i = sum_{k : i in A_k} y_k                  PAPER.md:96-98 (eq. 7)
+ *   2. voxel dose            z_j = sum_i D_ij x_i                           PAPER.md:65    (eq. 1, 2)
+ *   3. objective + gradient  F(z), pi_j = dF/dz_j                           PAPER.md:75-83 (eq. 3-5),
+ *                                                                           :246-254 (eq. 9-10), :136
+ *   4. beamlet gradient      w_i = sum_j D_ij pi_j                          PAPER.md:138-140 (eq. 8)
+ *   5. row pricing           per MLC leaf row the contiguous interval with the most negative sum
+ *                            of w (ties: smallest left leaf, then smallest right leaf)
+ *                                                                           PAPER.md:140-167
+ *   6. beam selection        price_b = sum of the row minima of beam b; b* = argmin_b (ties: smallest b)
+ *                                                                           PAPER.md:169
+ *   7. aperture dose column  a_K = sum_{i in A_K} D_i.                      PAPER.md:69 (eq. 2)
+ *   8. restricted master     min_{y >= 0} F(A y) by gradient projection
+ *   9. the column-generation loop over 1-8
+ *
+ * Conventions
+ *   - D is passed voxel-major: row j = voxel, column i = beamlet (the paper writes D_ij with i the
+ *     beamlet).  Values fp32, indices int32.
+ *   - Beamlets are numbered beam-major, then MLC leaf row, then left to right, so each leaf row
+ *     is a contiguous range of beamlet ids [row_bl_ptr[r], row_bl_ptr[r+1]).
+ *   - Leaf positions are 0-based half-open [left, right) column offsets inside the leaf row: the
+ *     open beamlets of row r are row_bl_ptr[r]+left .. row_bl_ptr[r]+right-1.  In the paper's
+ *     1-based notation left = l*, right = r* - 1 (open beamlets l*+1 .. r*-1, PAPER.md:140,
+ *     156-165).  A closed row is (0, 0) (the paper's initial (l*, r*) = (0, 1)).
+ *   - Every function returns a dao_status; nothing throws, aborts or prints.  Functions that
+ *     return host scalars synchronise the context's stream once, at their end; dao_run
+ *     synchronises once per column-generation iteration.
+ *   - The library never allocates device memory: the caller (PyTorch in the Python binding)
+ *     provides one persistent workspace and one create-time scratch buffer whose sizes
+ *     dao_workspace_bytes reports, and the CUDA stream all work is issued on.
+ *   - Inputs are only read during dao_workspace_bytes / dao_create; nothing of the caller's is
+ *     referenced afterwards.  Pointers flagged DAO_MEM_DEVICE must be device pointers valid on
+ *     the current device; DAO_MEM_HOST pointers are ordinary host memory (pinned or pageable).
+ *   - A context is not thread-safe and is bound to the stream given at creation.
+ *   - There is no CPU fallback: without a CUDA device every call that needs one fails with
+ *     DAO_E_CUDA.
+ */
+#ifndef DAO_H_
+#define DAO_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dao_ctx dao_ctx;   /* opaque; one per plan */
+
+typedef enum {
+  DAO_OK = 0,
+  DAO_E_ARG = 1,          /* null pointer, negative size, non-finite / negative value, bad option */
+  DAO_E_SHAPE = 2,        /* inconsistent sizes, non-monotone pointers, index out of range, capacity too small */
+  DAO_E_CUDA = 3,         /* a CUDA call failed; text in dao_last_error */
+  DAO_E_ALLOC = 4,        /* workspace / scratch too small or misaligned */
+  DAO_E_STATE = 5,        /* call not valid in the context's current state */
+  DAO_E_UNSUPPORTED = 6   /* nnz >= 2^31, more than 255 structures, more than DAO_MAX_APERTURES apertures */
+} dao_status;
+
+typedef enum { DAO_MEM_HOST = 0, DAO_MEM_DEVICE = 1 } dao_memspace;
+
+#define DAO_MAX_APERTURES 128      /* upper bound on dao_options.k_max */
+
+/* The beamlet dose-deposition matrix D_ij, CSR, rows = voxels, columns = beamlets. */
+typedef struct {
+  int32_t n_vox, n_bl;
+  int64_t nnz;               /* < 2^31 */
+  const int32_t *row_ptr;    /* [n_vox+1], row_ptr[0] = 0, non-decreasing, row_ptr[n_vox] = nnz */
+  const int32_t *col_idx;    /* [nnz], strictly ascending inside a row, in [0, n_bl) */
+  const float *val;          /* [nnz], finite, >= 0 */
+  dao_memspace mem;          /* where the three arrays live */
+} dao_csr;
+
+/* MLC geometry: which beamlets form a leaf row, which leaf rows form a beam. */
+typedef struct {
+  int32_t n_beams, n_rows;
+  const int32_t *beam_row_ptr;   /* [n_beams+1] host, into leaf rows; beam_row_ptr[n_beams] = n_rows */
+  const int32_t *row_bl_ptr;     /* [n_rows+1]  host, into beamlets;  row_bl_ptr[n_rows] = n_bl */
+} dao_mlc;
+
+/* Structures, thresholds and weights of eq. (9)-(10).  One structure per voxel. */
+typedef struct {
+  int32_t n_struct;              /* <= 255 */
+  const int32_t *vox_struct;     /* [n_vox] structure id in [0, n_struct) or -1 (no penalty); same memspace as D */
+  const float *t_under;          /* [n_struct] host: T_s^-  (under-dose threshold) */
+  const float *w_under;          /* [n_struct] host: alpha_s (0 for non-targets) */
+  const float *t_over;           /* [n_struct] host: T_s^+  (over-dose threshold) */
+  const float *w_over;           /* [n_struct] host: beta_s */
+} dao_structs;
+
+/* Options.  Zero-initialise, then dao_default_options, then override. */
+typedef struct {
+  int32_t k_max;             /* capacity of the aperture pool, 1..DAO_MAX_APERTURES (default 50) */
+  int32_t master_max_iter;   /* cap on projected-gradient iterations per master solve (default 2000) */
+  double master_tol;         /* stop when max_k |p_k| * max(1, max_k y_k) <= master_tol * F, p = projected
+                                steepest-descent direction (default 1e-7); reading S2 */
+  double price_tol;          /* optimal iff price_b* >= -price_tol * max_i |w_i| * (rows in b*) (default 1e-6, the
+                                fp32 noise floor of w), or iff the best candidate duplicates an aperture of the
+                                pool (its negative price is then residue of the master solve); S3, S6 */
+  int32_t master_method;     /* 0 = plain gradient projection, 1 = gradient projection with conjugate
+                                (Polak-Ribiere+) directions on the free face (default 1) */
+  int32_t sell_sigma;        /* sorting window (rows) of the internal sliced-ELL layout of D; 1 = keep the
+                                caller's voxel order; 0 = library default */
+  int32_t timers;            /* non-zero: CUDA-event timers per kernel class in dao_run (default 1) */
+  int32_t reserved;
+} dao_options;
+
+typedef struct {
+  size_t workspace_bytes;    /* persistent device memory, lives as long as the context */
+  size_t scratch_bytes;      /* device memory needed only during dao_create */
+} dao_sizes;
+
+typedef struct {
+  int32_t beam;              /* b*: beam of the candidate aperture */
+  int32_t converged;         /* 1: no improving aperture exists, no candidate stored */
+  double price;              /* reduced cost of the candidate = price_b* (< 0 when it improves) */
+  double objective;          /* F(z) at the current intensities */
+  double w_abs_max;          /* max_i |w_i| (used by the optimality test) */
+  int32_t n_open_beamlets;   /* beamlets opened by the candidate */
+  int32_t duplicate;         /* 1: the candidate equals an aperture already in the pool (reading S6) */
+} dao_price_info;
+
+typedef struct {
+  int32_t n_apertures;       /* pool size after the call */
+  int32_t n_pg_iter;         /* projected-gradient iterations taken */
+  int32_t hit_max_iter;      /* 1: stopped by master_max_iter */
+  int32_t n_restarts;        /* conjugate-direction restarts (method 1) */
+  double objective;          /* F(A y) at return */
+  double kkt_residual;       /* max_k of |grad_k| where y_k > 0 and max(0, -grad_k) where y_k = 0 */
+  double pg_norm;            /* max_k |p_k| at return */
+} dao_master_info;
+
+typedef struct {
+  int32_t n_apertures;
+  int32_t n_iterations;      /* column-generation iterations executed by this call */
+  int32_t converged;         /* 1: stopped because pricing found no improving aperture */
+  int32_t n_duplicates;      /* iterations whose candidate was already in the pool (S6) */
+  int64_t n_pg_iter_total;
+  double objective;          /* F of the final plan, from the dose SpMV z = D x */
+  double seconds_total;      /* device time of the call (CUDA events) */
+  /* per kernel class, summed over iterations; zero when options.timers == 0 */
+  double seconds_intensity, seconds_spmv, seconds_spmv_t, seconds_price, seconds_column, seconds_master;
+} dao_run_info;
+
+/* One record per column-generation iteration, retrievable after dao_run / dao_solve_master. */
+typedef struct {
+  int32_t k;                 /* pool size after the iteration */
+  int32_t beam;
+  int32_t n_pg_iter;
+  int32_t duplicate;
+  double price;
+  double objective_before;   /* F before the aperture was added (at pricing time) */
+  double objective;          /* F(A y) after the master solve */
+  double kkt_residual;
+} dao_iter_record;
+
+typedef struct {
+  int32_t cap_apertures, cap_rows;   /* in: capacities of the arrays below */
+  int32_t n_apertures, n_rows_used;  /* out (also set when the capacity is too small -> DAO_E_SHAPE) */
+  int32_t *beam;                     /* [cap_apertures] host */
+  float *intensity;                  /* [cap_apertures] host, y_k */
+  int32_t *ap_row_ptr;               /* [cap_apertures+1] host, into left/right (the rows of that beam, in order) */
+  int32_t *left, *right;             /* [cap_rows] host, half-open leaf positions */
+  double objective;                  /* F of the plan */
+} dao_plan;
+
+typedef enum {               /* dao_get_vector selectors; lengths in elements */
+  DAO_VEC_Z = 0,             /* float  [n_vox]  dose of the last evaluation, caller's voxel order */
+  DAO_VEC_G = 1,             /* float  [n_vox]  pi_j = dF/dz_j */
+  DAO_VEC_W = 2,             /* float  [n_bl]   beamlet gradient */
+  DAO_VEC_X = 3,             /* float  [n_bl]   beamlet intensities */
+  DAO_VEC_Y = 4,             /* double [k_max]  aperture intensities (first n_apertures valid) */
+  DAO_VEC_VSTAR = 5,         /* double [n_rows] row minima of the last pricing */
+  DAO_VEC_LEFT = 6,          /* int32  [n_rows] */
+  DAO_VEC_RIGHT = 7,         /* int32  [n_rows] */
+  DAO_VEC_BEAM_PRICE = 8,    /* double [n_beams] */
+  DAO_VEC_HISTORY = 9,       /* dao_iter_record [k_max] (first n_apertures valid) */
+  DAO_VEC_MASTER_Z = 10      /* double [n_vox]  z = A y as the master holds it, caller's voxel order */
+} dao_vector;
+
+void dao_default_options(dao_options *opt);
+
+/* Sizes of the two device buffers dao_create needs for this problem.  Reads D->row_ptr. */
+dao_status dao_workspace_bytes(const dao_csr *D, const dao_mlc *mlc, const dao_structs *s,
+                               const dao_options *opt, dao_sizes *out);
+
+/* Validate the inputs, copy them to the device, build the internal layouts (sliced-ELL of D, CSR
+ * of D^T, pricing tables, per-structure penalty table) inside `workspace`, and start with an empty
+ * aperture pool (z = 0).  Both buffers must be 256-byte aligned device memory of at least the
+ * sizes dao_workspace_bytes reported; `scratch` may be released when the call returns.
+ * cuda_stream is a cudaStream_t (NULL = legacy default stream).  On failure *out = NULL and the
+ * message is available from dao_last_error(NULL). */
+dao_status dao_create(const dao_csr *D, const dao_mlc *mlc, const dao_structs *s, const dao_options *opt,
+                      void *workspace, size_t workspace_bytes, void *scratch, size_t scratch_bytes,
+                      void *cuda_stream, dao_ctx **out);
+
+/* Steps 1-6 at the current intensities.  Stores the candidate aperture; the pool is unchanged. */
+dao_status dao_price(dao_ctx *ctx, dao_price_info *out);
+
+/* Steps 7-8: append the pending candidate (DAO_E_STATE if there is none or the pool is full), then
+ * solve the restricted master problem over the pool on the device. */
+dao_status dao_solve_master(dao_ctx *ctx, dao_master_info *out);
+
+/* Step 9: repeat price -> add -> master until the pool holds max_apertures apertures or pricing
+ * proves optimality.  One host synchronisation per iteration.  Ends with a final dose evaluation
+ * (steps 1-3) so that DAO_VEC_Z / objective describe the returned plan. */
+dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out);
+
+/* Copy the plan into caller-allocated host arrays. */
+dao_status dao_get_plan(dao_ctx *ctx, dao_plan *out);
+
+/* Empty the pool (y, z back to the state after dao_create); keeps the matrix layouts. */
+dao_status dao_reset(dao_ctx *ctx);
+
+dao_status dao_destroy(dao_ctx *ctx);
+
+/* Message of the last failure of this context (ctx = NULL: of the last failed dao_create /
+ * dao_workspace_bytes on this thread).  Owned by the library, valid until the next call. */
+const char *dao_last_error(const dao_ctx *ctx);
+
+/* ---- test / bench hooks (parity harness, BASELINE.json configs[3] kernel sweep) ---------------- */
+
+/* Copy an internal vector to `dst` (host or device memory, see dao_vector for type and length). */
+dao_status dao_get_vector(dao_ctx *ctx, int32_t which, void *dst, dao_memspace mem);
+
+/* Problem dimensions and layout facts. */
+typedef struct {
+  int32_t n_vox, n_bl, n_beams, n_rows, n_struct, k_max;
+  int64_t nnz;               /* of D as given */
+  int64_t sell_elems;        /* stored elements of the sliced-ELL copy (>= nnz: padding) */
+  int32_t sell_slice_rows, sell_sigma;
+  int32_t n_sm, reserved;
+} dao_dims;
+dao_status dao_get_dims(const dao_ctx *ctx, dao_dims *out);
+
+/* Isolated kernels on caller-provided DEVICE vectors in the caller's voxel / beamlet order.
+ * Asynchronous on the context's stream (no synchronisation). */
+dao_status dao_spmv(dao_ctx *ctx, const float *x_dev, float *z_dev);        /* z = D x        [n_bl] -> [n_vox] */
+dao_status dao_spmv_t(dao_ctx *ctx, const float *g_dev, float *w_dev);      /* w = D^T g      [n_vox] -> [n_bl] */
+/* Dose + objective + gradient for given beamlet intensities: steps 2-3.  Synchronises. */
+dao_status dao_eval_x(dao_ctx *ctx, const float *x_dev, double *objective);
+/* Steps 5-6 on a caller-provided fp32 beamlet-gradient vector (DEVICE, [n_bl]) and caller-provided
+ * MLC tables (DEVICE, n_rows+1 / n_beams+1 entries; pass NULL, NULL, 0, 0 to use the context's).
+ * Outputs are DEVICE arrays: left/right int32 [n_rows], vstar double [n_rows], beam_price double
+ * [n_beams], best int32 [1].  Asynchronous. */
+dao_status dao_price_from_w(dao_ctx *ctx, const float *w_dev, const int32_t *row_bl_ptr_dev,
+                            const int32_t *beam_row_ptr_dev, int32_t n_rows, int32_t n_beams,
+                            int32_t *left_dev, int32_t *right_dev, double *vstar_dev,
+                            double *beam_price_dev, int32_t *best_dev);
+/* Load a pool of apertures (host arrays laid out as in dao_plan) with intensities y (host, may be
+ * NULL = zeros) replacing the current pool: builds the dose columns (step 7) but does not solve.
+ * Lets the parity harness solve the master on the oracle's pool. */
+dao_status dao_set_pool(dao_ctx *ctx, int32_t n_apertures, const int32_t *beam, const int32_t *ap_row_ptr,
+                        const int32_t *left, const int32_t *right, const double *y);
+/* Solve the restricted master over the current pool without adding a column. */
+dao_status dao_resolve_master(dao_ctx *ctx, dao_master_info *out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DAO_H_ */

@@ -1,0 +1,192 @@
+// dao_internal.cuh -- shared declarations of the CUDA library behind include/dao.h.
+// Nothing here is shared with oracle/ (the fp64 CPU oracle is independent test infrastructure).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "dao.h"
+
+namespace dao {
+
+// ------------------------------------------------------------------------------------------
+// Tunables (compile time)
+// ------------------------------------------------------------------------------------------
+constexpr int kSellC = 8;              // rows per sliced-ELL slice (quarter warp); 32/kSellC slices per warp
+constexpr int kSpmvThreads = 512;      // CTA size of the SELL SpMV kernel
+constexpr int kSpmvXSmemMax = 24576;   // x is staged in shared memory when n_bl <= this (96 KB fp32)
+constexpr int kTChunk = 4096;          // elements of D^T per CTA in the transposed SpMV
+constexpr int kTThreads = 256;
+constexpr int kMasterThreads = 512;    // CTA size of the persistent master kernel (one CTA per SM)
+constexpr int kMasterTile = 2048;      // voxels of g staged in shared memory per tile in the master
+constexpr int kMaxStruct = 255;
+constexpr int kNoStruct = 255;         // sid value of a voxel without penalty
+constexpr int kMaxRedux = DAO_MAX_APERTURES + 8;   // doubles per grid reduction in the master
+
+// ------------------------------------------------------------------------------------------
+// Device-resident state shared by the kernels of one context (one instance in global memory).
+// The host reads it once per column-generation iteration.
+// ------------------------------------------------------------------------------------------
+struct DevState {
+  // pool
+  int32_t K;               // apertures in the pool
+  int32_t done;            // 1: pricing proved optimality
+  // pending candidate (result of the last pricing)
+  int32_t cand_valid;
+  int32_t cand_beam;
+  int32_t cand_dup;
+  int32_t cand_nopen;
+  double cand_price;
+  double w_abs_max;
+  // last dose evaluation
+  double F;
+  // last master solve
+  int32_t m_iters;
+  int32_t m_hit_max;
+  int32_t m_restarts;
+  int32_t m_added;         // 1: the master appended the candidate
+  double m_F;
+  double m_kkt;
+  double m_pg;
+  // counters used by last-block reductions (self-resetting)
+  uint32_t ticket_spmv;
+  uint32_t ticket_misc;
+  // grid barrier of the master kernel
+  uint32_t bar_count;
+  uint32_t bar_gen;
+  int64_t pg_iter_total;
+  int32_t n_duplicates;
+  int32_t pad_;
+};
+
+struct StructEntry {       // per-structure penalty parameters of eq. (9)-(10), already divided by |v_s|
+  double a;                // alpha_s / |v_s|
+  double b;                // beta_s  / |v_s|
+  double tm;               // T_s^-
+  double tp;               // T_s^+
+};
+
+// All device pointers of a context.  Voxel-space arrays are in the INTERNAL voxel order
+// (internal row i holds the caller's voxel perm[i]).
+struct DevPtrs {
+  // sliced ELL of D
+  int32_t *sell_col;
+  float *sell_val;
+  uint32_t *slice_off;     // [n_slices+1] element offsets
+  int32_t *perm;           // [n_vox_pad] internal -> caller voxel (-1 for padding rows)
+  int32_t *inv_perm;       // [n_vox]     caller voxel -> internal
+  uint8_t *sid;            // [n_vox_pad] structure id or kNoStruct
+  StructEntry *stab;       // [256]
+  // CSR of D^T (rows = beamlets, entries = internal voxel ids)
+  int32_t *t_ptr;          // [n_bl+1]
+  int32_t *t_row;          // [nnz padded to kTChunk]
+  float *t_val;
+  int32_t *t_first_row;    // [n_tchunks]
+  int32_t *t_seg_base;     // [n_tchunks+1]
+  double *t_segsum;        // [n_tsegs]
+  // MLC tables
+  int32_t *beam_row_ptr;   // [n_beams+1]
+  int32_t *row_bl_ptr;     // [n_rows+1]
+  int32_t *bl_row;         // [n_bl]
+  int32_t *row_beam;       // [n_rows]
+  // vectors
+  float *x;                // [n_bl]
+  float *xmask;            // [n_bl]
+  float *z;                // [n_vox_pad]
+  float *g;                // [n_vox_pad]
+  float *w;                // [n_bl]
+  double *f_part;          // [grid of the spmv kernel]
+  // pricing
+  double *vstar;           // [n_rows]
+  int32_t *left, *right;   // [n_rows]
+  double *row_absmax;      // [n_rows]
+  double *beam_price;      // [n_beams]
+  double *beam_absmax;     // [n_beams]
+  // pool
+  int32_t *ap_beam;        // [k_max]
+  int32_t *ap_left;        // [k_max * max_rows_per_beam]
+  int32_t *ap_right;
+  float *A;                // [k_max][n_vox_pad] aperture-major dose block
+  double *y;               // [k_max]
+  // master
+  double *mz;              // [n_vox_pad] z = A y
+  double *mdz;             // [n_vox_pad] dz = A p
+  double *m_part;          // [2][n_cta][kMaxRedux] partials of the grid reductions
+  double *m_result;        // [2][kMaxRedux]
+  // history
+  dao_iter_record *history;  // [k_max]
+  DevState *state;
+  void *io_scratch;        // small staging buffer for get_vector / hooks ([max(n_vox_pad,n_bl)] 8-byte)
+};
+
+struct Ctx {
+  // problem
+  int32_t n_vox = 0, n_bl = 0, n_beams = 0, n_rows = 0, n_struct = 0;
+  int64_t nnz = 0;
+  int32_t n_vox_pad = 0;        // n_vox rounded up to a multiple of 128
+  int32_t max_rows_per_beam = 0;
+  int32_t n_slices = 0;
+  int64_t sell_elems = 0;
+  int32_t n_tchunks = 0, n_tsegs = 0;
+  dao_options opt{};
+  // host copies of small tables
+  std::vector<int32_t> beam_row_ptr, row_bl_ptr;
+  // device
+  DevPtrs d{};
+  cudaStream_t stream = nullptr;
+  int device = 0, n_sm = 0;
+  int spmv_grid = 0, master_grid = 0;
+  size_t master_smem = 0;
+  bool x_in_smem = true;
+  // host mirror (pinned) of DevState for the once-per-iteration read-back
+  DevState *h_state = nullptr;
+  // host bookkeeping
+  int32_t K = 0;                // pool size as last seen by the host
+  bool have_candidate = false;
+  double objective = 0.0;
+  cudaEvent_t ev[8] = {};
+  std::string err;
+};
+
+// ------------------------------------------------------------------------------------------
+// helpers
+// ------------------------------------------------------------------------------------------
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+#define DAO_CUDA_OK(ctx, call)                                                            \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess) {                                                              \
+      (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e_);                    \
+      return DAO_E_CUDA;                                                                  \
+    }                                                                                     \
+  } while (0)
+
+// kernels / launchers implemented in the .cu files --------------------------------------------
+// dao_setup.cu
+struct HostLayout;   // SELL slice table and permutation computed on the host from row_ptr
+dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_structs *s, void *workspace,
+                       size_t workspace_bytes, void *scratch, size_t scratch_bytes);
+dao_status setup_sizes(const dao_csr *D, const dao_mlc *mlc, const dao_structs *s, const dao_options *opt,
+                       dao_sizes *out, std::string *err);
+
+// dao_spmv.cu
+enum SpmvMode { kSpmvObjective = 0, kSpmvPlain = 1, kSpmvColumn = 2, kSpmvPlainUserOrder = 3 };
+cudaError_t launch_spmv(Ctx *c, SpmvMode mode, const float *x, float *out);
+cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out);
+cudaError_t launch_intensity(Ctx *c);
+
+// dao_pricing.cu
+cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, const int32_t *beam_row_ptr,
+                           int32_t n_rows, int32_t n_beams, int32_t *left, int32_t *right, double *vstar,
+                           double *row_absmax, double *beam_price, double *beam_absmax, int32_t *best_out,
+                           bool update_state);
+cudaError_t launch_append_candidate(Ctx *c);
+
+// dao_master.cu
+cudaError_t master_configure(Ctx *c);
+cudaError_t launch_master(Ctx *c, bool add_candidate);
+
+}  // namespace dao

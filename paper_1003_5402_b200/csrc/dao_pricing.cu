@@ -1,0 +1,263 @@
+// dao_pricing.cu -- the pricing sub-problem, PAPER.md:136-169 (eq. 8):
+//   step 5  per MLC leaf row the contiguous interval with the most negative sum of w
+//   step 6  per-beam sum of the row minima, beam with the smallest sum, optimality test,
+//           and the bookkeeping that turns the winner into the pending candidate aperture.
+#include "dao_internal.cuh"
+
+#include <math_constants.h>
+
+namespace dao {
+
+// ------------------------------------------------------------------------------------------
+// step 5.  One warp per leaf row.  With S_0 = 0 and S_r = w_1 + .. + w_r (fp64 sums of the fp32
+// inputs) the printed scan returns
+//     v* = min_r ( S_r - max_{0<=l<=r} S_l ),   l = first index attaining the prefix maximum,
+// taking the first r that attains the minimum; the closed row wins every tie at 0.  This equals
+// the lexicographically smallest (value, l, r) over all intervals (reading S4).
+// The warp does an inclusive sum scan, an inclusive (max, first-argmax) scan and an argmin
+// reduction per tile of 32 beamlets, carrying (S, max, argmax, best) between tiles.
+// Output in the ABI convention: half-open [left, right) = [l, r), closed row = (0, 0).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_price_rows(const float *__restrict__ w,
+                                                    const int32_t *__restrict__ row_bl_ptr, int32_t n_rows,
+                                                    double *__restrict__ vstar, int32_t *__restrict__ left,
+                                                    int32_t *__restrict__ right,
+                                                    double *__restrict__ row_absmax) {
+  const int lane = threadIdx.x & 31;
+  const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (row >= n_rows) return;
+  const int32_t b0 = row_bl_ptr[row];
+  const int32_t n = row_bl_ptr[row + 1] - b0;
+  const unsigned FULL = 0xffffffffu;
+
+  double carry = 0.0;                  // S at the end of the previous tile
+  double run_max = 0.0;                // max_{0<=l<=r} S_l so far (S_0 = 0 at l = 0)
+  int32_t run_arg = 0;
+  double best = 0.0;                   // v*
+  int32_t best_l = 0, best_r = 0;      // closed
+  double amax = 0.0;
+
+  for (int32_t base = 0; base < n; base += 32) {
+    const int32_t idx = base + lane;
+    const bool valid = idx < n;
+    const double wv = valid ? (double)w[b0 + idx] : 0.0;
+    amax = fmax(amax, fabs(wv));
+    // inclusive prefix sum
+    double s = wv;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const double t = __shfl_up_sync(FULL, s, o);
+      if (lane >= o) s += t;
+    }
+    const double P = carry + s;        // S_r with r = idx + 1
+    // inclusive prefix (max, first argmax)
+    double mv = valid ? P : -CUDART_INF;
+    int32_t mi = idx + 1;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const double tv = __shfl_up_sync(FULL, mv, o);
+      const int32_t ti = __shfl_up_sync(FULL, mi, o);
+      if (lane >= o && tv >= mv) { mv = tv; mi = ti; }   // ties keep the smaller index
+    }
+    if (run_max >= mv) { mv = run_max; mi = run_arg; }
+    // candidate of this r: value, l, r
+    double cv = valid ? (P - mv) : 0.0;
+    int32_t cl = mi, cr = idx + 1;
+    if (!(cv < 0.0)) { cv = 0.0; cl = 0; cr = 0; }        // never open a non-improving interval
+    // lexicographic argmin over the tile
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const double ov = __shfl_xor_sync(FULL, cv, o);
+      const int32_t ol = __shfl_xor_sync(FULL, cl, o);
+      const int32_t orr = __shfl_xor_sync(FULL, cr, o);
+      const bool take = (ov < cv) || (ov == cv && (ol < cl || (ol == cl && orr < cr)));
+      if (take) { cv = ov; cl = ol; cr = orr; }
+    }
+    if ((cv < best) || (cv == best && cv < 0.0 && (cl < best_l || (cl == best_l && cr < best_r)))) {
+      best = cv; best_l = cl; best_r = cr;
+    }
+    carry += __shfl_sync(FULL, s, 31);
+    run_max = __shfl_sync(FULL, mv, 31);
+    run_arg = __shfl_sync(FULL, mi, 31);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(FULL, amax, o));
+  if (lane == 0) {
+    vstar[row] = best;
+    left[row] = best_l;
+    right[row] = best_r;
+    row_absmax[row] = amax;
+  }
+}
+
+// step 6a: price_b = sum over the rows of beam b of v* (PAPER.md:169).  One warp per beam,
+// lane-strided partial sums in row order, then a fixed shuffle tree.
+__global__ void __launch_bounds__(256) k_price_beams(const double *__restrict__ vstar,
+                                                     const double *__restrict__ row_absmax,
+                                                     const int32_t *__restrict__ beam_row_ptr, int32_t n_beams,
+                                                     double *__restrict__ beam_price,
+                                                     double *__restrict__ beam_absmax) {
+  const int lane = threadIdx.x & 31;
+  const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (b >= n_beams) return;
+  double s = 0.0, a = 0.0;
+  for (int32_t r = beam_row_ptr[b] + lane; r < beam_row_ptr[b + 1]; r += 32) {
+    s += vstar[r];
+    a = fmax(a, row_absmax[r]);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    s += __shfl_xor_sync(0xffffffffu, s, o);
+    a = fmax(a, __shfl_xor_sync(0xffffffffu, a, o));
+  }
+  if (lane == 0) {
+    beam_price[b] = s;
+    beam_absmax[b] = a;
+  }
+}
+
+// step 6b: b* = argmin_b price_b (ties: smallest b), optimality test (reading S3), candidate
+// bookkeeping.  One CTA.
+__global__ void __launch_bounds__(256) k_price_select(const double *__restrict__ beam_price,
+                                                      const double *__restrict__ beam_absmax, int32_t n_beams,
+                                                      const int32_t *__restrict__ beam_row_ptr,
+                                                      const int32_t *__restrict__ left,
+                                                      const int32_t *__restrict__ right, int32_t *best_out,
+                                                      DevState *st, double price_tol, int32_t k_max,
+                                                      int32_t max_rows, const int32_t *__restrict__ ap_beam,
+                                                      const int32_t *__restrict__ ap_left,
+                                                      const int32_t *__restrict__ ap_right) {
+  __shared__ double sv[256];
+  __shared__ int32_t sb[256];
+  __shared__ double sa[256];
+  __shared__ int32_t s_cnt[256];
+  const int t = threadIdx.x;
+  double bv = CUDART_INF, am = 0.0;
+  int32_t bb = 0x7fffffff;
+  for (int32_t b = t; b < n_beams; b += 256) {
+    const double v = beam_price[b];
+    if (v < bv) { bv = v; bb = b; }     // ascending b within a thread: ties keep the smaller b
+    am = fmax(am, beam_absmax[b]);
+  }
+  sv[t] = bv; sb[t] = bb; sa[t] = am;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (t < o) {
+      const double ov = sv[t + o];
+      const int32_t ob = sb[t + o];
+      if (ov < sv[t] || (ov == sv[t] && ob < sb[t])) { sv[t] = ov; sb[t] = ob; }
+      sa[t] = fmax(sa[t], sa[t + o]);
+    }
+    __syncthreads();
+  }
+  const int32_t best = sb[0];
+  const double price = sv[0];
+  const double absmax = sa[0];
+  if (best_out != nullptr && t == 0) *best_out = best;
+  if (st == nullptr) return;
+  // candidate bookkeeping
+  const int32_t r0 = beam_row_ptr[best], r1 = beam_row_ptr[best + 1];
+  int32_t cnt = 0;
+  for (int32_t r = r0 + t; r < r1; r += 256) cnt += right[r] - left[r];
+  s_cnt[t] = cnt;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (t < o) s_cnt[t] += s_cnt[t + o];
+    __syncthreads();
+  }
+  // duplicate of an aperture already in the pool? (reading S6: counted, still accepted)
+  __shared__ int32_t s_dup;
+  if (t == 0) s_dup = 0;
+  __syncthreads();
+  const int32_t K = st->K;
+  for (int32_t k = 0; k < K; ++k) {
+    if (ap_beam[k] != best) continue;
+    int32_t diff = 0;
+    for (int32_t r = r0 + t; r < r1; r += 256) {
+      const int32_t m = r - r0;
+      diff |= (ap_left[k * max_rows + m] != left[r]) | (ap_right[k * max_rows + m] != right[r]);
+    }
+    const int any = __syncthreads_or(diff);
+    if (!any && t == 0) s_dup = 1;
+  }
+  __syncthreads();
+  if (t == 0) {
+    // Optimal iff no aperture has a negative reduced cost.  Numerically (readings
+    // S3, S6): the price must be below -price_tol * max|w| * rows, and a candidate identical to a
+    // pool aperture is numerical residue of the master solve (its exact reduced cost is >= 0 and
+    // it is the minimiser), so it also ends the column generation.
+    const bool converged = !(price < -price_tol * absmax * (double)(r1 - r0)) || (s_dup != 0);
+    if (s_dup) st->n_duplicates += 1;
+    st->cand_beam = best;
+    st->cand_price = price;
+    st->w_abs_max = absmax;
+    st->cand_nopen = s_cnt[0];
+    st->cand_dup = s_dup;
+    st->done = converged ? 1 : 0;
+    st->cand_valid = (!converged && K < k_max) ? 1 : 0;
+  }
+}
+
+cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, const int32_t *beam_row_ptr,
+                           int32_t n_rows, int32_t n_beams, int32_t *left, int32_t *right, double *vstar,
+                           double *row_absmax, double *beam_price, double *beam_absmax, int32_t *best_out,
+                           bool update_state) {
+  const int wpb = 8;
+  if (n_rows > 0) {
+    k_price_rows<<<(n_rows + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(w, row_bl_ptr, n_rows, vstar, left,
+                                                                      right, row_absmax);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  k_price_beams<<<(n_beams + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(vstar, row_absmax, beam_row_ptr, n_beams,
+                                                                       beam_price, beam_absmax);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  k_price_select<<<1, 256, 0, c->stream>>>(beam_price, beam_absmax, n_beams, beam_row_ptr, left, right, best_out,
+                                           update_state ? c->d.state : nullptr, c->opt.price_tol, c->opt.k_max,
+                                           c->max_rows_per_beam, c->d.ap_beam, c->d.ap_left, c->d.ap_right);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// Append the pending candidate to the pool tables at index K and write its 0/1 beamlet mask
+// (the x of step 7, a_K = D 1_A).  The pool size itself is advanced by the master kernel.
+// ------------------------------------------------------------------------------------------
+__global__ void k_append_candidate(const DevState *__restrict__ st, int32_t n_bl, int32_t max_rows,
+                                   const int32_t *__restrict__ bl_row, const int32_t *__restrict__ row_beam,
+                                   const int32_t *__restrict__ beam_row_ptr,
+                                   const int32_t *__restrict__ row_bl_ptr, const int32_t *__restrict__ left,
+                                   const int32_t *__restrict__ right, int32_t *__restrict__ ap_beam,
+                                   int32_t *__restrict__ ap_left, int32_t *__restrict__ ap_right,
+                                   float *__restrict__ xmask) {
+  if (!st->cand_valid) return;
+  const int32_t K = st->K, b = st->cand_beam;
+  const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n_bl) {
+    const int32_t r = bl_row[i];
+    float m = 0.f;
+    if (row_beam[r] == b) {
+      const int32_t c = i - row_bl_ptr[r];
+      m = (c >= left[r] && c < right[r]) ? 1.f : 0.f;
+    }
+    xmask[i] = m;
+  }
+  const int32_t r0 = beam_row_ptr[b], nr = beam_row_ptr[b + 1] - r0;
+  if (i == 0) ap_beam[K] = b;
+  if (i < max_rows) {
+    ap_left[K * max_rows + i] = i < nr ? left[r0 + i] : 0;
+    ap_right[K * max_rows + i] = i < nr ? right[r0 + i] : 0;
+  }
+}
+
+cudaError_t launch_append_candidate(Ctx *c) {
+  const int t = 128;
+  const int n = c->n_bl > c->max_rows_per_beam ? c->n_bl : c->max_rows_per_beam;
+  k_append_candidate<<<(n + t - 1) / t, t, 0, c->stream>>>(c->d.state, c->n_bl, c->max_rows_per_beam, c->d.bl_row,
+                                                           c->d.row_beam, c->d.beam_row_ptr, c->d.row_bl_ptr,
+                                                           c->d.left, c->d.right, c->d.ap_beam, c->d.ap_left,
+                                                           c->d.ap_right, c->d.xmask);
+  return cudaGetLastError();
+}
+
+}  // namespace dao
