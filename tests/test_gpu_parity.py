@@ -201,7 +201,7 @@ def test_master_on_oracle_pool(D, mini):
     assert m.n_apertures == 15 and not m.hit_max_iter
     assert abs(m.objective - plan.objective) <= 1e-5 * plan.objective
     f_chk, grad = orc.master_gradient(plan.A, y, vp)          # KKT of the GPU's y in the oracle's arithmetic
-    assert abs(f_chk - m.objective) <= 1e-9 * f_chk
+    assert abs(f_chk - m.objective) <= 1e-6 * f_chk      # A is stored in fp32 on the GPU
     assert (grad >= -1e-5 * max(1.0, f_chk)).all()
     assert (np.abs(grad[y > 0]) <= 1e-5 * max(1.0, f_chk)).all()
 
