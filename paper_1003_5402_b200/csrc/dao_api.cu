@@ -39,14 +39,6 @@ __global__ void k_to_user_order(int32_t n_vox_pad, const int32_t *__restrict__ p
   if (j >= 0) out[j] = in[i];
 }
 
-__global__ void k_to_internal_order(int32_t n_vox_pad, const int32_t *__restrict__ perm, const float *__restrict__ in,
-                                    float *__restrict__ out) {
-  const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_vox_pad) return;
-  const int32_t j = perm[i];
-  out[i] = j >= 0 ? in[j] : 0.f;
-}
-
 // 0/1 beamlet mask of pool aperture k (for dao_set_pool)
 __global__ void k_pool_mask(int32_t k, int32_t n_bl, int32_t max_rows, const int32_t *__restrict__ bl_row,
                             const int32_t *__restrict__ row_beam, const int32_t *__restrict__ beam_row_ptr,
@@ -362,14 +354,8 @@ dao_status dao_get_vector(dao_ctx *ctx, int32_t which, void *dst, dao_memspace m
   size_t bytes = 0;
   const int t = 256, gv = (c->n_vox_pad + t - 1) / t;
   switch (which) {
-    case DAO_VEC_Z:
-    case DAO_VEC_G: {
-      float *tmp = reinterpret_cast<float *>(c->d.io_scratch);
-      k_to_user_order<float><<<gv, t, 0, c->stream>>>(c->n_vox_pad, c->d.perm, which == DAO_VEC_Z ? c->d.z : c->d.g, tmp);
-      API_CUDA(cudaGetLastError());
-      src = tmp; bytes = (size_t)c->n_vox * 4;
-      break;
-    }
+    case DAO_VEC_Z: src = c->d.z; bytes = (size_t)c->n_vox * 4; break;      // kept in the caller's order
+    case DAO_VEC_G: src = c->d.g; bytes = (size_t)c->n_vox * 4; break;
     case DAO_VEC_MASTER_Z: {
       double *tmp = reinterpret_cast<double *>(c->d.io_scratch);
       k_to_user_order<double><<<gv, t, 0, c->stream>>>(c->n_vox_pad, c->d.perm, c->d.mz, tmp);
@@ -402,11 +388,7 @@ dao_status dao_spmv(dao_ctx *ctx, const float *x_dev, float *z_dev) {
 dao_status dao_spmv_t(dao_ctx *ctx, const float *g_dev, float *w_dev) {
   Ctx *c = reinterpret_cast<Ctx *>(ctx);
   if (!c || !g_dev || !w_dev) return DAO_E_ARG;
-  float *tmp = reinterpret_cast<float *>(c->d.io_scratch);
-  const int t = 256;
-  k_to_internal_order<<<(c->n_vox_pad + t - 1) / t, t, 0, c->stream>>>(c->n_vox_pad, c->d.perm, g_dev, tmp);
-  API_CUDA(cudaGetLastError());
-  API_CUDA(launch_spmv_t(c, tmp, w_dev));
+  API_CUDA(launch_spmv_t(c, g_dev, w_dev));
   return DAO_OK;
 }
 

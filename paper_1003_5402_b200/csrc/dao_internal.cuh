@@ -14,11 +14,13 @@ namespace dao {
 // ------------------------------------------------------------------------------------------
 // Tunables (compile time)
 // ------------------------------------------------------------------------------------------
-constexpr int kSellC = 8;              // rows per sliced-ELL slice (quarter warp); 32/kSellC slices per warp
-constexpr int kSpmvThreads = 512;      // CTA size of the SELL SpMV kernel
+constexpr int kSellC = 32;             // rows per sliced-ELL slice: one warp, lane = row
+constexpr int kSpmvThreads = 512;      // CTA size of the direct-load SELL SpMV kernel
+constexpr int kSpmvRingThreads = 512;  // max CTA size of the TMA-ring SELL SpMV kernel (one CTA per SM)
 constexpr int kSpmvXSmemMax = 24576;   // x is staged in shared memory when n_bl <= this (96 KB fp32)
 constexpr int kTChunk = 4096;          // elements of D^T per CTA in the transposed SpMV
 constexpr int kTThreads = 256;
+constexpr int kTCtasPerSm = 6;         // persistent CTAs per SM of the transposed SpMV
 constexpr int kMasterThreads = 512;    // CTA size of the persistent master kernel (one CTA per SM)
 constexpr int kMasterTile = 2048;      // voxels of g staged in shared memory per tile in the master
 constexpr int kMaxStruct = 255;
@@ -69,7 +71,9 @@ struct StructEntry {       // per-structure penalty parameters of eq. (9)-(10), 
 };
 
 // All device pointers of a context.  Voxel-space arrays are in the INTERNAL voxel order
-// (internal row i holds the caller's voxel perm[i]).
+// (internal row i holds the caller's voxel perm[i]) EXCEPT z and g, which the dose SpMV scatters
+// straight into the caller's order (D^T gathers g by caller voxel id, where a beamlet's voxels
+// form contiguous runs).
 struct DevPtrs {
   // sliced ELL of D
   int32_t *sell_col;
@@ -81,7 +85,7 @@ struct DevPtrs {
   StructEntry *stab;       // [256]
   // CSR of D^T (rows = beamlets, entries = internal voxel ids)
   int32_t *t_ptr;          // [n_bl+1]
-  int32_t *t_row;          // [nnz padded to kTChunk]
+  int32_t *t_row;          // [nnz padded to kTChunk] caller voxel ids, ascending inside a row
   float *t_val;
   int32_t *t_first_row;    // [n_tchunks]
   int32_t *t_seg_base;     // [n_tchunks+1]
@@ -94,8 +98,8 @@ struct DevPtrs {
   // vectors
   float *x;                // [n_bl]
   float *xmask;            // [n_bl]
-  float *z;                // [n_vox_pad]
-  float *g;                // [n_vox_pad]
+  float *z;                // [n_vox_pad] caller order
+  float *g;                // [n_vox_pad] caller order
   float *w;                // [n_bl]
   double *f_part;          // [grid of the spmv kernel]
   // pricing
@@ -140,6 +144,7 @@ struct Ctx {
   int spmv_grid = 0, master_grid = 0;
   size_t master_smem = 0;
   bool x_in_smem = true;
+  int spmv_ring_warps = 0;      // > 0: the TMA-ring SpMV variant with that many warps per CTA
   // host mirror (pinned) of DevState for the once-per-iteration read-back
   DevState *h_state = nullptr;
   // host bookkeeping
@@ -177,6 +182,7 @@ enum SpmvMode { kSpmvObjective = 0, kSpmvPlain = 1, kSpmvColumn = 2, kSpmvPlainU
 cudaError_t launch_spmv(Ctx *c, SpmvMode mode, const float *x, float *out);
 cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out);
 cudaError_t launch_intensity(Ctx *c);
+void spmv_configure(Ctx *c);
 
 // dao_pricing.cu
 cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, const int32_t *beam_row_ptr,

@@ -1,7 +1,7 @@
 // dao_setup.cu -- dao_workspace_bytes / dao_create: validation, upload, and the one-time
 // construction of the device layouts:
-//   * sliced-ELL copy of D in an internal voxel order (rows sorted by length inside windows of
-//     `sell_sigma` rows so that the 8-row slices carry ~1 % padding),
+//   * sliced-ELL copy of D in an internal voxel order (rows sorted by length, by default over
+//     the whole matrix, so that the 32-row slices carry ~0 % padding),
 //   * explicit CSR of D^T (PAPER.md:171 rebuilds the transpose every iteration with Thrust; D is
 //     fixed here, so it is built once) by a stable LSD radix sort on the column index,
 //   * chunk tables of the transposed SpMV, MLC lookup tables, the per-structure penalty table
@@ -24,10 +24,13 @@ struct HostLayout {
   std::vector<int32_t> perm;          // [n_vox_pad] internal -> caller (-1 padding)
   std::vector<int32_t> inv_perm;      // [n_vox]
   std::vector<uint32_t> slice_off;    // [n_slices+1]
-  std::vector<int32_t> int_row_ptr;   // [n_vox+1] prefix of row lengths in internal order
 };
 
-static int effective_sigma(const dao_options *opt) { return opt->sell_sigma > 0 ? opt->sell_sigma : 512; }
+// 0 = library default = one window over all rows (global sort by length: no padding beyond the
+// 32-row slice granularity; z and g are scattered to the caller's order, so nothing else depends on it)
+static int effective_sigma(const dao_options *opt, int32_t n_vox) {
+  return opt->sell_sigma > 0 ? opt->sell_sigma : std::max(n_vox, 1);
+}
 
 static dao_status make_layout(const int32_t *row_ptr, int32_t n_vox, int sigma, HostLayout *L, std::string *err) {
   L->n_vox_pad = (int32_t)align_up((size_t)std::max(n_vox, 1), 128);
@@ -35,7 +38,15 @@ static dao_status make_layout(const int32_t *row_ptr, int32_t n_vox, int sigma, 
   L->perm.assign(L->n_vox_pad, -1);
   L->inv_perm.assign(n_vox, 0);
   std::iota(L->perm.begin(), L->perm.begin() + n_vox, 0);
-  if (sigma > 1) {
+  if (sigma >= n_vox && n_vox > 1) {
+    // one window: stable counting sort by descending row length
+    int32_t max_len = 0;
+    for (int32_t j = 0; j < n_vox; ++j) max_len = std::max(max_len, row_ptr[j + 1] - row_ptr[j]);
+    std::vector<int32_t> start((size_t)max_len + 2, 0);
+    for (int32_t j = 0; j < n_vox; ++j) ++start[(size_t)(max_len - (row_ptr[j + 1] - row_ptr[j])) + 1];
+    for (size_t b = 1; b < start.size(); ++b) start[b] += start[b - 1];
+    for (int32_t j = 0; j < n_vox; ++j) L->perm[start[(size_t)(max_len - (row_ptr[j + 1] - row_ptr[j]))]++] = j;
+  } else if (sigma > 1) {
     for (int32_t s = 0; s < n_vox; s += sigma) {
       const int32_t e = std::min(n_vox, s + sigma);
       std::stable_sort(L->perm.begin() + s, L->perm.begin() + e, [&](int32_t a, int32_t b) {
@@ -45,7 +56,6 @@ static dao_status make_layout(const int32_t *row_ptr, int32_t n_vox, int sigma, 
   }
   for (int32_t i = 0; i < n_vox; ++i) L->inv_perm[L->perm[i]] = i;
   L->slice_off.assign(L->n_slices + 1, 0);
-  L->int_row_ptr.assign(n_vox + 1, 0);
   int64_t total = 0;
   for (int32_t s = 0; s < L->n_slices; ++s) {
     int32_t mx = 0;
@@ -62,10 +72,6 @@ static dao_status make_layout(const int32_t *row_ptr, int32_t n_vox, int sigma, 
   }
   L->slice_off[L->n_slices] = (uint32_t)total;
   L->sell_elems = total;
-  for (int32_t i = 0; i < n_vox; ++i) {
-    const int32_t j = L->perm[i];
-    L->int_row_ptr[i + 1] = L->int_row_ptr[i] + (row_ptr[j + 1] - row_ptr[j]);
-  }
   return DAO_OK;
 }
 
@@ -141,7 +147,6 @@ static void carve_workspace(Carver &cv, const Dims &dm, const HostLayout &L, Dev
 struct ScratchPtrs {
   int32_t *row_ptr, *col, *vs;
   float *val;
-  int32_t *int_row_ptr;
   int32_t *keyA, *rowA, *keyB, *rowB;
   float *valA, *valB;
   int32_t *tile_hist;
@@ -160,7 +165,6 @@ static void carve_scratch(Carver &cv, const Dims &dm, bool host_inputs, ScratchP
     s->row_ptr = s->col = s->vs = nullptr;
     s->val = nullptr;
   }
-  s->int_row_ptr = cv.take<int32_t>((size_t)dm.n_vox + 1);
   s->keyA = cv.take<int32_t>(nz);
   s->rowA = cv.take<int32_t>(nz);
   s->valA = cv.take<float>(nz);
@@ -260,7 +264,7 @@ dao_status setup_sizes(const dao_csr *D, const dao_mlc *mlc, const dao_structs *
   st = fetch_row_ptr(D, &rp, err);
   if (st != DAO_OK) return st;
   HostLayout L;
-  st = make_layout(rp.data(), D->n_vox, effective_sigma(opt), &L, err);
+  st = make_layout(rp.data(), D->n_vox, effective_sigma(opt, D->n_vox), &L, err);
   if (st != DAO_OK) return st;
   Carver cw{nullptr};
   DevPtrs dp{};
@@ -331,23 +335,21 @@ __global__ void k_fill_sid(int32_t n_vox_pad, const int32_t *__restrict__ perm, 
   sid[i] = (uint8_t)(s < 0 ? kNoStruct : s);
 }
 
-// expand D into (column key, internal row, value) triples enumerated internal-row-major, and
-// count the entries of every column (for t_ptr).
-__global__ void k_expand(int32_t n_vox, const int32_t *__restrict__ perm, const int32_t *__restrict__ int_row_ptr,
-                         const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col,
+// expand D into (column key, voxel row, value) triples in CSR order (voxel ids are the caller's),
+// and count the entries of every column (for t_ptr).
+__global__ void k_expand(int32_t n_vox, const int32_t *__restrict__ row_ptr, const int32_t *__restrict__ col,
                          const float *__restrict__ val, int32_t *__restrict__ key, int32_t *__restrict__ row,
                          float *__restrict__ v, int32_t *__restrict__ col_count /* [n_bl+1], pre-zeroed */) {
   const int lane = threadIdx.x & 31;
   const int64_t warp_g = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int64_t n_warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
-  for (int64_t i = warp_g; i < n_vox; i += n_warps) {
-    const int32_t j = perm[i];
-    const int32_t src = row_ptr[j], n = row_ptr[j + 1] - src, dst = int_row_ptr[i];
-    for (int32_t e = lane; e < n; e += 32) {
-      const int32_t c = col[src + e];
-      key[dst + e] = c;
-      row[dst + e] = (int32_t)i;
-      v[dst + e] = val[src + e];
+  for (int64_t j = warp_g; j < n_vox; j += n_warps) {
+    const int32_t lo = row_ptr[j], hi = row_ptr[j + 1];
+    for (int32_t e = lo + lane; e < hi; e += 32) {
+      const int32_t c = col[e];
+      key[e] = c;
+      row[e] = (int32_t)j;
+      v[e] = val[e];
       atomicAdd(&col_count[c + 1], 1);
     }
   }
@@ -513,7 +515,7 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   st = fetch_row_ptr(D, &rp, &c->err);
   if (st != DAO_OK) return st;
   HostLayout L;
-  c->opt.sell_sigma = effective_sigma(&c->opt);
+  c->opt.sell_sigma = effective_sigma(&c->opt, D->n_vox);
   st = make_layout(rp.data(), D->n_vox, c->opt.sell_sigma, &L, &c->err);
   if (st != DAO_OK) return st;
 
@@ -582,7 +584,6 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   SETUP_CUDA(cudaMemcpyAsync(d.perm, L.perm.data(), (size_t)L.n_vox_pad * 4, cudaMemcpyHostToDevice, q));
   SETUP_CUDA(cudaMemcpyAsync(d.inv_perm, L.inv_perm.data(), (size_t)dm.n_vox * 4, cudaMemcpyHostToDevice, q));
   SETUP_CUDA(cudaMemcpyAsync(d.slice_off, L.slice_off.data(), ((size_t)L.n_slices + 1) * 4, cudaMemcpyHostToDevice, q));
-  SETUP_CUDA(cudaMemcpyAsync(sp.int_row_ptr, L.int_row_ptr.data(), ((size_t)dm.n_vox + 1) * 4, cudaMemcpyHostToDevice, q));
   k_fill_sell<<<grid_for(L.n_vox_pad, 128), 128, 0, q>>>(L.n_vox_pad, d.perm, d.slice_off, d_row_ptr, d_col, d_val,
                                                         d.sell_col, d.sell_val);
   SETUP_CUDA(cudaGetLastError());
@@ -597,8 +598,8 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   SETUP_CUDA(cudaMemsetAsync(d.t_val, 0, ((size_t)ntc * kTChunk + 64) * 4, q));
   std::vector<int32_t> h_tptr((size_t)dm.n_bl + 1, 0);
   if (dm.nnz > 0) {
-    k_expand<<<grid_for((int64_t)dm.n_vox * 32, 256, c->n_sm * 16), 256, 0, q>>>(dm.n_vox, d.perm, sp.int_row_ptr, d_row_ptr, d_col,
-                                                                             d_val, sp.keyA, sp.rowA, sp.valA, d.t_ptr);
+    k_expand<<<grid_for((int64_t)dm.n_vox * 32, 256, c->n_sm * 16), 256, 0, q>>>(dm.n_vox, d_row_ptr, d_col, d_val, sp.keyA,
+                                                                             sp.rowA, sp.valA, d.t_ptr);
     SETUP_CUDA(cudaGetLastError());
     k_scan_inclusive<<<1, 1024, 0, q>>>(d.t_ptr, (int64_t)dm.n_bl + 1);
     SETUP_CUDA(cudaGetLastError());
@@ -681,8 +682,7 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   SETUP_CUDA(cudaMemsetAsync(d.vstar, 0, (size_t)dm.n_rows * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.beam_price, 0, (size_t)dm.n_beams * 8, q));
 
-  c->x_in_smem = dm.n_bl <= kSpmvXSmemMax;
-  c->spmv_grid = c->n_sm * 2;
+  spmv_configure(c);
   SETUP_CUDA(master_configure(c));
   SETUP_CUDA(cudaStreamSynchronize(q));
   return DAO_OK;

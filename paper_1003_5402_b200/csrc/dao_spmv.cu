@@ -1,44 +1,12 @@
-// dao_spmv.cu -- the bandwidth-bound kernels of the hot path:
+// dao_spmv.cu -- steps 1, 2, 3, 7 of the hot path:
 //   step 1  x_i = sum_{k : i in A_k} y_k                 (eq. 7)
 //   step 2  z = D x over a sliced-ELL copy of D          (eq. 1)
 //   step 3  F(z), pi = dF/dz fused into the epilogue     (PAPER.md:75-83 eq. 3-5, :246-254 eq. 9-10, :136)
-//   step 4  w = D^T pi over an explicit CSR of D^T       (eq. 8)
 //   step 7  a_K = D 1_A (same kernel as step 2)          (eq. 2)
 #include "dao_internal.cuh"
+#include "dao_ptx.cuh"
 
 namespace dao {
-
-// streaming 32-bit loads that do not allocate in L1 (the matrix is read once per pass)
-__device__ __forceinline__ int32_t ld_stream_i32(const int32_t *p) {
-  int32_t v;
-  asm volatile("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(v) : "l"(p));
-  return v;
-}
-__device__ __forceinline__ float ld_stream_f32(const float *p) {
-  float v;
-  asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(v) : "l"(p));
-  return v;
-}
-__device__ __forceinline__ int4 ld_stream_i32x4(const int4 *p) {
-  int4 v;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
-               : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
-               : "l"(p));
-  return v;
-}
-__device__ __forceinline__ float4 ld_stream_f32x4(const float4 *p) {
-  float4 v;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
-               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
-               : "l"(p));
-  return v;
-}
-
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;
-}
 
 // ------------------------------------------------------------------------------------------
 // step 1: beamlet intensities (eq. 7).  One thread per beamlet, apertures visited in pool order,
@@ -76,11 +44,11 @@ cudaError_t launch_intensity(Ctx *c) {
 }
 
 // ------------------------------------------------------------------------------------------
-// steps 2, 3, 7: sliced-ELL SpMV.  A warp owns 32 consecutive internal rows = 32/C slices of C
-// rows; lane -> (slice, row in slice).  Element k of a row sits at slice_off + k*C + row, so a
-// warp-wide load touches 32/C fully used 4*C-byte segments.  Per-lane fp64 accumulation in the
-// caller's column order (= ascending k), no cross-lane reduction.  Persistent grid: warps stride
-// over the row groups.
+// steps 2, 3, 7: sliced-ELL SpMV.  A warp owns one slice of 32 consecutive internal rows, lane =
+// row; element k of a row sits at slice_off + 32 k + lane, so every warp-wide access is one fully
+// used 128-byte line.  Per-lane fp64 accumulation in the caller's column order (= ascending k, the
+// order of the oracle's row loop), no cross-lane reduction.  Persistent grid: warps stride over
+// the slices.
 // ------------------------------------------------------------------------------------------
 struct SpmvParams {
   const int32_t *col;
@@ -88,7 +56,7 @@ struct SpmvParams {
   const uint32_t *slice_off;
   const float *x;
   int32_t n_bl;
-  int32_t n_groups;          // groups of 32 rows
+  int32_t n_slices;          // slices of 32 rows
   int32_t n_vox_pad;
   // outputs
   float *out;                // z (objective / plain) or the dose block A (column mode)
@@ -100,16 +68,179 @@ struct SpmvParams {
   DevState *st;
 };
 
-template <int C, bool XS, int MODE>
+// per-row epilogue: objective / gradient (step 3) or plain store
+template <int MODE>
+__device__ __forceinline__ void spmv_store(const SpmvParams &p, float *out, const StructEntry *stab_s, int i,
+                                           double acc, double &f_acc) {
+  if (MODE == kSpmvObjective) {
+    const int s = p.sid[i];
+    double gv = 0.0;
+    if (s != kNoStruct) {
+      const StructEntry e = stab_s[s];
+      const double u = fmax(e.tm - acc, 0.0);
+      const double o = fmax(acc - e.tp, 0.0);
+      f_acc += e.a * u * u + e.b * o * o;
+      gv = -2.0 * e.a * u + 2.0 * e.b * o;
+    }
+    const int32_t j = p.perm[i];         // z and pi are kept in the caller's voxel order
+    if (j >= 0) {
+      out[j] = (float)acc;
+      p.g[j] = (float)gv;
+    }
+  } else if (MODE == kSpmvPlainUserOrder) {
+    const int32_t j = p.perm[i];
+    if (j >= 0) out[j] = (float)acc;
+  } else {
+    out[i] = (float)acc;
+  }
+}
+
+// block partial of F, then the last block to finish adds the partials in block order
+__device__ __forceinline__ void spmv_finish_objective(const SpmvParams &p, double f_acc, double *red /*[nwarps]*/) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  __shared__ bool is_last;
+  f_acc = warp_sum_f64(f_acc);
+  if (lane == 0) red[warp] = f_acc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double s = 0.0;
+    for (int w = 0; w < nw; ++w) s += red[w];
+    p.f_part[blockIdx.x] = s;
+    __threadfence();
+    const uint32_t t = atomicAdd(&p.st->ticket_spmv, 1u);
+    is_last = (t == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (is_last && warp == 0) {
+    __threadfence();
+    double s = 0.0;
+    for (int b = lane; b < (int)gridDim.x; b += 32) s += __ldcg(p.f_part + b);
+    s = warp_sum_f64(s);
+    if (lane == 0) {
+      p.st->F = s;
+      p.st->ticket_spmv = 0u;
+    }
+  }
+}
+
+// ---- variant A: the matrix streams through a warp-private cp.async.bulk (TMA) ring ---------------
+// Every warp keeps kRingStages chunks of kRingK k-steps (kRingK * 32 * 8 bytes) in flight into its
+// own shared-memory ring, completion signalled on per-stage mbarriers; lane 0 is the producer, the
+// whole warp consumes.  Bytes in flight per SM = warps * stages * 4 KB, independent of registers.
+constexpr int kRingK = 16;                                   // k-steps per chunk
+constexpr int kRingStages = 3;
+constexpr int kRingChunkElems = kRingK * 32;                 // per array
+constexpr int kRingStageBytes = kRingChunkElems * 8;         // col + val
+
+struct RingCursor {          // position in a warp's list of chunks
+  int slice;                 // current slice (strided over the grid)
+  int k0;                    // first k-step of the next chunk in that slice
+  uint32_t off;              // slice_off[slice]
+  int len;                   // k-steps of the slice
+};
+
+template <int MODE>
+__global__ void __launch_bounds__(kSpmvRingThreads, 1) k_spmv_ring(SpmvParams p) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int nw = blockDim.x >> 5;
+  // layout: ring [nw][stages][col chunk | val chunk], barriers, x
+  unsigned char *ring = smem_raw;
+  uint64_t *bars = reinterpret_cast<uint64_t *>(ring + (size_t)nw * kRingStages * kRingStageBytes);
+  float *xs = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(bars) + align_up_c(nw * kRingStages * 8, 128));
+  __shared__ double red[kSpmvRingThreads / 32];
+  __shared__ StructEntry stab_s[MODE == kSpmvObjective ? 256 : 1];
+
+  float *out = p.out;
+  if (MODE == kSpmvColumn) {
+    if (!p.st->cand_valid) return;                       // nothing to add (converged or pool full)
+    out += (size_t)p.st->K * (size_t)p.n_vox_pad;
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) {
+    for (int s = 0; s < kRingStages; ++s) mbar_init(&bars[warp * kRingStages + s], 1);
+  }
+  fence_mbar_init();
+  for (int i = threadIdx.x; i < p.n_bl; i += blockDim.x) xs[i] = p.x[i];
+  if (MODE == kSpmvObjective) {
+    for (int i = threadIdx.x; i < 256; i += blockDim.x) stab_s[i] = p.stab[i];
+  }
+  __syncthreads();
+
+  const int stride = gridDim.x * nw;
+  const int first = blockIdx.x * nw + warp;
+  unsigned char *my_ring = ring + (size_t)warp * kRingStages * kRingStageBytes;
+  uint64_t *my_bars = bars + warp * kRingStages;
+
+  // producer cursor: skips empty slices
+  RingCursor pc;
+  pc.slice = first; pc.k0 = 0; pc.off = 0; pc.len = 0;
+  auto load_slice = [&](RingCursor &c) {
+    while (c.slice < p.n_slices) {
+      const uint32_t o = p.slice_off[c.slice];
+      const int len = (int)((p.slice_off[c.slice + 1] - o) >> 5);
+      if (len > 0) { c.off = o; c.len = len; c.k0 = 0; return; }
+      c.slice += stride;
+    }
+    c.len = 0;
+  };
+  load_slice(pc);
+  uint32_t n_issued = 0, n_consumed = 0;
+  auto issue = [&]() {                       // issue the chunk at the producer cursor (all lanes track it)
+    if (pc.slice >= p.n_slices) return;
+    const int kn = min(kRingK, pc.len - pc.k0);
+    const uint32_t bytes = (uint32_t)kn * 32u * 4u;
+    const int stage = n_issued % kRingStages;
+    if (lane == 0) {
+      unsigned char *dst = my_ring + (size_t)stage * kRingStageBytes;
+      const size_t e0 = (size_t)pc.off + (size_t)pc.k0 * 32;
+      mbar_arrive_expect_tx(&my_bars[stage], 2u * bytes);
+      bulk_g2s(dst, p.col + e0, bytes, &my_bars[stage]);
+      bulk_g2s(dst + kRingChunkElems * 4, p.val + e0, bytes, &my_bars[stage]);
+    }
+    ++n_issued;
+    pc.k0 += kn;
+    if (pc.k0 >= pc.len) { pc.slice += stride; load_slice(pc); }
+  };
+#pragma unroll
+  for (int s = 0; s < kRingStages; ++s) issue();
+
+  double f_acc = 0.0;
+  for (int slice = first; slice < p.n_slices; slice += stride) {
+    const uint32_t off = p.slice_off[slice];
+    const int len = (int)((p.slice_off[slice + 1] - off) >> 5);
+    double acc = 0.0;
+    for (int k0 = 0; k0 < len; k0 += kRingK) {
+      const int kn = min(kRingK, len - k0);
+      const int stage = n_consumed % kRingStages;
+      mbar_wait(&my_bars[stage], (n_consumed / kRingStages) & 1u);
+      const int32_t *sc = reinterpret_cast<const int32_t *>(my_ring + (size_t)stage * kRingStageBytes) + lane;
+      const float *sv = reinterpret_cast<const float *>(my_ring + (size_t)stage * kRingStageBytes + kRingChunkElems * 4) + lane;
+      if (kn == kRingK) {
+#pragma unroll
+        for (int k = 0; k < kRingK; ++k) acc = fma((double)sv[k * 32], (double)xs[sc[k * 32]], acc);
+      } else {
+        for (int k = 0; k < kn; ++k) acc = fma((double)sv[k * 32], (double)xs[sc[k * 32]], acc);
+      }
+      ++n_consumed;
+      __syncwarp();                          // every lane is done with the stage before it is refilled
+      issue();
+    }
+    spmv_store<MODE>(p, out, stab_s, slice * 32 + lane, acc, f_acc);
+  }
+  if (MODE == kSpmvObjective) spmv_finish_objective(p, f_acc, red);
+}
+
+// ---- variant B: direct global loads (used when x does not fit next to the ring) -------------------
+template <bool XS, int MODE>
 __global__ void __launch_bounds__(kSpmvThreads, 2) k_spmv_sell(SpmvParams p) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   float *xs = reinterpret_cast<float *>(smem_raw);
   __shared__ double red[kSpmvThreads / 32];
   __shared__ StructEntry stab_s[MODE == kSpmvObjective ? 256 : 1];
 
   float *out = p.out;
   if (MODE == kSpmvColumn) {
-    if (!p.st->cand_valid) return;                       // nothing to add (converged or pool full)
+    if (!p.st->cand_valid) return;
     out += (size_t)p.st->K * (size_t)p.n_vox_pad;
   }
   if (XS) {
@@ -120,20 +251,13 @@ __global__ void __launch_bounds__(kSpmvThreads, 2) k_spmv_sell(SpmvParams p) {
   }
   __syncthreads();
 
-  const int lane = threadIdx.x & 31;
-  const int warp = threadIdx.x >> 5;
-  const int warps_per_block = blockDim.x >> 5;
-  const int sub = lane / C;              // which slice of the group
-  const int r = lane % C;                // row inside the slice
-  constexpr int SPG = 32 / C;            // slices per group
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
   double f_acc = 0.0;
-
-  for (int grp = blockIdx.x * warps_per_block + warp; grp < p.n_groups; grp += gridDim.x * warps_per_block) {
-    const int slice = grp * SPG + sub;
+  for (int slice = blockIdx.x * nw + warp; slice < p.n_slices; slice += gridDim.x * nw) {
     const uint32_t off = p.slice_off[slice];
-    const int len = (int)((p.slice_off[slice + 1] - off) / C);
-    const int32_t *pc = p.col + off + r;
-    const float *pv = p.val + off + r;
+    const int len = (int)((p.slice_off[slice + 1] - off) >> 5);
+    const int32_t *pc = p.col + off + lane;
+    const float *pv = p.val + off + lane;
     double acc = 0.0;
     int k = 0;
 #pragma unroll 1
@@ -142,8 +266,8 @@ __global__ void __launch_bounds__(kSpmvThreads, 2) k_spmv_sell(SpmvParams p) {
       float vv[8];
 #pragma unroll
       for (int u = 0; u < 8; ++u) {
-        cc[u] = ld_stream_i32(pc + (k + u) * C);
-        vv[u] = ld_stream_f32(pv + (k + u) * C);
+        cc[u] = ld_stream_i32(pc + (k + u) * 32);
+        vv[u] = ld_stream_f32(pv + (k + u) * 32);
       }
 #pragma unroll
       for (int u = 0; u < 8; ++u) {
@@ -152,58 +276,14 @@ __global__ void __launch_bounds__(kSpmvThreads, 2) k_spmv_sell(SpmvParams p) {
       }
     }
     for (; k < len; ++k) {
-      const int32_t cc = ld_stream_i32(pc + k * C);
-      const float vv = ld_stream_f32(pv + k * C);
+      const int32_t cc = ld_stream_i32(pc + k * 32);
+      const float vv = ld_stream_f32(pv + k * 32);
       const float xv = XS ? xs[cc] : __ldg(p.x + cc);
       acc = fma((double)vv, (double)xv, acc);
     }
-    const int i = grp * 32 + lane;       // internal row
-    if (MODE == kSpmvObjective) {
-      const int s = p.sid[i];
-      double gv = 0.0;
-      if (s != kNoStruct) {
-        const StructEntry e = stab_s[s];
-        const double u = fmax(e.tm - acc, 0.0);
-        const double o = fmax(acc - e.tp, 0.0);
-        f_acc += e.a * u * u + e.b * o * o;
-        gv = -2.0 * e.a * u + 2.0 * e.b * o;
-      }
-      out[i] = (float)acc;
-      p.g[i] = (float)gv;
-    } else if (MODE == kSpmvPlainUserOrder) {
-      const int32_t j = p.perm[i];
-      if (j >= 0) out[j] = (float)acc;
-    } else {
-      out[i] = (float)acc;
-    }
+    spmv_store<MODE>(p, out, stab_s, slice * 32 + lane, acc, f_acc);
   }
-
-  if (MODE == kSpmvObjective) {
-    // block partial of F, then the last block to finish adds the partials in block order
-    f_acc = warp_sum(f_acc);
-    if (lane == 0) red[warp] = f_acc;
-    __syncthreads();
-    __shared__ bool is_last;
-    if (threadIdx.x == 0) {
-      double s = 0.0;
-      for (int w = 0; w < warps_per_block; ++w) s += red[w];
-      p.f_part[blockIdx.x] = s;
-      __threadfence();
-      const uint32_t t = atomicAdd(&p.st->ticket_spmv, 1u);
-      is_last = (t == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (is_last && warp == 0) {
-      __threadfence();
-      double s = 0.0;
-      for (int b = lane; b < (int)gridDim.x; b += 32) s += __ldcg(p.f_part + b);
-      s = warp_sum(s);
-      if (lane == 0) {
-        p.st->F = s;
-        p.st->ticket_spmv = 0u;
-      }
-    }
-  }
+  if (MODE == kSpmvObjective) spmv_finish_objective(p, f_acc, red);
 }
 
 template <int MODE>
@@ -214,7 +294,7 @@ static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out) {
   p.slice_off = c->d.slice_off;
   p.x = x;
   p.n_bl = c->n_bl;
-  p.n_groups = c->n_vox_pad / 32;
+  p.n_slices = c->n_slices;
   p.n_vox_pad = c->n_vox_pad;
   p.out = out;
   p.g = c->d.g;
@@ -223,18 +303,30 @@ static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out) {
   p.perm = c->d.perm;
   p.f_part = c->d.f_part;
   p.st = c->d.state;
-  const int groups_per_block = kSpmvThreads / 32;
-  int grid = (p.n_groups + groups_per_block - 1) / groups_per_block;
+  if (c->spmv_ring_warps > 0) {
+    const int nw = c->spmv_ring_warps;
+    const size_t smem = (size_t)nw * kRingStages * kRingStageBytes + align_up((size_t)nw * kRingStages * 8, 128) +
+                        align_up((size_t)c->n_bl * 4, 128);
+    auto kern = k_spmv_ring<MODE>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int grid = (p.n_slices + nw - 1) / nw;
+    if (grid > c->n_sm) grid = c->n_sm;
+    kern<<<grid, nw * 32, smem, c->stream>>>(p);
+    return cudaGetLastError();
+  }
+  const int per_block = kSpmvThreads / 32;
+  int grid = (p.n_slices + per_block - 1) / per_block;
   if (grid > c->spmv_grid) grid = c->spmv_grid;
   if (grid < 1) grid = 1;
   if (c->x_in_smem) {
     const size_t smem = (size_t)c->n_bl * sizeof(float);
-    auto kern = k_spmv_sell<kSellC, true, MODE>;
+    auto kern = k_spmv_sell<true, MODE>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, kSpmvThreads, smem, c->stream>>>(p);
   } else {
-    k_spmv_sell<kSellC, false, MODE><<<grid, kSpmvThreads, 0, c->stream>>>(p);
+    k_spmv_sell<false, MODE><<<grid, kSpmvThreads, 0, c->stream>>>(p);
   }
   return cudaGetLastError();
 }
@@ -248,98 +340,18 @@ cudaError_t launch_spmv(Ctx *c, SpmvMode mode, const float *x, float *out) {
   }
 }
 
-// ------------------------------------------------------------------------------------------
-// step 4: w = D^T g over the explicit CSR of D^T (rows = beamlets, ~10^4 entries each).  The
-// entry array is cut into chunks of kTChunk elements, one CTA per chunk.  A chunk that lies in
-// one row (the common case) is reduced with 128-bit streaming loads; a chunk that straddles
-// rows takes a generic warp-per-row-segment path.  Every (chunk, row) segment sum goes to its
-// own slot; k_spmvt_finish adds the slots of a row in chunk order, so w is bit-reproducible
-// without atomics.  g is gathered through L1/L2 (4 n_vox bytes, L2 resident).
-// ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kTThreads) k_spmvt(const int32_t *__restrict__ t_ptr,
-                                                     const int32_t *__restrict__ t_row,
-                                                     const float *__restrict__ t_val, int64_t nnz,
-                                                     const int32_t *__restrict__ first_row,
-                                                     const int32_t *__restrict__ seg_base,
-                                                     const float *__restrict__ g, double *__restrict__ segsum) {
-  __shared__ double red[kTThreads / 32];
-  const int c = blockIdx.x;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int64_t cbeg = (int64_t)c * kTChunk;
-  int64_t cend = cbeg + kTChunk;
-  const bool full = cend <= nnz;
-  if (!full) cend = nnz;
-  const int first = first_row[c];
-  const int nseg = seg_base[c + 1] - seg_base[c];
-  if (nseg == 1 && full) {
-    double acc = 0.0;
-    const int4 *pr = reinterpret_cast<const int4 *>(t_row + cbeg);
-    const float4 *pv = reinterpret_cast<const float4 *>(t_val + cbeg);
-    constexpr int IT = kTChunk / (4 * kTThreads);
-    int4 rr[IT];
-    float4 vv[IT];
-#pragma unroll
-    for (int it = 0; it < IT; ++it) {
-      rr[it] = ld_stream_i32x4(pr + it * kTThreads + threadIdx.x);
-      vv[it] = ld_stream_f32x4(pv + it * kTThreads + threadIdx.x);
-    }
-#pragma unroll
-    for (int it = 0; it < IT; ++it) {
-      const float g0 = __ldg(g + rr[it].x), g1 = __ldg(g + rr[it].y);
-      const float g2 = __ldg(g + rr[it].z), g3 = __ldg(g + rr[it].w);
-      acc = fma((double)vv[it].x, (double)g0, acc);
-      acc = fma((double)vv[it].y, (double)g1, acc);
-      acc = fma((double)vv[it].z, (double)g2, acc);
-      acc = fma((double)vv[it].w, (double)g3, acc);
-    }
-    acc = warp_sum(acc);
-    if (lane == 0) red[warp] = acc;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      double s = 0.0;
-#pragma unroll
-      for (int w = 0; w < kTThreads / 32; ++w) s += red[w];
-      segsum[seg_base[c]] = s;
-    }
-  } else {
-    for (int sgi = warp; sgi < nseg; sgi += kTThreads / 32) {
-      const int row = first + sgi;
-      int64_t lo = t_ptr[row], hi = t_ptr[row + 1];
-      if (lo < cbeg) lo = cbeg;
-      if (hi > cend) hi = cend;
-      double acc = 0.0;
-      for (int64_t e = lo + lane; e < hi; e += 32) acc = fma((double)t_val[e], (double)__ldg(g + t_row[e]), acc);
-      acc = warp_sum(acc);
-      if (lane == 0) segsum[seg_base[c] + sgi] = acc;
-    }
+// Decide which SpMV variant a context uses: the TMA ring with as many warps as fit beside x.
+void spmv_configure(Ctx *c) {
+  c->x_in_smem = c->n_bl <= kSpmvXSmemMax;
+  c->spmv_grid = c->n_sm * 2;
+  c->spmv_ring_warps = 0;
+  if (c->opt.reserved & 1) return;                       // test hook: force the direct-load variant
+  const size_t budget = 227 * 1024 - 12 * 1024;          // dynamic smem left beside the static tables
+  const size_t xbytes = align_up((size_t)c->n_bl * 4, 128);
+  for (int nw = kSpmvRingThreads / 32; nw >= 8; nw -= 2) {
+    const size_t need = (size_t)nw * kRingStages * kRingStageBytes + align_up((size_t)nw * kRingStages * 8, 128) + xbytes;
+    if (need <= budget) { c->spmv_ring_warps = nw; break; }
   }
-}
-
-__global__ void k_spmvt_finish(int32_t n_bl, const int32_t *__restrict__ t_ptr,
-                               const int32_t *__restrict__ first_row, const int32_t *__restrict__ seg_base,
-                               const double *__restrict__ segsum, float *__restrict__ w) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_bl) return;
-  const int64_t lo = t_ptr[i], hi = t_ptr[i + 1];
-  double s = 0.0;
-  if (hi > lo) {
-    const int ca = (int)(lo / kTChunk), cb = (int)((hi - 1) / kTChunk);
-    for (int c = ca; c <= cb; ++c) s += segsum[seg_base[c] + (i - first_row[c])];
-  }
-  w[i] = (float)s;
-}
-
-cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out) {
-  if (c->n_tchunks > 0) {
-    k_spmvt<<<c->n_tchunks, kTThreads, 0, c->stream>>>(c->d.t_ptr, c->d.t_row, c->d.t_val, c->nnz,
-                                                        c->d.t_first_row, c->d.t_seg_base, g, c->d.t_segsum);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-  }
-  const int t = 128;
-  k_spmvt_finish<<<(c->n_bl + t - 1) / t, t, 0, c->stream>>>(c->n_bl, c->d.t_ptr, c->d.t_first_row,
-                                                             c->d.t_seg_base, c->d.t_segsum, w_out);
-  return cudaGetLastError();
 }
 
 }  // namespace dao
