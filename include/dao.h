@@ -106,7 +106,8 @@ typedef struct {
   int32_t sell_sigma;        /* sorting window (rows) of the internal sliced-ELL layout of D; 1 = keep the
                                 caller's voxel order; 0 = library default */
   int32_t timers;            /* non-zero: CUDA-event timers per kernel class in dao_run (default 1) */
-  int32_t reserved;
+  int32_t reserved;          /* test/bench hooks, 0 in production: bit 0 forces the direct-load SpMV variant,
+                                bit 1 turns on the master's phase timers (DAO_VEC_MASTER_PHASES) */
 } dao_options;
 
 typedef struct {
@@ -179,7 +180,12 @@ typedef enum {               /* dao_get_vector selectors; lengths in elements */
   DAO_VEC_RIGHT = 7,         /* int32  [n_rows] */
   DAO_VEC_BEAM_PRICE = 8,    /* double [n_beams] */
   DAO_VEC_HISTORY = 9,       /* dao_iter_record [k_max] (first n_apertures valid) */
-  DAO_VEC_MASTER_Z = 10      /* double [n_vox]  z = A y as the master holds it, caller's voxel order */
+  DAO_VEC_MASTER_Z = 10,     /* double [n_vox]  z = A y as the master holds it, caller's voxel order */
+  DAO_VEC_MASTER_PHASES = 11 /* uint64 [16]     phase timers of the master kernel, accumulated since dao_create when
+                                dao_options.reserved has bit 1 (value 2) set, else zeros.  Nanoseconds of CTA 0 in:
+                                0 set-up and z = A y, 1 gradient pass over A, 2 gradient reduction, 3 direction,
+                                4 dz = A p pass, 5 curvature reduction, 6 line search, 10 publish; counts:
+                                7 line-search evaluations, 8 projected-gradient iterations, 9 calls */
 } dao_vector;
 
 void dao_default_options(dao_options *opt);

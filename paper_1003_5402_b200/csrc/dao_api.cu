@@ -370,6 +370,7 @@ dao_status dao_get_vector(dao_ctx *ctx, int32_t which, void *dst, dao_memspace m
     case DAO_VEC_LEFT: src = c->d.left; bytes = (size_t)c->n_rows * 4; break;
     case DAO_VEC_RIGHT: src = c->d.right; bytes = (size_t)c->n_rows * 4; break;
     case DAO_VEC_BEAM_PRICE: src = c->d.beam_price; bytes = (size_t)c->n_beams * 8; break;
+    case DAO_VEC_MASTER_PHASES: src = c->d.m_prof; bytes = (size_t)kMasterProfSlots * 8; break;
     case DAO_VEC_HISTORY: src = c->d.history; bytes = (size_t)c->opt.k_max * sizeof(dao_iter_record); break;
     default: return fail(c, DAO_E_ARG, "unknown vector selector");
   }

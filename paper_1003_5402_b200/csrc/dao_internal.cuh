@@ -21,8 +21,14 @@ constexpr int kSpmvXSmemMax = 24576;   // x is staged in shared memory when n_bl
 constexpr int kTChunk = 4096;          // elements of D^T per CTA in the transposed SpMV
 constexpr int kTThreads = 256;
 constexpr int kTCtasPerSm = 6;         // persistent CTAs per SM of the transposed SpMV
-constexpr int kMasterThreads = 512;    // CTA size of the persistent master kernel (one CTA per SM)
-constexpr int kMasterTile = 2048;      // voxels of g staged in shared memory per tile in the master
+constexpr int kMasterWorkers = 512;    // worker threads of the persistent master kernel (one CTA per SM)
+constexpr int kMasterThreads = kMasterWorkers + 32;   // + the producer warp that streams A through the ring
+constexpr int kMasterTileVox = 4096;   // voxels per ring stage: 16 worker warps x 2 strips x 128
+constexpr int kMasterStageBytes = kMasterTileVox * 4;
+constexpr int kMasterMaxStages = 10;
+constexpr int kMasterProfSlots = 16;   // phase timers of the master (ns): 0 init, 1 G pass, 2 G reduce, 3 direction,
+                                       // 4 D pass, 5 D reduce, 6 line search; 7 line-search evaluations,
+                                       // 8 iterations, 9 calls, 10 publish
 constexpr int kMaxStruct = 255;
 constexpr int kNoStruct = 255;         // sid value of a voxel without penalty
 constexpr int kMaxRedux = DAO_MAX_APERTURES + 8;   // doubles per grid reduction in the master
@@ -117,8 +123,10 @@ struct DevPtrs {
   // master
   double *mz;              // [n_vox_pad] z = A y
   double *mdz;             // [n_vox_pad] dz = A p
-  double *m_part;          // [2][n_cta][kMaxRedux] partials of the grid reductions
-  double *m_result;        // [2][kMaxRedux]
+  uint4 *ll_part;          // [2][n_cta][kMaxRedux] flagged slots {lo32, epoch, hi32, epoch} of the grid reductions
+  uint4 *ll_result;        // [2][kMaxRedux]
+  uint32_t *m_epoch;       // reduction epoch (monotone over the life of the context)
+  unsigned long long *m_prof;  // [kMasterProfSlots]
   // history
   dao_iter_record *history;  // [k_max]
   DevState *state;
@@ -143,6 +151,7 @@ struct Ctx {
   int device = 0, n_sm = 0;
   int spmv_grid = 0, master_grid = 0;
   size_t master_smem = 0;
+  int master_slab = 0, master_stages = 0, master_z_in_smem = 0;
   bool x_in_smem = true;
   int spmv_ring_warps = 0;      // > 0: the TMA-ring SpMV variant with that many warps per CTA
   // host mirror (pinned) of DevState for the once-per-iteration read-back

@@ -1,32 +1,50 @@
 // dao_master.cu -- step 8, the restricted master problem  min_{y >= 0} F(A y)
-// by gradient projection, kept entirely on the device: ONE persistent cooperative kernel, one
-// CTA per SM, each CTA owning a fixed slab of voxels (so its part of the dense aperture-dose
-// block A stays in the L2 slice it was read from).  Per projected-gradient iteration:
-//   G  z <- z + t dz, g = dF/dz on the slab (tile by tile through shared memory),
-//      grad_k = a_k . g for every aperture k           -> one pass over A, one grid reduction
+// by gradient projection, kept entirely on the device: ONE persistent cooperative kernel, one CTA
+// per SM, each CTA owning a fixed slab of voxels.  The slab's dose z, search image dz (fp64) and
+// structure ids live in shared memory for the whole solve; the dense aperture-dose block A streams
+// through a shared-memory ring filled by a dedicated producer warp with cp.async.bulk (TMA 1-D
+// copies, one 16 KB stage per aperture column and tile), so that ~100 KB per SM are in flight
+// whatever the register count.  Every pass over A reads the same stage sequence, so the producer
+// simply runs ahead: the first stages of the next pass are already resident while the grid
+// reduces.  Per projected-gradient iteration:
+//   G  z <- z + t dz, g = dF/dz on the slab, grad_k = a_k . g   -> one pass over A, one grid reduction
 //   P  every CTA derives the same search direction p (projected steepest descent, optionally
 //      with Polak-Ribiere+ conjugation on the free face) from the reduced gradient
-//   D  dz = A p on the slab, curvature phi''(0)        -> one pass over A, one grid reduction
+//   D  dz = A p on the slab, curvature phi''(0)                  -> one pass over A, one grid reduction
 //   L  safeguarded Newton search for the root of phi'(t) = dz . g(z + t dz) on [0, t_max]
-//                                                       -> passes over (z, dz) only
+//                                                                -> shared memory only
+// Grid reductions carry their data in flagged 16-byte slots ({lo32, epoch, hi32, epoch}): a
+// reader polls the data itself, there is no counter and no separate release/acquire hop.  Small
+// reductions (<= 8 values) are one hop (every CTA reads every CTA's slot); the gradient reduction
+// is two hops (CTA i sums value i over the grid in CTA order and publishes it).  All sums are fp64
+// in a fixed order: bit-reproducible, identical in every CTA.
 // The paper defers the step rule to Men et al. 2009 / Bazaraa et al.; the rule used
-// here is DESIGN.md reading S2.  All reductions are fp64 and in a fixed order (bit-reproducible).
+// here is DESIGN.md reading S2.
 #include "dao_internal.cuh"
+#include "dao_ptx.cuh"
 
 #include <math_constants.h>
+
+#include <algorithm>
 
 namespace dao {
 
 struct MasterParams {
   const float *A;
   int32_t n_vox_pad;
+  int32_t slab;            // voxels per CTA (multiple of 128)
+  int32_t n_stages;        // ring stages of kMasterStageBytes
+  int32_t z_in_smem;       // 1: z, dz, sid of the slab live in shared memory
+  int32_t n_struct;
   const uint8_t *sid;
   const StructEntry *stab;
   double *mz;
   double *mdz;
   double *y;
-  double *part;            // [grid][kMaxRedux]
-  double *result;          // [kMaxRedux]
+  uint4 *ll_part;          // [2][grid][kMaxRedux] flagged slots
+  uint4 *ll_result;        // [2][kMaxRedux]
+  uint32_t *epoch;         // reduction counter, survives dao_reset
+  unsigned long long *prof;  // optional [kMasterProfSlots] phase timers (ns), CTA 0 only
   DevState *st;
   dao_iter_record *history;
   const int32_t *ap_beam;
@@ -38,20 +56,11 @@ struct MasterParams {
 };
 
 constexpr double kLineSearchTol = 1e-4;   // |phi'(t)| <= kLineSearchTol * |phi'(0)| ends the line search
+constexpr int kNW = kMasterWorkers / 32;  // worker warps
 
-__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t *p) {
-  uint32_t v;
-  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ void red_release_add_u32(uint32_t *p, uint32_t v) {
-  asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-__device__ __forceinline__ double warp_sum_d(double v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;
-}
+// ---- small helpers ---------------------------------------------------------------------------
+__device__ __forceinline__ void wsync() { asm volatile("bar.sync 1, %0;" ::"n"(kMasterWorkers) : "memory"); }
+
 __device__ __forceinline__ double warp_max_d(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
@@ -62,81 +71,287 @@ __device__ __forceinline__ double warp_min_d(double v) {
   for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
   return v;
 }
-
-// Grid-wide sum of n (<= kMaxRedux) doubles: every CTA contributes vals[0..n), every CTA gets the
-// totals in out[0..n).  The last CTA to arrive adds the per-CTA partials in CTA order, publishes
-// the result and releases the others (sense = generation counter).  Requires co-resident CTAs
-// (cooperative launch).
-__device__ void grid_reduce(const MasterParams &p, int n, const double *vals, double *out) {
-  __shared__ uint32_t s_gen;
-  __shared__ int s_last;
-  const int tid = threadIdx.x;
-  double *mine = p.part + (size_t)blockIdx.x * kMaxRedux;
-  if (tid < n) mine[tid] = vals[tid];
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) {
-    s_gen = ld_acquire_u32(&p.st->bar_gen);
-    const uint32_t ticket = atomicAdd(&p.st->bar_count, 1u);
-    s_last = (ticket == gridDim.x - 1);
-  }
-  __syncthreads();
-  if (s_last) {
-    __threadfence();
-    // n_pad = n rounded up to a power of two <= blockDim; thread (i, part) adds the partials of the
-    // CTAs b = part, part + P, ... in that order; the P parts of a value are then added in order.
-    int n_pad = 1;
-    while (n_pad < n) n_pad <<= 1;
-    const int P = (int)blockDim.x / n_pad;          // >= 2 (n <= kMaxRedux <= blockDim/2)
-    const int i = tid % n_pad, part = tid / n_pad;
-    double s = 0.0;
-    if (i < n && part < P) {
-      for (unsigned b = part; b < gridDim.x; b += P) s += __ldcg(p.part + (size_t)b * kMaxRedux + i);
-    }
-    __shared__ double s_red[kMasterThreads];
-    s_red[tid] = s;
-    __syncthreads();
-    if (tid < n) {
-      double t = 0.0;
-      for (int q = 0; q < P; ++q) t += s_red[q * n_pad + tid];
-      p.result[tid] = t;
-    }
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) {
-      p.st->bar_count = 0u;
-      __threadfence();
-      red_release_add_u32(&p.st->bar_gen, 1u);
-    }
-  } else {
-    if (tid == 0) {
-      while (ld_acquire_u32(&p.st->bar_gen) == s_gen) { __nanosleep(20); }
-    }
-  }
-  __syncthreads();
-  if (tid < n) out[tid] = __ldcg(p.result + tid);
-  __syncthreads();
+__device__ __forceinline__ unsigned long long gtimer() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
 }
+
+// ---- flagged slots ---------------------------------------------------------------------------
+__device__ __forceinline__ void ll_store(uint4 *slot, double v, uint32_t ep) {
+  const unsigned long long u = (unsigned long long)__double_as_longlong(v);
+  asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(slot), "r"((uint32_t)u), "r"(ep),
+               "r"((uint32_t)(u >> 32)), "r"(ep)
+               : "memory");
+}
+__device__ __forceinline__ uint4 ll_load(const uint4 *slot) {
+  uint4 w;
+  asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w)
+               : "l"(slot)
+               : "memory");
+  return w;
+}
+__device__ __forceinline__ double ll_value(const uint4 &w) {
+  return __longlong_as_double((long long)(((unsigned long long)w.z << 32) | (unsigned long long)w.x));
+}
+
+// One warp sums value `i` of every CTA's slot of this epoch: lane l takes the CTAs l, l+32, ...
+// in that order, then a shuffle tree.  Every lane returns the total.
+constexpr int kMaxGridOver32 = 5;          // supports grids up to 160 CTAs (master_configure caps the grid)
+__device__ __forceinline__ double ll_warp_gather(const uint4 *part /*[grid][kMaxRedux]*/, int i, uint32_t ep,
+                                                 int lane) {
+  const int grid = (int)gridDim.x;
+  uint4 w[kMaxGridOver32];
+#pragma unroll
+  for (int j = 0; j < kMaxGridOver32; ++j) {
+    const int b = lane + 32 * j;
+    if (b < grid) w[j] = ll_load(part + (size_t)b * kMaxRedux + i);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int j = 0; j < kMaxGridOver32; ++j) {
+    const int b = lane + 32 * j;
+    if (b < grid) {
+      while (w[j].y != ep || w[j].w != ep) w[j] = ll_load(part + (size_t)b * kMaxRedux + i);
+      s += ll_value(w[j]);
+    }
+  }
+  return warp_sum_f64(s);
+}
+
+struct Reducer {
+  uint4 *part;      // [2][grid][kMaxRedux]
+  uint4 *result;    // [2][kMaxRedux]
+  uint32_t ep;      // epoch of the last reduction
+
+  // n <= kNW values: every CTA reads every CTA's slot (one hop).  vals/out in shared memory.
+  __device__ __noinline__ void small(int n, const double *vals, double *out) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    ++ep;
+    uint4 *buf = part + (size_t)(ep & 1u) * gridDim.x * kMaxRedux;
+    if (tid < n) ll_store(buf + (size_t)blockIdx.x * kMaxRedux + tid, vals[tid], ep);
+    if (warp < n) {
+      const double s = ll_warp_gather(buf, warp, ep, lane);
+      if (lane == 0) out[warp] = s;
+    }
+    wsync();
+  }
+  // n <= kMaxRedux values: CTA i sums value i (two hops).
+  __device__ __noinline__ void large(int n, const double *vals, double *out) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    ++ep;
+    uint4 *buf = part + (size_t)(ep & 1u) * gridDim.x * kMaxRedux;
+    uint4 *res = result + (size_t)(ep & 1u) * kMaxRedux;
+    if (tid < n) ll_store(buf + (size_t)blockIdx.x * kMaxRedux + tid, vals[tid], ep);
+    // values this CTA owns: i = blockIdx.x + j * gridDim.x, one warp each
+    for (int i = (int)blockIdx.x + warp * (int)gridDim.x; i < n; i += kNW * (int)gridDim.x) {
+      const double s = ll_warp_gather(buf, i, ep, lane);
+      if (lane == 0) ll_store(res + i, s, ep);
+    }
+    if (tid < n) {
+      uint4 w = ll_load(res + tid);
+      while (w.y != ep || w.w != ep) w = ll_load(res + tid);
+      out[tid] = ll_value(w);
+    }
+    wsync();
+  }
+};
 
 // Block-wide sums of NV per-thread doubles -> vals[0..NV) (fixed order: shuffle tree, then warps in order)
 template <int NV>
-__device__ void block_sum(double (&v)[NV], double *scratch /*[nwarps*NV]*/, double *vals) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+__device__ __forceinline__ void block_sum(double (&v)[NV], double *scratch /*[kNW*NV]*/, double *vals) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
-    const double s = warp_sum_d(v[i]);
+    const double s = warp_sum_f64(v[i]);
     if (lane == 0) scratch[warp * NV + i] = s;
   }
-  __syncthreads();
+  wsync();
   if (threadIdx.x < NV) {
     double s = 0.0;
-    for (int w = 0; w < nw; ++w) s += scratch[w * NV + threadIdx.x];
+    for (int w = 0; w < kNW; ++w) s += scratch[w * NV + threadIdx.x];
     vals[threadIdx.x] = s;
   }
-  __syncthreads();
+  wsync();
 }
 
+// Transposed butterfly: every lane holds 8 partial sums d[0..8); afterwards every lane of quad q
+// (= lane >> 2) holds the warp total of value  (q & 1) + 2 ((q >> 1) & 1) + 4 ((q >> 2) & 1)
+// ... i.e. value index bit0 = lane bit 2, bit1 = lane bit 3, bit2 = lane bit 4.  9 shuffles
+// instead of 40.
+__device__ __forceinline__ double butterfly8(const double (&d)[8], int lane) {
+  const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+  double e[4];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const double mine = b4 ? d[j + 4] : d[j], other = b4 ? d[j] : d[j + 4];
+    e[j] = mine + __shfl_xor_sync(0xffffffffu, other, 16);
+  }
+  double f[2];
+#pragma unroll
+  for (int j = 0; j < 2; ++j) {
+    const double mine = b3 ? e[j + 2] : e[j], other = b3 ? e[j] : e[j + 2];
+    f[j] = mine + __shfl_xor_sync(0xffffffffu, other, 8);
+  }
+  double g = (b2 ? f[1] : f[0]) + __shfl_xor_sync(0xffffffffu, b2 ? f[0] : f[1], 4);
+  g += __shfl_xor_sync(0xffffffffu, g, 2);
+  g += __shfl_xor_sync(0xffffffffu, g, 1);
+  return g;
+}
+__device__ __forceinline__ int butterfly8_index(int lane) {
+  return ((lane >> 2) & 1) | (((lane >> 3) & 1) << 1) | (((lane >> 4) & 1) << 2);
+}
+
+
+// Phase P: the search direction from the reduced gradient (one warp; every CTA computes the same).
+__device__ __noinline__ void master_direction(int K, int iters, bool force_restart, int since_restart, int method,
+                                              int max_iter, double tol, double F, double *y_s, double *grad_s,
+                                              double *pg_s, double *pgold_s, double *p_s, double *vals_s, double *sc,
+                                              int *si, unsigned *free_prev_s) {
+  const int lane = threadIdx.x & 31;
+    double pg_max = 0.0, y_max = 1.0, kkt_l = 0.0, num = 0.0, den = 0.0;
+    unsigned free_now[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int k = q * 32 + lane;
+      bool fr = false;
+      if (k < K) {
+        const double gk = grad_s[k], yk = y_s[k];
+        fr = (yk > 0.0) || (gk < 0.0);
+        const double pgk = fr ? -gk : 0.0;
+        pg_s[k] = pgk;
+        pg_max = fmax(pg_max, fabs(pgk));
+        y_max = fmax(y_max, yk);
+        kkt_l = fmax(kkt_l, (yk > 0.0) ? fabs(gk) : fmax(-gk, 0.0));
+        num += pgk * (pgk - pgold_s[k]);
+        den += pgold_s[k] * pgold_s[k];
+      }
+      free_now[q] = __ballot_sync(0xffffffffu, fr);
+    }
+    pg_max = warp_max_d(pg_max);
+    y_max = warp_max_d(y_max);
+    kkt_l = warp_max_d(kkt_l);
+    num = warp_sum_f64(num);
+    den = warp_sum_f64(den);
+    const bool conv = pg_max * y_max <= tol * fmax(F, 1e-300);
+    const bool stop = conv || iters >= max_iter;
+    bool same_free = true;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) same_free = same_free && (free_now[q] == free_prev_s[q]);
+    bool restart = force_restart || !same_free || method == 0 || since_restart >= K + 8 || !(den > 0.0);
+    double beta = 0.0;
+    if (!restart) beta = fmax(num / den, 0.0);
+    if (beta == 0.0) restart = true;
+    // direction, rounded to fp32-representable values
+    double slope = 0.0;
+    bool infeasible = false;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int k = q * 32 + lane;
+      if (k < K) {
+        double pk = pg_s[k];
+        if (!restart && pk != 0.0) pk = fma(beta, p_s[k], pk);
+        if (!restart && pg_s[k] == 0.0) pk = 0.0;
+        pk = (double)(float)pk;
+        if (pk < 0.0 && !(y_s[k] > 0.0)) infeasible = true;
+        slope = fma(pk, grad_s[k], slope);
+        vals_s[k] = pk;     // tentative
+      }
+    }
+    slope = warp_sum_f64(slope);
+    infeasible = __any_sync(0xffffffffu, infeasible);
+    if (!restart && (infeasible || !(slope < 0.0))) {
+      restart = true;
+      slope = 0.0;
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const int k = q * 32 + lane;
+        if (k < K) {
+          const double pk = (double)(float)pg_s[k];
+          slope = fma(pk, grad_s[k], slope);
+          vals_s[k] = pk;
+        }
+      }
+      slope = warp_sum_f64(slope);
+    }
+    double tmax = CUDART_INF;
+    int kb = 0x7fffffff;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int k = q * 32 + lane;
+      if (k < K) {
+        const double pk = vals_s[k];
+        p_s[k] = pk;
+        pgold_s[k] = pg_s[k];
+        if (pk < 0.0) {
+          const double tk = y_s[k] / (-pk);
+          if (tk < tmax) { tmax = tk; kb = k; }
+        }
+      }
+    }
+    {
+      const double tmin = warp_min_d(tmax);
+      const unsigned m = __ballot_sync(0xffffffffu, tmax == tmin && kb != 0x7fffffff);
+      int kb_w = 0x7fffffff;
+      if (m) {
+        // smallest k among the lanes that attain the minimum
+        int cand_k = (tmax == tmin) ? kb : 0x7fffffff;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) cand_k = min(cand_k, __shfl_xor_sync(0xffffffffu, cand_k, o));
+        kb_w = cand_k;
+      }
+      tmax = tmin;
+      kb = kb_w;
+    }
+    if (lane == 0) {
+      sc[1] = slope; sc[2] = tmax; sc[3] = pg_max; sc[4] = kkt_l;
+      si[0] = stop ? 1 : 0; si[1] = (stop && !conv) ? 1 : 0; si[2] = kb; si[3] = restart ? 1 : 0;
+      si[4] = (!(slope < 0.0)) ? 1 : 0;
+    }
+    if (lane == 0) {
+#pragma unroll
+      for (int q = 0; q < 4; ++q) free_prev_s[q] = free_now[q];
+    }
+}
+
+// ---- the A stream ----------------------------------------------------------------------------
+// Stage sequence of ONE pass: for tile (kMasterTileVox voxels of the slab) { for k < K { A[k][tile] } }.
+// The producer repeats that sequence for ever; consumers walk it with the same counters.
+struct RingPos {
+  int stage;
+  uint32_t phase;
+  __device__ __forceinline__ void advance(int n_stages) {
+    if (++stage == n_stages) { stage = 0; phase ^= 1u; }
+  }
+};
+
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(smem_addr(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
+}
+
+struct MasterSmem {          // carved from dynamic shared memory by every thread identically
+  unsigned char *ring;       // [n_stages][kMasterStageBytes]
+  uint64_t *full, *empty;    // [n_stages]
+  double *zs, *dzs;          // [slab] (shared or this CTA's part of the global arrays)
+  const uint8_t *sids;       // [slab]
+  StructEntry *stab;         // [n_struct]
+  double *warp_part;         // [kNW][kpad]
+};
+
 __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
+  extern __shared__ __align__(128) unsigned char dyn_smem[];
   // ---- shared state (replicated in every CTA, evolves identically everywhere) ----
   __shared__ double y_s[DAO_MAX_APERTURES];
   __shared__ double grad_s[kMaxRedux];
@@ -145,16 +360,15 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
   __shared__ double p_s[DAO_MAX_APERTURES];        // search direction (fp32-representable values)
   __shared__ double vals_s[kMaxRedux];
   __shared__ double red_s[kMaxRedux];
-  __shared__ double g_tile[kMasterTile];
-  // per-warp partials; aliases g_tile (only used once the tile loop of a phase is over)
-  static_assert(kMasterTile >= (kMasterThreads / 32) * DAO_MAX_APERTURES, "warp_part must fit in g_tile");
-  double *warp_part = g_tile;
-  __shared__ StructEntry stab_s[256];
+  __shared__ double scratch_s[kNW * 4];
   __shared__ double sc[16];                        // broadcast scalars
   __shared__ int si[8];
+  __shared__ unsigned free_prev_s[4];
+  __shared__ volatile int s_stop;
+  __shared__ volatile unsigned s_consumed_stage, s_consumed_phase;
+  __shared__ unsigned long long prof_s[kMasterProfSlots];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  constexpr int NW = kMasterThreads / 32;
   const int K0 = p.st->K;
   const int cand = p.st->cand_valid;
   const int added = (p.add_candidate && cand) ? 1 : 0;
@@ -164,238 +378,262 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
     return;
   }
 
-  for (int i = tid; i < 256; i += blockDim.x) stab_s[i] = p.stab[i];
+  // slab of voxels owned by this CTA
+  const int vpad = p.n_vox_pad;
+  const long long v0l = (long long)blockIdx.x * p.slab;
+  const int v0 = (int)(v0l < vpad ? v0l : vpad);
+  const int v1 = (v0 + p.slab < vpad) ? v0 + p.slab : vpad;
+  const int slab_len = v1 - v0;                                      // multiple of 128 (vpad is)
+  const int n_tiles = (slab_len + kMasterTileVox - 1) / kMasterTileVox;
+  const int NS = p.n_stages;
+
+  MasterSmem sm;
+  {
+    unsigned char *q = dyn_smem;
+    sm.ring = q; q += (size_t)NS * kMasterStageBytes;
+    sm.full = reinterpret_cast<uint64_t *>(q); q += align_up_c((size_t)NS * 8, 128);
+    sm.empty = reinterpret_cast<uint64_t *>(q); q += align_up_c((size_t)NS * 8, 128);
+    sm.stab = reinterpret_cast<StructEntry *>(q); q += align_up_c((size_t)p.n_struct * sizeof(StructEntry), 128);
+    sm.warp_part = reinterpret_cast<double *>(q); q += (size_t)kNW * DAO_MAX_APERTURES * 8;
+    if (p.z_in_smem) {
+      sm.zs = reinterpret_cast<double *>(q); q += (size_t)p.slab * 8;
+      sm.dzs = reinterpret_cast<double *>(q); q += (size_t)p.slab * 8;
+      sm.sids = q;
+    } else {
+      sm.zs = p.mz + v0; sm.dzs = p.mdz + v0; sm.sids = p.sid + v0;
+    }
+  }
+  if (tid == 0) {
+    for (int s = 0; s < NS; ++s) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], kNW); }
+    s_stop = 0;
+    for (int i = 0; i < kMasterProfSlots; ++i) prof_s[i] = 0ull;
+  }
+  fence_mbar_init();
+  __syncthreads();
+
+  // =============================== producer warp ================================================
+  if (warp == kNW) {
+    if (lane == 0) {
+      RingPos pp{0, 0u};
+      bool first_round = true;
+      bool stop = slab_len == 0;
+      while (!stop) {
+        for (int tile = 0; tile < n_tiles && !stop; ++tile) {
+          const int t0 = tile * kMasterTileVox;
+          const uint32_t bytes = (uint32_t)min(kMasterTileVox, slab_len - t0) * 4u;
+          const float *src = p.A + (size_t)v0 + (size_t)t0;
+          for (int k = 0; k < K; ++k) {
+            if (!first_round) {
+              while (!mbar_try_wait(&sm.empty[pp.stage], pp.phase ^ 1u)) {
+                if (s_stop) { stop = true; break; }
+              }
+              if (stop) break;
+            }
+            mbar_arrive_expect_tx(&sm.full[pp.stage], bytes);
+            bulk_g2s(sm.ring + (size_t)pp.stage * kMasterStageBytes, src + (size_t)k * vpad, bytes, &sm.full[pp.stage]);
+            pp.advance(NS);
+            if (pp.stage == 0) first_round = false;
+          }
+        }
+      }
+      if (slab_len == 0) {
+        while (!s_stop) { __nanosleep(200); }
+      } else {
+        // drain: every issued stage must have landed before the CTA may exit
+        while (!s_stop) { __nanosleep(100); }
+        RingPos cp{(int)s_consumed_stage, s_consumed_phase};
+        while (cp.stage != pp.stage || cp.phase != pp.phase) {
+          mbar_wait(&sm.full[cp.stage], cp.phase);
+          cp.advance(NS);
+        }
+      }
+    }
+    __syncthreads();     // matches the final barrier of the workers
+    return;
+  }
+
+  // =============================== worker warps =================================================
+  for (int i = tid; i < p.n_struct; i += kMasterWorkers) sm.stab[i] = p.stab[i];
   if (tid < DAO_MAX_APERTURES) {
     y_s[tid] = (tid < K0) ? p.y[tid] : 0.0;
     pgold_s[tid] = 0.0;
     p_s[tid] = 0.0;
   }
-  __syncthreads();
+  if (tid < 4) free_prev_s[tid] = 0u;
+  if (p.z_in_smem) {
+    uint8_t *sids = const_cast<uint8_t *>(sm.sids);
+    for (int i = tid; i < slab_len; i += kMasterWorkers) sids[i] = p.sid[v0 + i];
+  }
+  Reducer red{p.ll_part, p.ll_result, 0u};
+  if (tid == 0) si[7] = (int)*p.epoch;
+  wsync();
+  red.ep = (uint32_t)si[7];
 
-  // slab of voxels owned by this CTA (multiple of 128 so that every warp strip is full)
-  const int vpad = p.n_vox_pad;
-  int slab = (vpad + (int)gridDim.x - 1) / (int)gridDim.x;
-  slab = (slab + 127) / 128 * 128;
-  const long long v0l = (long long)blockIdx.x * slab;
-  const int v0 = (int)(v0l < vpad ? v0l : vpad);
-  const int v1 = (v0 + slab < vpad) ? v0 + slab : vpad;
+  const bool prof = (p.prof != nullptr) && blockIdx.x == 0 && tid == 0;
+  unsigned long long tprof = prof ? gtimer() : 0ull;
+#define PROF_MARK(slot)                                   \
+  do {                                                    \
+    if (prof) {                                           \
+      const unsigned long long now_ = gtimer();           \
+      prof_s[slot] += now_ - tprof;                       \
+      tprof = now_;                                       \
+    }                                                     \
+  } while (0)
+
+  RingPos cp{0, 0u};                       // consumer position in the A stream
+  // strips of this warp inside a tile: warp and warp + kNW (128 voxels each, 4 per lane)
+  const int l0 = warp * 128 + lane * 4, l1 = (warp + kNW) * 128 + lane * 4;
+
+  // one D-type pass: out[i] = sum_k coef[k] A[k][i] on the slab (fp64, k ascending)
+  auto pass_d = [&](const double *coef, double *out) {
+    for (int tile = 0; tile < n_tiles; ++tile) {
+      const int t0 = tile * kMasterTileVox;
+      const int tn = min(kMasterTileVox, slab_len - t0);
+      const bool a0 = l0 < tn, a1 = l1 < tn;
+      double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+      for (int k = 0; k < K; ++k) {
+        const double ck = coef[k];
+        mbar_wait(&sm.full[cp.stage], cp.phase);
+        if (ck != 0.0) {
+          const unsigned char *st = sm.ring + (size_t)cp.stage * kMasterStageBytes;
+          if (a0) {
+            const float4 a = *reinterpret_cast<const float4 *>(st + (size_t)l0 * 4);
+            acc[0] = fma(ck, (double)a.x, acc[0]); acc[1] = fma(ck, (double)a.y, acc[1]);
+            acc[2] = fma(ck, (double)a.z, acc[2]); acc[3] = fma(ck, (double)a.w, acc[3]);
+          }
+          if (a1) {
+            const float4 a = *reinterpret_cast<const float4 *>(st + (size_t)l1 * 4);
+            acc[4] = fma(ck, (double)a.x, acc[4]); acc[5] = fma(ck, (double)a.y, acc[5]);
+            acc[6] = fma(ck, (double)a.z, acc[6]); acc[7] = fma(ck, (double)a.w, acc[7]);
+          }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&sm.empty[cp.stage]);
+        cp.advance(NS);
+      }
+      if (a0) {
+        double2 *o = reinterpret_cast<double2 *>(out + t0 + l0);
+        o[0] = make_double2(acc[0], acc[1]); o[1] = make_double2(acc[2], acc[3]);
+      }
+      if (a1) {
+        double2 *o = reinterpret_cast<double2 *>(out + t0 + l1);
+        o[0] = make_double2(acc[4], acc[5]); o[1] = make_double2(acc[6], acc[7]);
+      }
+    }
+  };
 
   // ---- z = A y on the slab (fp64), dz = 0 ----
-  for (int v = v0 + tid * 4; v < v1; v += blockDim.x * 4) {
-    double a0 = 0, a1 = 0, a2 = 0, a3 = 0;
-    for (int k = 0; k < K; ++k) {
-      const double yk = y_s[k];
-      if (yk == 0.0) continue;
-      const float4 a = *reinterpret_cast<const float4 *>(p.A + (size_t)k * vpad + v);
-      a0 = fma(yk, (double)a.x, a0); a1 = fma(yk, (double)a.y, a1);
-      a2 = fma(yk, (double)a.z, a2); a3 = fma(yk, (double)a.w, a3);
+  {
+    bool any = false;
+    for (int k = 0; k < K0; ++k) any = any || (y_s[k] != 0.0);
+    if (any) {
+      pass_d(y_s, sm.zs);
+    } else {
+      for (int i = tid; i < slab_len; i += kMasterWorkers) sm.zs[i] = 0.0;
     }
-    p.mz[v] = a0; p.mz[v + 1] = a1; p.mz[v + 2] = a2; p.mz[v + 3] = a3;
-    p.mdz[v] = 0.0; p.mdz[v + 1] = 0.0; p.mdz[v + 2] = 0.0; p.mdz[v + 3] = 0.0;
+    for (int i = tid; i < slab_len; i += kMasterWorkers) sm.dzs[i] = 0.0;
   }
-  __syncthreads();
+  wsync();
+  PROF_MARK(0);
 
   double t_step = 0.0;          // step to apply to z at the start of the next G phase
   int iters = 0, restarts = 0, since_restart = 0;
   bool force_restart = true;
-  unsigned free_prev[4] = {0u, 0u, 0u, 0u};
   int hit_max = 0;
   double F = 0.0, kkt = 0.0, pgmax = 0.0;
 
   for (;;) {
     // ================= phase G: z += t dz, g(z), grad = A^T g, F ==========================
-    double accq[4] = {0.0, 0.0, 0.0, 0.0};   // lane l holds grad partials of k = q*32 + l (this warp's strips)
     double f_acc = 0.0;
-    for (int tile0 = v0; tile0 < v1; tile0 += kMasterTile) {
-      const int tn = (v1 - tile0 < kMasterTile) ? (v1 - tile0) : kMasterTile;
-      for (int i = tid; i < tn; i += blockDim.x) {
-        const int v = tile0 + i;
-        double z = p.mz[v];
-        if (t_step != 0.0) { z = fma(t_step, p.mdz[v], z); p.mz[v] = z; }
-        const int s = p.sid[v];
-        double gv = 0.0;
-        if (s != kNoStruct) {
-          const StructEntry e = stab_s[s];
-          const double u = fmax(e.tm - z, 0.0), o = fmax(z - e.tp, 0.0);
-          f_acc += e.a * u * u + e.b * o * o;
-          gv = -2.0 * e.a * u + 2.0 * e.b * o;
-        }
-        g_tile[i] = gv;
-      }
-      __syncthreads();
-      // warp `warp` owns the 128-voxel strips warp, warp+NW, ... of the tile; lane owns 4 voxels
-      for (int s0 = warp * 128; s0 < tn; s0 += NW * 128) {
-        const int vi = s0 + lane * 4;
-        const double g0 = g_tile[vi], g1 = g_tile[vi + 1], g2 = g_tile[vi + 2], g3 = g_tile[vi + 3];
-        const float *base = p.A + (size_t)(tile0 + vi);
+    for (int tile = 0; tile < n_tiles; ++tile) {
+      const int t0 = tile * kMasterTileVox;
+      const int tn = min(kMasterTileVox, slab_len - t0);
+      const bool a0 = l0 < tn, a1 = l1 < tn;
+      double g[8];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const int kq = q * 32;
-          if (kq >= K) break;
-          const int kn = (K - kq < 32) ? (K - kq) : 32;
-          int l = 0;
-          for (; l + 4 <= kn; l += 4) {
-            float4 a[4];
+      for (int h = 0; h < 2; ++h) {
+        const bool act = h ? a1 : a0;
+        const int i0 = t0 + (h ? l1 : l0);
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
-              a[u] = *reinterpret_cast<const float4 *>(base + (size_t)(kq + l + u) * vpad);
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-              double d = (double)a[u].x * g0;
-              d = fma((double)a[u].y, g1, d);
-              d = fma((double)a[u].z, g2, d);
-              d = fma((double)a[u].w, g3, d);
-              d = warp_sum_d(d);
-              if (lane == l + u) accq[q] += d;
+        for (int u = 0; u < 4; ++u) {
+          double gv = 0.0;
+          if (act) {
+            double z = sm.zs[i0 + u];
+            if (t_step != 0.0) { z = fma(t_step, sm.dzs[i0 + u], z); sm.zs[i0 + u] = z; }
+            const int s = sm.sids[i0 + u];
+            if (s != kNoStruct) {
+              const StructEntry e = sm.stab[s];
+              const double un = fmax(e.tm - z, 0.0), ov = fmax(z - e.tp, 0.0);
+              f_acc += e.a * un * un + e.b * ov * ov;
+              gv = -2.0 * e.a * un + 2.0 * e.b * ov;
             }
           }
-          for (; l < kn; ++l) {
-            const float4 a = *reinterpret_cast<const float4 *>(base + (size_t)(kq + l) * vpad);
-            double d = (double)a.x * g0;
-            d = fma((double)a.y, g1, d);
-            d = fma((double)a.z, g2, d);
-            d = fma((double)a.w, g3, d);
-            d = warp_sum_d(d);
-            if (lane == l) accq[q] += d;
-          }
+          g[h * 4 + u] = gv;
         }
       }
-      __syncthreads();
-    }
-    // combine the warps of the CTA in warp order
+      for (int kb = 0; kb < K; kb += 8) {
+        double d[8];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      const int k = q * 32 + lane;
-      if (k < K) warp_part[warp * DAO_MAX_APERTURES + k] = accq[q];
+        for (int j = 0; j < 8; ++j) {
+          d[j] = 0.0;
+          if (kb + j < K) {
+            mbar_wait(&sm.full[cp.stage], cp.phase);
+            const unsigned char *st = sm.ring + (size_t)cp.stage * kMasterStageBytes;
+            if (a0) {
+              const float4 a = *reinterpret_cast<const float4 *>(st + (size_t)l0 * 4);
+              double q = (double)a.x * g[0];
+              q = fma((double)a.y, g[1], q); q = fma((double)a.z, g[2], q); q = fma((double)a.w, g[3], q);
+              d[j] = q;
+            }
+            if (a1) {
+              const float4 a = *reinterpret_cast<const float4 *>(st + (size_t)l1 * 4);
+              double q = (double)a.x * g[4];
+              q = fma((double)a.y, g[5], q); q = fma((double)a.z, g[6], q); q = fma((double)a.w, g[7], q);
+              d[j] += q;
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sm.empty[cp.stage]);
+            cp.advance(NS);
+          }
+        }
+        const double r = butterfly8(d, lane);
+        const int kk = kb + butterfly8_index(lane);
+        if ((lane & 3) == 0) {
+          double *slot = sm.warp_part + warp * DAO_MAX_APERTURES + kk;
+          *slot = (tile == 0) ? r : (*slot + r);
+        }
+      }
     }
     {
-      const double fs = warp_sum_d(f_acc);
-      if (lane == 0) red_s[warp] = fs;
+      const double fs = warp_sum_f64(f_acc);
+      if (lane == 0) scratch_s[warp] = fs;
     }
-    __syncthreads();
+    wsync();
     if (tid < K) {
       double s = 0.0;
-      for (int w = 0; w < NW; ++w) s += warp_part[w * DAO_MAX_APERTURES + tid];
+      if (n_tiles > 0)
+        for (int w = 0; w < kNW; ++w) s += sm.warp_part[w * DAO_MAX_APERTURES + tid];
       vals_s[tid] = s;
     }
     if (tid == K) {
       double s = 0.0;
-      for (int w = 0; w < NW; ++w) s += red_s[w];
+      for (int w = 0; w < kNW; ++w) s += scratch_s[w];
       vals_s[K] = s;
     }
-    __syncthreads();
-    grid_reduce(p, K + 1, vals_s, grad_s /* K grads, then F */);
-    if (tid == 0) sc[0] = grad_s[K];
-    __syncthreads();
-    F = sc[0];
+    wsync();
+    PROF_MARK(1);
+    red.large(K + 1, vals_s, grad_s /* K grads, then F */);
+    F = grad_s[K];
+    PROF_MARK(2);
 
     // ================= phase P: direction (warp 0, identical in every CTA) ================
-    if (warp == 0) {
-      double pg_max = 0.0, y_max = 1.0, kkt_l = 0.0, num = 0.0, den = 0.0;
-      unsigned free_now[4] = {0u, 0u, 0u, 0u};
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const int k = q * 32 + lane;
-        bool fr = false;
-        if (k < K) {
-          const double gk = grad_s[k], yk = y_s[k];
-          fr = (yk > 0.0) || (gk < 0.0);
-          const double pgk = fr ? -gk : 0.0;
-          pg_s[k] = pgk;
-          pg_max = fmax(pg_max, fabs(pgk));
-          y_max = fmax(y_max, yk);
-          kkt_l = fmax(kkt_l, (yk > 0.0) ? fabs(gk) : fmax(-gk, 0.0));
-          num += pgk * (pgk - pgold_s[k]);
-          den += pgold_s[k] * pgold_s[k];
-        }
-        free_now[q] = __ballot_sync(0xffffffffu, fr);
-      }
-      pg_max = warp_max_d(pg_max);
-      y_max = warp_max_d(y_max);
-      kkt_l = warp_max_d(kkt_l);
-      num = warp_sum_d(num);
-      den = warp_sum_d(den);
-      const bool conv = pg_max * y_max <= p.tol * fmax(F, 1e-300);
-      const bool stop = conv || iters >= p.max_iter;
-      bool same_free = true;
-#pragma unroll
-      for (int q = 0; q < 4; ++q) same_free = same_free && (free_now[q] == free_prev[q]);
-      bool restart = force_restart || !same_free || p.method == 0 || since_restart >= K + 8 || !(den > 0.0);
-      double beta = 0.0;
-      if (!restart) beta = fmax(num / den, 0.0);
-      if (beta == 0.0) restart = true;
-      // direction, rounded to fp32-representable values
-      double slope = 0.0;
-      bool infeasible = false;
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const int k = q * 32 + lane;
-        if (k < K) {
-          double pk = pg_s[k];
-          if (!restart && pk != 0.0) pk = fma(beta, p_s[k], pk);
-          if (!restart && pg_s[k] == 0.0) pk = 0.0;
-          pk = (double)(float)pk;
-          if (pk < 0.0 && !(y_s[k] > 0.0)) infeasible = true;
-          slope = fma(pk, grad_s[k], slope);
-          vals_s[k] = pk;     // tentative
-        }
-      }
-      slope = warp_sum_d(slope);
-      infeasible = __any_sync(0xffffffffu, infeasible);
-      if (!restart && (infeasible || !(slope < 0.0))) {
-        restart = true;
-        slope = 0.0;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const int k = q * 32 + lane;
-          if (k < K) {
-            const double pk = (double)(float)pg_s[k];
-            slope = fma(pk, grad_s[k], slope);
-            vals_s[k] = pk;
-          }
-        }
-        slope = warp_sum_d(slope);
-      }
-      double tmax = CUDART_INF;
-      int kb = 0x7fffffff;
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const int k = q * 32 + lane;
-        if (k < K) {
-          const double pk = vals_s[k];
-          p_s[k] = pk;
-          pgold_s[k] = pg_s[k];
-          if (pk < 0.0) {
-            const double tk = y_s[k] / (-pk);
-            if (tk < tmax) { tmax = tk; kb = k; }
-          }
-        }
-      }
-      {
-        const double tmin = warp_min_d(tmax);
-        const unsigned m = __ballot_sync(0xffffffffu, tmax == tmin && kb != 0x7fffffff);
-        int kb_w = 0x7fffffff;
-        if (m) {
-          // smallest k among the lanes that attain the minimum
-          int cand_k = (tmax == tmin) ? kb : 0x7fffffff;
-#pragma unroll
-          for (int o = 16; o > 0; o >>= 1) cand_k = min(cand_k, __shfl_xor_sync(0xffffffffu, cand_k, o));
-          kb_w = cand_k;
-        }
-        tmax = tmin;
-        kb = kb_w;
-      }
-      if (lane == 0) {
-        sc[1] = slope; sc[2] = tmax; sc[3] = pg_max; sc[4] = kkt_l;
-        si[0] = stop ? 1 : 0; si[1] = (stop && !conv) ? 1 : 0; si[2] = kb; si[3] = restart ? 1 : 0;
-        si[4] = (!(slope < 0.0)) ? 1 : 0;
-      }
-#pragma unroll
-      for (int q = 0; q < 4; ++q) free_prev[q] = free_now[q];
-    }
-    __syncthreads();
+    if (warp == 0)
+      master_direction(K, iters, force_restart, since_restart, p.method, p.max_iter, p.tol, F, y_s, grad_s, pg_s,
+                       pgold_s, p_s, vals_s, sc, si, free_prev_s);
+    wsync();
     pgmax = sc[3];
     kkt = sc[4];
+    PROF_MARK(3);
     if (si[0] || si[4]) { hit_max = si[1]; break; }   // converged, iteration cap, or no descent left
     const double slope0 = sc[1], tmax = sc[2];
     const int kb = si[2];
@@ -403,48 +641,37 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
     force_restart = false;
 
     // ================= phase D: dz = A p, curvature =======================================
+    pass_d(p_s, sm.dzs);
     double h_acc = 0.0;
-    for (int vb = v0 + warp * 128; vb < v1; vb += NW * 128) {
-      const int v = vb + lane * 4;
-      const float *base = p.A + (size_t)v;
-      double d0 = 0, d1 = 0, d2 = 0, d3 = 0;
-      int k = 0;
-      for (; k + 4 <= K; k += 4) {
-        float4 a[4];
+    for (int tile = 0; tile < n_tiles; ++tile) {
+      const int t0 = tile * kMasterTileVox;
+      const int tn = min(kMasterTileVox, slab_len - t0);
 #pragma unroll
-        for (int u = 0; u < 4; ++u) a[u] = *reinterpret_cast<const float4 *>(base + (size_t)(k + u) * vpad);
+      for (int h = 0; h < 2; ++h) {
+        const int li = h ? l1 : l0;
+        if (li < tn) {
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const double pk = p_s[k + u];
-          d0 = fma(pk, (double)a[u].x, d0); d1 = fma(pk, (double)a[u].y, d1);
-          d2 = fma(pk, (double)a[u].z, d2); d3 = fma(pk, (double)a[u].w, d3);
-        }
-      }
-      for (; k < K; ++k) {
-        const float4 a = *reinterpret_cast<const float4 *>(base + (size_t)k * vpad);
-        const double pk = p_s[k];
-        d0 = fma(pk, (double)a.x, d0); d1 = fma(pk, (double)a.y, d1);
-        d2 = fma(pk, (double)a.z, d2); d3 = fma(pk, (double)a.w, d3);
-      }
-      const double dd[4] = {d0, d1, d2, d3};
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        p.mdz[v + u] = dd[u];
-        const int s = p.sid[v + u];
-        if (s != kNoStruct) {
-          const StructEntry e = stab_s[s];
-          const double z = p.mz[v + u];
-          const double c = (z < e.tm ? e.a : 0.0) + (z > e.tp ? e.b : 0.0);
-          h_acc = fma(2.0 * c * dd[u], dd[u], h_acc);
+          for (int u = 0; u < 4; ++u) {
+            const int i = t0 + li + u;
+            const int s = sm.sids[i];
+            if (s != kNoStruct) {
+              const StructEntry e = sm.stab[s];
+              const double z = sm.zs[i], dd = sm.dzs[i];
+              const double c = (z < e.tm ? e.a : 0.0) + (z > e.tp ? e.b : 0.0);
+              h_acc = fma(2.0 * c * dd, dd, h_acc);
+            }
+          }
         }
       }
     }
     {
       double hv[1] = {h_acc};
-      block_sum<1>(hv, warp_part, vals_s);
+      block_sum<1>(hv, scratch_s, vals_s);
     }
-    grid_reduce(p, 1, vals_s, red_s);
+    PROF_MARK(4);
+    red.small(1, vals_s, red_s);
     const double h0 = red_s[0];
+    PROF_MARK(5);
 
     // ================= phase L: root of phi'(t) on [0, tmax] ==============================
     // phi' is non-decreasing and piecewise linear; phi'(0) = slope0 < 0.
@@ -454,12 +681,12 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
     bool hit_bound = false;
     for (int ls = 0; ls < 40; ++ls) {
       double acc3[3] = {0.0, 0.0, 0.0};   // phi'(t), phi''(t), F(t)
-      for (int v = v0 + tid; v < v1; v += blockDim.x) {
-        const int s = p.sid[v];
+      for (int i = tid; i < slab_len; i += kMasterWorkers) {
+        const int s = sm.sids[i];
         if (s == kNoStruct) continue;
-        const StructEntry e = stab_s[s];
-        const double dz = p.mdz[v];
-        const double z = fma(t, dz, p.mz[v]);
+        const StructEntry e = sm.stab[s];
+        const double dz = sm.dzs[i];
+        const double z = fma(t, dz, sm.zs[i]);
         const double u = fmax(e.tm - z, 0.0), o = fmax(z - e.tp, 0.0);
         const double gv = -2.0 * e.a * u + 2.0 * e.b * o;
         const double c = (u > 0.0 ? e.a : 0.0) + (o > 0.0 ? e.b : 0.0);
@@ -467,8 +694,9 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
         acc3[1] = fma(2.0 * c * dz, dz, acc3[1]);
         acc3[2] += e.a * u * u + e.b * o * o;
       }
-      block_sum<3>(acc3, warp_part, vals_s);
-      grid_reduce(p, 3, vals_s, red_s);
+      block_sum<3>(acc3, scratch_s, vals_s);
+      red.small(3, vals_s, red_s);
+      if (prof) ++prof_s[7];
       const double s1 = red_s[0], s2 = red_s[1];
       if (fabs(s1) <= kLineSearchTol * fabs(slope0)) break;      // exact enough
       double tn;
@@ -498,13 +726,30 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
     if (hit_bound) force_restart = true;
     t_step = t;
     ++iters;
-    __syncthreads();
+    wsync();
+    PROF_MARK(6);
   }
 
   // ---- publish ----
+  if (p.z_in_smem) {
+    for (int i = tid; i < slab_len; i += kMasterWorkers) { p.mz[v0 + i] = sm.zs[i]; p.mdz[v0 + i] = sm.dzs[i]; }
+  }
+  if (tid == 0) {
+    s_consumed_stage = (unsigned)cp.stage;
+    s_consumed_phase = cp.phase;
+    __threadfence_block();
+    s_stop = 1;
+  }
   if (blockIdx.x == 0) {
     if (tid < K) p.y[tid] = y_s[tid];
     if (tid == 0) {
+      *p.epoch = red.ep;
+      if (p.prof) {
+        prof_s[8] += (unsigned long long)iters;
+        prof_s[9] += 1ull;
+        PROF_MARK(10);
+        for (int i = 0; i < kMasterProfSlots; ++i) p.prof[i] += prof_s[i];
+      }
       DevState *st = p.st;
       st->K = K;
       st->m_iters = iters;
@@ -530,14 +775,49 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
       }
     }
   }
+#undef PROF_MARK
+  __syncthreads();       // the producer warp joins after draining the ring
+}
+
+// Shared-memory plan: static tables + ring + (when it fits) the slab's z, dz, sid.
+static size_t master_fixed_smem(const Ctx *c, int n_stages) {
+  return (size_t)n_stages * kMasterStageBytes + 2 * align_up((size_t)n_stages * 8, 128) +
+         align_up((size_t)std::max(c->n_struct, 1) * sizeof(StructEntry), 128) + (size_t)kNW * DAO_MAX_APERTURES * 8;
 }
 
 cudaError_t master_configure(Ctx *c) {
+  c->master_grid = std::min(c->n_sm, 32 * kMaxGridOver32);      // one CTA per SM
+  int slab = (c->n_vox_pad + c->master_grid - 1) / c->master_grid;
+  slab = (slab + 127) / 128 * 128;
+  c->master_slab = slab;
+  cudaFuncAttributes fa;
+  cudaError_t e = cudaFuncGetAttributes(&fa, k_master);
+  if (e != cudaSuccess) return e;
+  int max_optin = 0;
+  e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device);
+  if (e != cudaSuccess) return e;
+  const size_t budget = (size_t)max_optin - fa.sharedSizeBytes - 1024;
+  const size_t slab_bytes = (size_t)slab * 17;
+  // prefer z in shared memory with >= 4 stages; otherwise z stays in global memory (L2)
+  c->master_z_in_smem = 0;
+  int stages = 0;
+  if (master_fixed_smem(c, 4) + slab_bytes <= budget) {
+    c->master_z_in_smem = 1;
+    stages = 4;
+    while (stages < kMasterMaxStages && master_fixed_smem(c, stages + 1) + slab_bytes <= budget) ++stages;
+  } else {
+    stages = 2;
+    while (stages < kMasterMaxStages && master_fixed_smem(c, stages + 1) <= budget) ++stages;
+    if (master_fixed_smem(c, stages) > budget) return cudaErrorLaunchOutOfResources;
+  }
+  c->master_stages = stages;
+  c->master_smem = master_fixed_smem(c, stages) + (c->master_z_in_smem ? align_up(slab_bytes, 128) : 0);
+  e = cudaFuncSetAttribute(k_master, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->master_smem);
+  if (e != cudaSuccess) return e;
   int nb = 0;
-  cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_master, kMasterThreads, 0);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_master, kMasterThreads, c->master_smem);
   if (e != cudaSuccess) return e;
   if (nb < 1) return cudaErrorLaunchOutOfResources;
-  c->master_grid = c->n_sm;      // one CTA per SM
   return cudaSuccess;
 }
 
@@ -545,13 +825,19 @@ cudaError_t launch_master(Ctx *c, bool add_candidate) {
   MasterParams p{};
   p.A = c->d.A;
   p.n_vox_pad = c->n_vox_pad;
+  p.slab = c->master_slab;
+  p.n_stages = c->master_stages;
+  p.z_in_smem = c->master_z_in_smem;
+  p.n_struct = std::max(c->n_struct, 1);
   p.sid = c->d.sid;
   p.stab = c->d.stab;
   p.mz = c->d.mz;
   p.mdz = c->d.mdz;
   p.y = c->d.y;
-  p.part = c->d.m_part;
-  p.result = c->d.m_result;
+  p.ll_part = c->d.ll_part;
+  p.ll_result = c->d.ll_result;
+  p.epoch = c->d.m_epoch;
+  p.prof = (c->opt.reserved & 2) ? c->d.m_prof : nullptr;
   p.st = c->d.state;
   p.history = c->d.history;
   p.ap_beam = c->d.ap_beam;
@@ -561,8 +847,8 @@ cudaError_t launch_master(Ctx *c, bool add_candidate) {
   p.k_max = c->opt.k_max;
   p.tol = c->opt.master_tol;
   void *args[] = {&p};
-  return cudaLaunchCooperativeKernel((void *)k_master, dim3(c->master_grid), dim3(kMasterThreads), args, 0,
-                                     c->stream);
+  return cudaLaunchCooperativeKernel((void *)k_master, dim3(c->master_grid), dim3(kMasterThreads), args,
+                                     c->master_smem, c->stream);
 }
 
 }  // namespace dao

@@ -136,8 +136,10 @@ static void carve_workspace(Carver &cv, const Dims &dm, const HostLayout &L, Dev
   d->y = cv.take<double>((size_t)DAO_MAX_APERTURES);
   d->mz = cv.take<double>(vp);
   d->mdz = cv.take<double>(vp);
-  d->m_part = cv.take<double>((size_t)(n_sm + 8) * kMaxRedux);
-  d->m_result = cv.take<double>((size_t)kMaxRedux);
+  d->ll_part = cv.take<uint4>((size_t)2 * (n_sm + 8) * kMaxRedux);
+  d->ll_result = cv.take<uint4>((size_t)2 * kMaxRedux);
+  d->m_epoch = cv.take<uint32_t>(64);
+  d->m_prof = cv.take<unsigned long long>(kMasterProfSlots);
   d->history = cv.take<dao_iter_record>((size_t)dm.k_max);
   d->state = cv.take<DevState>(1);
   d->io_scratch = cv.take<double>(std::max<size_t>(vp, (size_t)std::max(dm.n_bl, dm.n_rows)) + 64);
@@ -673,6 +675,10 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   SETUP_CUDA(cudaMemsetAsync(d.y, 0, DAO_MAX_APERTURES * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.mz, 0, vp * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.mdz, 0, vp * 8, q));
+  SETUP_CUDA(cudaMemsetAsync(d.ll_part, 0, (size_t)2 * (c->n_sm + 8) * kMaxRedux * sizeof(uint4), q));
+  SETUP_CUDA(cudaMemsetAsync(d.ll_result, 0, (size_t)2 * kMaxRedux * sizeof(uint4), q));
+  SETUP_CUDA(cudaMemsetAsync(d.m_epoch, 0, 64 * 4, q));
+  SETUP_CUDA(cudaMemsetAsync(d.m_prof, 0, kMasterProfSlots * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.ap_beam, 0, (size_t)dm.k_max * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.ap_left, 0, (size_t)dm.k_max * dm.max_rows * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.ap_right, 0, (size_t)dm.k_max * dm.max_rows * 4, q));

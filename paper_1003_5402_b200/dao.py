@@ -23,7 +23,7 @@ STATUS_NAMES = {0: "DAO_OK", 1: "DAO_E_ARG", 2: "DAO_E_SHAPE", 3: "DAO_E_CUDA", 
 MEM_HOST, MEM_DEVICE = 0, 1
 MAX_APERTURES = 128
 (VEC_Z, VEC_G, VEC_W, VEC_X, VEC_Y, VEC_VSTAR, VEC_LEFT, VEC_RIGHT, VEC_BEAM_PRICE, VEC_HISTORY,
- VEC_MASTER_Z) = range(11)
+ VEC_MASTER_Z, VEC_MASTER_PHASES) = range(12)
 
 EXPORTS = ["dao_default_options", "dao_workspace_bytes", "dao_create", "dao_price", "dao_solve_master",
            "dao_run", "dao_get_plan", "dao_reset", "dao_destroy", "dao_last_error", "dao_get_vector",
@@ -287,7 +287,7 @@ class Dao:
                   VEC_X: (self.n_bl, np.float32), VEC_Y: (k_max, np.float64), VEC_VSTAR: (self.n_rows, np.float64),
                   VEC_LEFT: (self.n_rows, np.int32), VEC_RIGHT: (self.n_rows, np.int32),
                   VEC_BEAM_PRICE: (self.n_beams, np.float64), VEC_HISTORY: (k_max, ITER_RECORD_DTYPE),
-                  VEC_MASTER_Z: (self.n_vox, np.float64)}
+                  VEC_MASTER_Z: (self.n_vox, np.float64), VEC_MASTER_PHASES: (16, np.uint64)}
         n, dt = shapes[which]
         out = np.zeros(n, dtype=dt)
         self._check(self.lib.dao_get_vector(self._ctx, C.c_int32(which), C.c_void_p(_np_ptr(out)), C.c_int(MEM_HOST)))
