@@ -101,6 +101,9 @@ typedef struct {
   double price_tol;          /* optimal iff price_b* >= -price_tol * max_i |w_i| * (rows in b*) (default 1e-6, the
                                 fp32 noise floor of w), or iff the best candidate duplicates an aperture of the
                                 pool (its negative price is then residue of the master solve); S3, S6 */
+  double master_ls_tol;      /* a step t along the search direction is accepted when |phi'(t)| <= master_ls_tol *
+                                |phi'(0)| (phi(t) = F(z + t dz)) or when it ends on a bound still descending;
+                                otherwise t is refined by a safeguarded Newton search (default 0.01); S2 */
   int32_t master_method;     /* 0 = plain gradient projection, 1 = gradient projection with conjugate
                                 (Polak-Ribiere+) directions on the free face (default 1) */
   int32_t sell_sigma;        /* sorting window (rows) of the internal sliced-ELL layout of D; 1 = keep the

@@ -102,6 +102,7 @@ void dao_default_options(dao_options *opt) {
   opt->master_tol = 1e-7;
   opt->price_tol = 1e-6;
   opt->master_method = 1;
+  opt->master_ls_tol = 0.01;
   opt->sell_sigma = 0;
   opt->timers = 1;
 }

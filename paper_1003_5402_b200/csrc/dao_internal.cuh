@@ -26,6 +26,7 @@ constexpr int kMasterThreads = kMasterWorkers + 32;   // + the producer warp tha
 constexpr int kMasterTileVox = 4096;   // voxels per ring stage: 16 worker warps x 2 strips x 128
 constexpr int kMasterStageBytes = kMasterTileVox * 4;
 constexpr int kMasterMaxStages = 10;
+constexpr int kMasterMaxGrid = 160;    // CTAs of the master kernel (one per SM, capped)
 constexpr int kMasterProfSlots = 16;   // phase timers of the master (ns): 0 init, 1 G pass, 2 G reduce, 3 direction,
                                        // 4 D pass, 5 D reduce, 6 line search; 7 line-search evaluations,
                                        // 8 iterations, 9 calls, 10 publish

@@ -53,9 +53,9 @@ struct MasterParams {
   int32_t method;
   int32_t k_max;
   double tol;
+  double ls_tol;           // |phi'(t)| <= ls_tol * |phi'(0)| accepts a step
 };
 
-constexpr double kLineSearchTol = 1e-4;   // |phi'(t)| <= kLineSearchTol * |phi'(0)| ends the line search
 constexpr int kNW = kMasterWorkers / 32;  // worker warps
 
 // ---- small helpers ---------------------------------------------------------------------------
@@ -97,8 +97,10 @@ __device__ __forceinline__ double ll_value(const uint4 &w) {
 }
 
 // One warp sums value `i` of every CTA's slot of this epoch: lane l takes the CTAs l, l+32, ...
-// in that order, then a shuffle tree.  Every lane returns the total.
-constexpr int kMaxGridOver32 = 5;          // supports grids up to 160 CTAs (master_configure caps the grid)
+// in that order, then a shuffle tree (fixed order).  Every lane returns the total.
+// (A push variant -- every CTA stores into a private inbox of every reader -- was measured slower:
+// 3.8 us against 2.6 us for the small reduction on B200.)
+constexpr int kMaxGridOver32 = (kMasterMaxGrid + 31) / 32;
 __device__ __forceinline__ double ll_warp_gather(const uint4 *part /*[grid][kMaxRedux]*/, int i, uint32_t ep,
                                                  int lane) {
   const int grid = (int)gridDim.x;
@@ -137,7 +139,7 @@ struct Reducer {
     }
     wsync();
   }
-  // n <= kMaxRedux values: CTA i sums value i (two hops).
+  // n <= kMaxRedux values: CTA i sums value i and publishes the total (two hops).
   __device__ __noinline__ void large(int n, const double *vals, double *out) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     ++ep;
@@ -205,114 +207,105 @@ __device__ __forceinline__ int butterfly8_index(int lane) {
 
 
 // Phase P: the search direction from the reduced gradient (one warp; every CTA computes the same).
+// Lane l holds the apertures l, l + 32, ... in registers.  Outputs: p_s (direction, fp32-representable
+// values), pgold_s, free_prev_s, and the scalars sc[1] slope phi'(0), sc[2] t_max, sc[3] max|pg|, sc[4] KKT
+// residual, si[0] stop, si[1] stopped by the iteration cap, si[2] index of the blocking variable, si[3]
+// restarted, si[4] no descent direction left.
 __device__ __noinline__ void master_direction(int K, int iters, bool force_restart, int since_restart, int method,
-                                              int max_iter, double tol, double F, double *y_s, double *grad_s,
-                                              double *pg_s, double *pgold_s, double *p_s, double *vals_s, double *sc,
-                                              int *si, unsigned *free_prev_s) {
+                                              int max_iter, double tol, double F, const double *y_s,
+                                              const double *grad_s, double *pgold_s, double *p_s, double *sc, int *si,
+                                              unsigned *free_prev_s) {
   const int lane = threadIdx.x & 31;
-    double pg_max = 0.0, y_max = 1.0, kkt_l = 0.0, num = 0.0, den = 0.0;
-    unsigned free_now[4] = {0u, 0u, 0u, 0u};
+  const int nq = (K + 31) >> 5;
+  double yk[4], gk[4], pgk[4], pk[4], pprev[4];
+  double pg_max = 0.0, y_max = 1.0, kkt_l = 0.0, num = 0.0, den = 0.0;
+  bool same_free = true;
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
+  for (int q = 0; q < 4; ++q) {
+    yk[q] = 0.0; gk[q] = 0.0; pgk[q] = 0.0; pk[q] = 0.0; pprev[q] = 0.0;
+    if (q < nq) {
       const int k = q * 32 + lane;
       bool fr = false;
       if (k < K) {
-        const double gk = grad_s[k], yk = y_s[k];
-        fr = (yk > 0.0) || (gk < 0.0);
-        const double pgk = fr ? -gk : 0.0;
-        pg_s[k] = pgk;
-        pg_max = fmax(pg_max, fabs(pgk));
-        y_max = fmax(y_max, yk);
-        kkt_l = fmax(kkt_l, (yk > 0.0) ? fabs(gk) : fmax(-gk, 0.0));
-        num += pgk * (pgk - pgold_s[k]);
-        den += pgold_s[k] * pgold_s[k];
+        gk[q] = grad_s[k]; yk[q] = y_s[k]; pprev[q] = p_s[k];
+        const double pold = pgold_s[k];
+        fr = (yk[q] > 0.0) || (gk[q] < 0.0);
+        pgk[q] = fr ? -gk[q] : 0.0;
+        pg_max = fmax(pg_max, fabs(pgk[q]));
+        y_max = fmax(y_max, yk[q]);
+        kkt_l = fmax(kkt_l, (yk[q] > 0.0) ? fabs(gk[q]) : fmax(-gk[q], 0.0));
+        num += pgk[q] * (pgk[q] - pold);
+        den += pold * pold;
       }
-      free_now[q] = __ballot_sync(0xffffffffu, fr);
+      const unsigned fn = __ballot_sync(0xffffffffu, fr);
+      same_free = same_free && (fn == free_prev_s[q]);
+      __syncwarp();
+      if (lane == 0) free_prev_s[q] = fn;
     }
-    pg_max = warp_max_d(pg_max);
-    y_max = warp_max_d(y_max);
-    kkt_l = warp_max_d(kkt_l);
-    num = warp_sum_f64(num);
-    den = warp_sum_f64(den);
-    const bool conv = pg_max * y_max <= tol * fmax(F, 1e-300);
-    const bool stop = conv || iters >= max_iter;
-    bool same_free = true;
+  }
+  pg_max = warp_max_d(pg_max);
+  y_max = warp_max_d(y_max);
+  kkt_l = warp_max_d(kkt_l);
+  num = warp_sum_f64(num);
+  den = warp_sum_f64(den);
+  const bool conv = pg_max * y_max <= tol * fmax(F, 1e-300);
+  const bool stop = conv || iters >= max_iter;
+  bool restart = force_restart || !same_free || method == 0 || since_restart >= K + 8 || !(den > 0.0);
+  double beta = 0.0;
+  if (!restart) beta = fmax(num / den, 0.0);
+  if (beta == 0.0) restart = true;
+  // direction, rounded to fp32-representable values
+  double slope = 0.0;
+  bool infeasible = false;
 #pragma unroll
-    for (int q = 0; q < 4; ++q) same_free = same_free && (free_now[q] == free_prev_s[q]);
-    bool restart = force_restart || !same_free || method == 0 || since_restart >= K + 8 || !(den > 0.0);
-    double beta = 0.0;
-    if (!restart) beta = fmax(num / den, 0.0);
-    if (beta == 0.0) restart = true;
-    // direction, rounded to fp32-representable values
-    double slope = 0.0;
-    bool infeasible = false;
+  for (int q = 0; q < 4; ++q) {
+    double v = pgk[q];
+    if (!restart && v != 0.0) v = fma(beta, pprev[q], v);
+    v = (double)(float)v;
+    if (v < 0.0 && !(yk[q] > 0.0)) infeasible = true;
+    slope = fma(v, gk[q], slope);
+    pk[q] = v;
+  }
+  slope = warp_sum_f64(slope);
+  infeasible = __any_sync(0xffffffffu, infeasible);
+  if (!restart && (infeasible || !(slope < 0.0))) {
+    restart = true;
+    slope = 0.0;
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-      const int k = q * 32 + lane;
-      if (k < K) {
-        double pk = pg_s[k];
-        if (!restart && pk != 0.0) pk = fma(beta, p_s[k], pk);
-        if (!restart && pg_s[k] == 0.0) pk = 0.0;
-        pk = (double)(float)pk;
-        if (pk < 0.0 && !(y_s[k] > 0.0)) infeasible = true;
-        slope = fma(pk, grad_s[k], slope);
-        vals_s[k] = pk;     // tentative
-      }
+      pk[q] = (double)(float)pgk[q];
+      slope = fma(pk[q], gk[q], slope);
     }
     slope = warp_sum_f64(slope);
-    infeasible = __any_sync(0xffffffffu, infeasible);
-    if (!restart && (infeasible || !(slope < 0.0))) {
-      restart = true;
-      slope = 0.0;
+  }
+  double tmax = CUDART_INF;
+  int kb = 0x7fffffff;
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const int k = q * 32 + lane;
-        if (k < K) {
-          const double pk = (double)(float)pg_s[k];
-          slope = fma(pk, grad_s[k], slope);
-          vals_s[k] = pk;
-        }
-      }
-      slope = warp_sum_f64(slope);
-    }
-    double tmax = CUDART_INF;
-    int kb = 0x7fffffff;
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      const int k = q * 32 + lane;
-      if (k < K) {
-        const double pk = vals_s[k];
-        p_s[k] = pk;
-        pgold_s[k] = pg_s[k];
-        if (pk < 0.0) {
-          const double tk = y_s[k] / (-pk);
-          if (tk < tmax) { tmax = tk; kb = k; }
-        }
+  for (int q = 0; q < 4; ++q) {
+    const int k = q * 32 + lane;
+    if (k < K) {
+      p_s[k] = pk[q];
+      pgold_s[k] = pgk[q];
+      if (pk[q] < 0.0) {
+        const double tk = yk[q] / (-pk[q]);
+        if (tk < tmax) { tmax = tk; kb = k; }
       }
     }
-    {
-      const double tmin = warp_min_d(tmax);
-      const unsigned m = __ballot_sync(0xffffffffu, tmax == tmin && kb != 0x7fffffff);
-      int kb_w = 0x7fffffff;
-      if (m) {
-        // smallest k among the lanes that attain the minimum
-        int cand_k = (tmax == tmin) ? kb : 0x7fffffff;
+  }
+  {
+    const double tmin = warp_min_d(tmax);
+    // smallest k among the lanes that attain the minimum
+    int cand_k = (tmax == tmin) ? kb : 0x7fffffff;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) cand_k = min(cand_k, __shfl_xor_sync(0xffffffffu, cand_k, o));
-        kb_w = cand_k;
-      }
-      tmax = tmin;
-      kb = kb_w;
-    }
-    if (lane == 0) {
-      sc[1] = slope; sc[2] = tmax; sc[3] = pg_max; sc[4] = kkt_l;
-      si[0] = stop ? 1 : 0; si[1] = (stop && !conv) ? 1 : 0; si[2] = kb; si[3] = restart ? 1 : 0;
-      si[4] = (!(slope < 0.0)) ? 1 : 0;
-    }
-    if (lane == 0) {
-#pragma unroll
-      for (int q = 0; q < 4; ++q) free_prev_s[q] = free_now[q];
-    }
+    for (int o = 16; o > 0; o >>= 1) cand_k = min(cand_k, __shfl_xor_sync(0xffffffffu, cand_k, o));
+    tmax = tmin;
+    kb = cand_k;
+  }
+  if (lane == 0) {
+    sc[1] = slope; sc[2] = tmax; sc[3] = pg_max; sc[4] = kkt_l;
+    si[0] = stop ? 1 : 0; si[1] = (stop && !conv) ? 1 : 0; si[2] = kb; si[3] = restart ? 1 : 0;
+    si[4] = (!(slope < 0.0)) ? 1 : 0;
+  }
 }
 
 // ---- the A stream ----------------------------------------------------------------------------
@@ -355,12 +348,11 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
   // ---- shared state (replicated in every CTA, evolves identically everywhere) ----
   __shared__ double y_s[DAO_MAX_APERTURES];
   __shared__ double grad_s[kMaxRedux];
-  __shared__ double pg_s[DAO_MAX_APERTURES];       // projected steepest descent of this iteration
   __shared__ double pgold_s[DAO_MAX_APERTURES];
   __shared__ double p_s[DAO_MAX_APERTURES];        // search direction (fp32-representable values)
   __shared__ double vals_s[kMaxRedux];
   __shared__ double red_s[kMaxRedux];
-  __shared__ double scratch_s[kNW * 4];
+  __shared__ double scratch_s[kNW * 4];            // >= kNW * 3
   __shared__ double sc[16];                        // broadcast scalars
   __shared__ int si[8];
   __shared__ unsigned free_prev_s[4];
@@ -462,7 +454,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
   if (tid < 4) free_prev_s[tid] = 0u;
   if (p.z_in_smem) {
     uint8_t *sids = const_cast<uint8_t *>(sm.sids);
-    for (int i = tid; i < slab_len; i += kMasterWorkers) sids[i] = p.sid[v0 + i];
+    for (int j = tid; j < slab_len; j += kMasterWorkers)      // j = position, see pos()
+      sids[j] = p.sid[v0 + (j & ~127) + (j & 31) * 4 + ((j >> 5) & 3)];
   }
   Reducer red{p.ll_part, p.ll_result, 0u};
   if (tid == 0) si[7] = (int)*p.epoch;
@@ -484,8 +477,17 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
   // strips of this warp inside a tile: warp and warp + kNW (128 voxels each, 4 per lane)
   const int l0 = warp * 128 + lane * 4, l1 = (warp + kNW) * 128 + lane * 4;
 
-  // one D-type pass: out[i] = sum_k coef[k] A[k][i] on the slab (fp64, k ascending)
-  auto pass_d = [&](const double *coef, double *out) {
+  // Position of voxel (strip, lane, u) of the slab in the z / dz / sid arrays.  In shared memory the 4
+  // voxels of a lane are stored 32 doubles apart (conflict-free 64-bit accesses); in global memory
+  // (slab too large for shared memory) the order is the plain voxel order.
+  const bool permuted = p.z_in_smem != 0;
+  auto pos = [&](int strip_base, int u) { return permuted ? strip_base + u * 32 + lane : strip_base + lane * 4 + u; };
+
+  // one D-type pass: out[i] = sum_k coef[k] A[k][i] on the slab (fp64, k ascending).  With
+  // t_commit != 0 the pending step is committed first: z += t_commit * out_old (same thread, same
+  // voxels).  With curv, returns this thread's part of phi''(0) = sum 2 c_j out_j^2.
+  auto pass_d = [&](const double *coef, double *out, double t_commit, bool curv) -> double {
+    double h_acc = 0.0;
     for (int tile = 0; tile < n_tiles; ++tile) {
       const int t0 = tile * kMasterTileVox;
       const int tn = min(kMasterTileVox, slab_len - t0);
@@ -511,15 +513,30 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
         if (lane == 0) mbar_arrive(&sm.empty[cp.stage]);
         cp.advance(NS);
       }
-      if (a0) {
-        double2 *o = reinterpret_cast<double2 *>(out + t0 + l0);
-        o[0] = make_double2(acc[0], acc[1]); o[1] = make_double2(acc[2], acc[3]);
-      }
-      if (a1) {
-        double2 *o = reinterpret_cast<double2 *>(out + t0 + l1);
-        o[0] = make_double2(acc[4], acc[5]); o[1] = make_double2(acc[6], acc[7]);
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        if (h ? a1 : a0) {
+          const int sb = t0 + (h ? warp + kNW : warp) * 128;
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int i = pos(sb, u);
+            const double dd = acc[h * 4 + u];
+            if (curv) {
+              double z = sm.zs[i];
+              if (t_commit != 0.0) { z = fma(t_commit, out[i], z); sm.zs[i] = z; }
+              const int s = sm.sids[i];
+              if (s != kNoStruct) {
+                const StructEntry e = sm.stab[s];
+                const double c = (z < e.tm ? e.a : 0.0) + (z > e.tp ? e.b : 0.0);
+                h_acc = fma(2.0 * c * dd, dd, h_acc);
+              }
+            }
+            out[i] = dd;
+          }
+        }
       }
     }
+    return h_acc;
   };
 
   // ---- z = A y on the slab (fp64), dz = 0 ----
@@ -527,7 +544,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
     bool any = false;
     for (int k = 0; k < K0; ++k) any = any || (y_s[k] != 0.0);
     if (any) {
-      pass_d(y_s, sm.zs);
+      pass_d(y_s, sm.zs, 0.0, false);
     } else {
       for (int i = tid; i < slab_len; i += kMasterWorkers) sm.zs[i] = 0.0;
     }
@@ -536,15 +553,22 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
   wsync();
   PROF_MARK(0);
 
-  double t_step = 0.0;          // step to apply to z at the start of the next G phase
+  // The step t along the current direction is NOT verified by a separate line-search evaluation:
+  // the next gradient pass runs at the trial point z + t dz and delivers phi'(t) = dz . g(z + t dz)
+  // (= p . grad) and phi''(t) with the same reduction.  Only when the trial point fails the test
+  // |phi'(t)| <= ls_tol |phi'(0)| is t refined (shared memory only) and the pass repeated.
+  double t_trial = 0.0;         // step of the trial point (0: no direction yet)
+  double slope0 = 0.0, tmax = CUDART_INF;
+  int kb = 0x7fffffff;
+  bool have_dir = false, forced = false;
   int iters = 0, restarts = 0, since_restart = 0;
   bool force_restart = true;
   int hit_max = 0;
-  double F = 0.0, kkt = 0.0, pgmax = 0.0;
+  double F = CUDART_INF, kkt = 0.0, pgmax = 0.0;
 
   for (;;) {
-    // ================= phase G: z += t dz, g(z), grad = A^T g, F ==========================
-    double f_acc = 0.0;
+    // ============ phase G: g(z + t dz), grad = A^T g, F, phi'(t), phi''(t) ================
+    double f_acc = 0.0, s1_acc = 0.0, s2_acc = 0.0;
     for (int tile = 0; tile < n_tiles; ++tile) {
       const int t0 = tile * kMasterTileVox;
       const int tn = min(kMasterTileVox, slab_len - t0);
@@ -553,30 +577,34 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         const bool act = h ? a1 : a0;
-        const int i0 = t0 + (h ? l1 : l0);
+        const int sb = t0 + (h ? warp + kNW : warp) * 128;
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
           double gv = 0.0;
           if (act) {
-            double z = sm.zs[i0 + u];
-            if (t_step != 0.0) { z = fma(t_step, sm.dzs[i0 + u], z); sm.zs[i0 + u] = z; }
-            const int s = sm.sids[i0 + u];
+            const int i = pos(sb, u);
+            const int s = sm.sids[i];
             if (s != kNoStruct) {
               const StructEntry e = sm.stab[s];
+              const double dz = sm.dzs[i];
+              const double z = fma(t_trial, dz, sm.zs[i]);
               const double un = fmax(e.tm - z, 0.0), ov = fmax(z - e.tp, 0.0);
               f_acc += e.a * un * un + e.b * ov * ov;
               gv = -2.0 * e.a * un + 2.0 * e.b * ov;
+              const double c = (un > 0.0 ? e.a : 0.0) + (ov > 0.0 ? e.b : 0.0);
+              s1_acc = fma(dz, gv, s1_acc);
+              s2_acc = fma(2.0 * c * dz, dz, s2_acc);
             }
           }
           g[h * 4 + u] = gv;
         }
       }
-      for (int kb = 0; kb < K; kb += 8) {
+      for (int kb8 = 0; kb8 < K; kb8 += 8) {
         double d[8];
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
           d[j] = 0.0;
-          if (kb + j < K) {
+          if (kb8 + j < K) {
             mbar_wait(&sm.full[cp.stage], cp.phase);
             const unsigned char *st = sm.ring + (size_t)cp.stage * kMasterStageBytes;
             if (a0) {
@@ -597,7 +625,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
           }
         }
         const double r = butterfly8(d, lane);
-        const int kk = kb + butterfly8_index(lane);
+        const int kk = kb8 + butterfly8_index(lane);
         if ((lane & 3) == 0) {
           double *slot = sm.warp_part + warp * DAO_MAX_APERTURES + kk;
           *slot = (tile == 0) ? r : (*slot + r);
@@ -605,8 +633,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
       }
     }
     {
-      const double fs = warp_sum_f64(f_acc);
-      if (lane == 0) scratch_s[warp] = fs;
+      const double fs = warp_sum_f64(f_acc), s1 = warp_sum_f64(s1_acc), s2 = warp_sum_f64(s2_acc);
+      if (lane == 0) { scratch_s[warp * 3] = fs; scratch_s[warp * 3 + 1] = s1; scratch_s[warp * 3 + 2] = s2; }
     }
     wsync();
     if (tid < K) {
@@ -614,56 +642,103 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
       if (n_tiles > 0)
         for (int w = 0; w < kNW; ++w) s += sm.warp_part[w * DAO_MAX_APERTURES + tid];
       vals_s[tid] = s;
-    }
-    if (tid == K) {
+    } else if (tid < K + 3) {
       double s = 0.0;
-      for (int w = 0; w < kNW; ++w) s += scratch_s[w];
-      vals_s[K] = s;
+      for (int w = 0; w < kNW; ++w) s += scratch_s[w * 3 + (tid - K)];
+      vals_s[tid] = s;
     }
     wsync();
     PROF_MARK(1);
-    red.large(K + 1, vals_s, grad_s /* K grads, then F */);
-    F = grad_s[K];
+    red.large(K + 3, vals_s, grad_s /* K grads, F, phi'(t), phi''(t) */);
+    const double F_trial = grad_s[K];
     PROF_MARK(2);
+
+    if (have_dir) {
+      const double s1 = grad_s[K + 1], s2 = grad_s[K + 2];
+      const bool at_bound = (t_trial >= tmax) && (s1 < 0.0);            // still descending at the bound
+      const bool ok = forced || ((fabs(s1) <= p.ls_tol * fabs(slope0) || at_bound) && F_trial <= F + 1e-13 * fabs(F));
+      if (!ok) {
+        // ---- refine t: root of phi'(t) on [0, tmax]; phi' is non-decreasing, piecewise linear ----
+        double lo = 0.0, slo = slope0, hi = CUDART_INF, shi = 0.0;
+        double t = t_trial, c1 = s1, c2 = s2;
+        for (int ls = 0; ls < 40; ++ls) {
+          if (fabs(c1) <= p.ls_tol * fabs(slope0)) break;          // exact enough
+          double tn;
+          if (c1 < 0.0) {
+            if (t >= tmax) break;                                    // descending at the bound
+            lo = t; slo = c1;
+            tn = (c2 > 0.0) ? t - c1 / c2 : 2.0 * t;
+            if (hi < CUDART_INF && !(tn < hi)) tn = lo + (hi - lo) * (-slo) / (shi - slo);
+            if (tn > tmax) tn = tmax;
+          } else {
+            hi = t; shi = c1;
+            tn = (c2 > 0.0) ? t - c1 / c2 : 0.5 * (lo + hi);
+            if (!(tn > lo)) tn = lo + (hi - lo) * (-slo) / (shi - slo);
+          }
+          if (!(tn > lo) || !(tn < hi)) tn = 0.5 * (lo + (hi < CUDART_INF ? hi : 2.0 * t));
+          if (hi < CUDART_INF && (hi - lo) <= 1e-15 * hi) { t = (c1 < 0.0) ? hi : lo; if (t <= 0.0) t = hi; break; }
+          if (tn == t) break;
+          t = tn;
+          double acc2[2] = {0.0, 0.0};   // phi'(t), phi''(t)
+          for (int i = tid; i < slab_len; i += kMasterWorkers) {
+            const int s = sm.sids[i];
+            if (s == kNoStruct) continue;
+            const StructEntry e = sm.stab[s];
+            const double dz = sm.dzs[i];
+            const double z = fma(t, dz, sm.zs[i]);
+            const double u = fmax(e.tm - z, 0.0), o = fmax(z - e.tp, 0.0);
+            const double gv = -2.0 * e.a * u + 2.0 * e.b * o;
+            const double c = (u > 0.0 ? e.a : 0.0) + (o > 0.0 ? e.b : 0.0);
+            acc2[0] = fma(dz, gv, acc2[0]);
+            acc2[1] = fma(2.0 * c * dz, dz, acc2[1]);
+          }
+          block_sum<2>(acc2, scratch_s, vals_s);
+          red.small(2, vals_s, red_s);
+          if (prof) ++prof_s[7];
+          c1 = red_s[0]; c2 = red_s[1];
+        }
+        if (prof) ++prof_s[11];
+        t_trial = t;
+        forced = true;
+        wsync();
+        PROF_MARK(6);
+        continue;                        // gradient pass again, at the refined step
+      }
+      // ---- accept: y += t p (every CTA identically); z is committed by the next D pass ----
+      if (tid < K) {
+        double yk = fma(t_trial, p_s[tid], y_s[tid]);
+        if (yk < 0.0) yk = 0.0;
+        if (at_bound && tid == kb) yk = 0.0;
+        y_s[tid] = yk;
+      }
+      if (at_bound) force_restart = true;
+      ++iters;
+      wsync();
+    }
+    F = F_trial;
 
     // ================= phase P: direction (warp 0, identical in every CTA) ================
     if (warp == 0)
-      master_direction(K, iters, force_restart, since_restart, p.method, p.max_iter, p.tol, F, y_s, grad_s, pg_s,
-                       pgold_s, p_s, vals_s, sc, si, free_prev_s);
+      master_direction(K, iters, force_restart, since_restart, p.method, p.max_iter, p.tol, F, y_s, grad_s, pgold_s,
+                       p_s, sc, si, free_prev_s);
     wsync();
     pgmax = sc[3];
     kkt = sc[4];
     PROF_MARK(3);
-    if (si[0] || si[4]) { hit_max = si[1]; break; }   // converged, iteration cap, or no descent left
-    const double slope0 = sc[1], tmax = sc[2];
-    const int kb = si[2];
+    if (si[0] || si[4]) {               // converged, iteration cap, or no descent left
+      hit_max = si[1];
+      if (t_trial != 0.0) {             // commit the accepted step
+        for (int i = tid; i < slab_len; i += kMasterWorkers) sm.zs[i] = fma(t_trial, sm.dzs[i], sm.zs[i]);
+      }
+      break;
+    }
+    slope0 = sc[1]; tmax = sc[2];
+    kb = si[2];
     if (si[3]) { ++restarts; since_restart = 0; } else { ++since_restart; }
     force_restart = false;
 
-    // ================= phase D: dz = A p, curvature =======================================
-    pass_d(p_s, sm.dzs);
-    double h_acc = 0.0;
-    for (int tile = 0; tile < n_tiles; ++tile) {
-      const int t0 = tile * kMasterTileVox;
-      const int tn = min(kMasterTileVox, slab_len - t0);
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const int li = h ? l1 : l0;
-        if (li < tn) {
-#pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            const int i = t0 + li + u;
-            const int s = sm.sids[i];
-            if (s != kNoStruct) {
-              const StructEntry e = sm.stab[s];
-              const double z = sm.zs[i], dd = sm.dzs[i];
-              const double c = (z < e.tm ? e.a : 0.0) + (z > e.tp ? e.b : 0.0);
-              h_acc = fma(2.0 * c * dd, dd, h_acc);
-            }
-          }
-        }
-      }
-    }
+    // ================= phase D: commit z, dz = A p, curvature =============================
+    const double h_acc = pass_d(p_s, sm.dzs, t_trial, true);
     {
       double hv[1] = {h_acc};
       block_sum<1>(hv, scratch_s, vals_s);
@@ -672,67 +747,22 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
     red.small(1, vals_s, red_s);
     const double h0 = red_s[0];
     PROF_MARK(5);
-
-    // ================= phase L: root of phi'(t) on [0, tmax] ==============================
-    // phi' is non-decreasing and piecewise linear; phi'(0) = slope0 < 0.
-    double lo = 0.0, slo = slope0, hi = CUDART_INF, shi = 0.0;
+    // Newton step on the ray (exact while the voxel active set does not change), clipped to the bound
     double t = (h0 > 0.0) ? (-slope0 / h0) : ((tmax < CUDART_INF) ? tmax : 1.0);
     if (t > tmax) t = tmax;
-    bool hit_bound = false;
-    for (int ls = 0; ls < 40; ++ls) {
-      double acc3[3] = {0.0, 0.0, 0.0};   // phi'(t), phi''(t), F(t)
-      for (int i = tid; i < slab_len; i += kMasterWorkers) {
-        const int s = sm.sids[i];
-        if (s == kNoStruct) continue;
-        const StructEntry e = sm.stab[s];
-        const double dz = sm.dzs[i];
-        const double z = fma(t, dz, sm.zs[i]);
-        const double u = fmax(e.tm - z, 0.0), o = fmax(z - e.tp, 0.0);
-        const double gv = -2.0 * e.a * u + 2.0 * e.b * o;
-        const double c = (u > 0.0 ? e.a : 0.0) + (o > 0.0 ? e.b : 0.0);
-        acc3[0] = fma(dz, gv, acc3[0]);
-        acc3[1] = fma(2.0 * c * dz, dz, acc3[1]);
-        acc3[2] += e.a * u * u + e.b * o * o;
-      }
-      block_sum<3>(acc3, scratch_s, vals_s);
-      red.small(3, vals_s, red_s);
-      if (prof) ++prof_s[7];
-      const double s1 = red_s[0], s2 = red_s[1];
-      if (fabs(s1) <= kLineSearchTol * fabs(slope0)) break;      // exact enough
-      double tn;
-      if (s1 < 0.0) {
-        if (t >= tmax) { hit_bound = true; break; }              // still descending at the bound
-        lo = t; slo = s1;
-        tn = (s2 > 0.0) ? t - s1 / s2 : 2.0 * t;
-        if (hi < CUDART_INF && !(tn < hi)) tn = lo + (hi - lo) * (-slo) / (shi - slo);
-        if (tn > tmax) tn = tmax;
-      } else {
-        hi = t; shi = s1;
-        tn = (s2 > 0.0) ? t - s1 / s2 : 0.5 * (lo + hi);
-        if (!(tn > lo)) tn = lo + (hi - lo) * (-slo) / (shi - slo);
-      }
-      if (!(tn > lo) || !(tn < hi)) tn = 0.5 * (lo + (hi < CUDART_INF ? hi : 2.0 * t));
-      if (hi < CUDART_INF && (hi - lo) <= 1e-15 * hi) { t = (s1 < 0.0) ? hi : lo; if (t <= 0.0) t = hi; break; }
-      if (tn == t) break;
-      t = tn;
-    }
-    // ================= update y (every CTA identically); z is updated in the next G phase ==
-    if (tid < K) {
-      double yk = fma(t, p_s[tid], y_s[tid]);
-      if (yk < 0.0) yk = 0.0;
-      if (hit_bound && tid == kb) yk = 0.0;
-      y_s[tid] = yk;
-    }
-    if (hit_bound) force_restart = true;
-    t_step = t;
-    ++iters;
-    wsync();
-    PROF_MARK(6);
+    t_trial = t;
+    have_dir = true;
+    forced = false;
   }
+  wsync();
 
   // ---- publish ----
   if (p.z_in_smem) {
-    for (int i = tid; i < slab_len; i += kMasterWorkers) { p.mz[v0 + i] = sm.zs[i]; p.mdz[v0 + i] = sm.dzs[i]; }
+    for (int j = tid; j < slab_len; j += kMasterWorkers) {
+      const int i = (j & ~127) + (j & 31) * 4 + ((j >> 5) & 3);
+      p.mz[v0 + i] = sm.zs[j];
+      p.mdz[v0 + i] = sm.dzs[j];
+    }
   }
   if (tid == 0) {
     s_consumed_stage = (unsigned)cp.stage;
@@ -786,7 +816,7 @@ static size_t master_fixed_smem(const Ctx *c, int n_stages) {
 }
 
 cudaError_t master_configure(Ctx *c) {
-  c->master_grid = std::min(c->n_sm, 32 * kMaxGridOver32);      // one CTA per SM
+  c->master_grid = std::min(c->n_sm, kMasterMaxGrid);      // one CTA per SM
   int slab = (c->n_vox_pad + c->master_grid - 1) / c->master_grid;
   slab = (slab + 127) / 128 * 128;
   c->master_slab = slab;
@@ -846,6 +876,7 @@ cudaError_t launch_master(Ctx *c, bool add_candidate) {
   p.method = c->opt.master_method;
   p.k_max = c->opt.k_max;
   p.tol = c->opt.master_tol;
+  p.ls_tol = c->opt.master_ls_tol;
   void *args[] = {&p};
   return cudaLaunchCooperativeKernel((void *)k_master, dim3(c->master_grid), dim3(kMasterThreads), args,
                                      c->master_smem, c->stream);

@@ -136,8 +136,11 @@ static void carve_workspace(Carver &cv, const Dims &dm, const HostLayout &L, Dev
   d->y = cv.take<double>((size_t)DAO_MAX_APERTURES);
   d->mz = cv.take<double>(vp);
   d->mdz = cv.take<double>(vp);
-  d->ll_part = cv.take<uint4>((size_t)2 * (n_sm + 8) * kMaxRedux);
-  d->ll_result = cv.take<uint4>((size_t)2 * kMaxRedux);
+  {
+    const size_t g = (size_t)std::min(n_sm, kMasterMaxGrid);
+    d->ll_part = cv.take<uint4>(2 * g * kMaxRedux);
+    d->ll_result = cv.take<uint4>(2 * kMaxRedux);
+  }
   d->m_epoch = cv.take<uint32_t>(64);
   d->m_prof = cv.take<unsigned long long>(kMasterProfSlots);
   d->history = cv.take<dao_iter_record>((size_t)dm.k_max);
@@ -205,7 +208,8 @@ static dao_status check_args(const dao_csr *D, const dao_mlc *mlc, const dao_str
   if (opt->k_max < 1) { *err = "k_max must be >= 1"; return DAO_E_ARG; }
   if (opt->k_max > DAO_MAX_APERTURES) { *err = "k_max > DAO_MAX_APERTURES"; return DAO_E_UNSUPPORTED; }
   if (opt->master_max_iter < 0 || !(opt->master_tol >= 0.0) || !(opt->price_tol >= 0.0) ||
-      (opt->master_method != 0 && opt->master_method != 1) || opt->sell_sigma < 0) {
+      (opt->master_method != 0 && opt->master_method != 1) || opt->sell_sigma < 0 ||
+      !(opt->master_ls_tol > 0.0) || !(opt->master_ls_tol < 1.0)) {
     *err = "bad option value"; return DAO_E_ARG;
   }
   // MLC tables (host)
@@ -675,8 +679,11 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   SETUP_CUDA(cudaMemsetAsync(d.y, 0, DAO_MAX_APERTURES * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.mz, 0, vp * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.mdz, 0, vp * 8, q));
-  SETUP_CUDA(cudaMemsetAsync(d.ll_part, 0, (size_t)2 * (c->n_sm + 8) * kMaxRedux * sizeof(uint4), q));
-  SETUP_CUDA(cudaMemsetAsync(d.ll_result, 0, (size_t)2 * kMaxRedux * sizeof(uint4), q));
+  {
+    const size_t g = (size_t)std::min(c->n_sm, kMasterMaxGrid);
+    SETUP_CUDA(cudaMemsetAsync(d.ll_part, 0, 2 * g * kMaxRedux * sizeof(uint4), q));
+    SETUP_CUDA(cudaMemsetAsync(d.ll_result, 0, 2 * kMaxRedux * sizeof(uint4), q));
+  }
   SETUP_CUDA(cudaMemsetAsync(d.m_epoch, 0, 64 * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.m_prof, 0, kMasterProfSlots * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.ap_beam, 0, (size_t)dm.k_max * 4, q));

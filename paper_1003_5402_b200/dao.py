@@ -55,7 +55,7 @@ class CStructs(C.Structure):
 
 class COptions(C.Structure):
     _fields_ = [("k_max", C.c_int32), ("master_max_iter", C.c_int32), ("master_tol", C.c_double),
-                ("price_tol", C.c_double), ("master_method", C.c_int32), ("sell_sigma", C.c_int32),
+                ("price_tol", C.c_double), ("master_ls_tol", C.c_double), ("master_method", C.c_int32), ("sell_sigma", C.c_int32),
                 ("timers", C.c_int32), ("reserved", C.c_int32)]
 
 
