@@ -90,6 +90,11 @@ typedef struct {
   const float *w_under;          /* [n_struct] host: alpha_s (0 for non-targets) */
   const float *t_over;           /* [n_struct] host: T_s^+  (over-dose threshold) */
   const float *w_over;           /* [n_struct] host: beta_s */
+  /* Re-optimisation mode (the per-voxel form eq. 3-4).  Both fields may be 0. */
+  const float *vox_threshold;    /* optional [n_vox], same memspace as D: T_j, replaces BOTH thresholds T_s^- and
+                                    T_s^+ of voxel j's structure (finite values) */
+  int32_t per_voxel_weights;     /* 0: weights alpha_s / |v_s|, beta_s / |v_s| (eq. 9-10); 1: alpha_s, beta_s are the
+                                    per-voxel weights alpha_j, beta_j of eq. 3-4 as they are (no division by |v_s|) */
 } dao_structs;
 
 /* Options.  Zero-initialise, then dao_default_options, then override. */

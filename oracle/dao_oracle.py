@@ -88,6 +88,26 @@ def voxel_params(vox_struct, t_under, w_under, t_over, w_over) -> VoxelParams:
     return VoxelParams(*out)
 
 
+def voxel_params_of(ph) -> VoxelParams:
+    """Per-voxel penalty parameters of a problem instance.  Default: eq. (9)-(10).  With
+    ``ph.per_voxel_weights`` the weights are the alpha_j, beta_j of eq. (3)-(4) as given (no division
+    by |v_s|); with ``ph.vox_threshold`` T_j replaces both thresholds -- together the paper's
+    re-optimisation mode (alpha_j = beta_j = 1, T_j = reference dose)."""
+    vp = voxel_params(ph.vox_struct, ph.t_under, ph.w_under, ph.t_over, ph.w_over)
+    vs = _i32(ph.vox_struct)
+    inside = vs >= 0
+    if getattr(ph, "per_voxel_weights", False):
+        a = np.zeros(vs.size); b = np.zeros(vs.size)
+        a[inside] = _f64(ph.w_under)[vs[inside]]
+        b[inside] = _f64(ph.w_over)[vs[inside]]
+        vp = VoxelParams(a, b, vp.tm, vp.tp)
+    vt = getattr(ph, "vox_threshold", None)
+    if vt is not None:
+        t = np.asarray(vt, dtype=np.float32).astype(np.float64)
+        vp = VoxelParams(vp.a, vp.b, t.copy(), t.copy())
+    return vp
+
+
 def objective(z, vp: VoxelParams) -> float:
     """O2: F(z), eq. (3)-(5) / (9)-(10)."""
     z = _f64(z)
@@ -243,7 +263,7 @@ def price_converged(pr: Pricing, w, beam_row_ptr, price_tol: float) -> bool:
 def run(ph, max_apertures: int, master_tol: float = 1e-10, master_max_iter: int = 20000,
         price_tol: float = 1e-9, method: str = "newton", keep_A: bool = False) -> Plan:
     """O9: the column-generation loop.  `ph` is any object with the Phantom fields."""
-    vp = voxel_params(ph.vox_struct, ph.t_under, ph.w_under, ph.t_over, ph.w_over)
+    vp = voxel_params_of(ph)
     n_vox, n_bl = ph.n_vox, ph.n_bl
     A = np.zeros((max_apertures, n_vox), dtype=np.float64)
     plan = Plan()

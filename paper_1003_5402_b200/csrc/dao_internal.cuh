@@ -90,6 +90,7 @@ struct DevPtrs {
   int32_t *inv_perm;       // [n_vox]     caller voxel -> internal
   uint8_t *sid;            // [n_vox_pad] structure id or kNoStruct
   StructEntry *stab;       // [256]
+  float *vt;               // [n_vox_pad] per-voxel threshold T_j (re-optimisation mode), internal order
   // CSR of D^T (rows = beamlets, entries = internal voxel ids)
   int32_t *t_ptr;          // [n_bl+1]
   int32_t *t_row;          // [nnz padded to kTChunk] caller voxel ids, ascending inside a row
@@ -154,6 +155,7 @@ struct Ctx {
   size_t master_smem = 0;
   int master_slab = 0, master_stages = 0, master_z_in_smem = 0;
   bool x_in_smem = true;
+  bool has_vt = false;          // per-voxel thresholds in use (d.vt)
   int spmv_ring_warps = 0;      // > 0: the TMA-ring SpMV variant with that many warps per CTA
   // host mirror (pinned) of DevState for the once-per-iteration read-back
   DevState *h_state = nullptr;

@@ -37,6 +37,7 @@ struct MasterParams {
   int32_t z_in_smem;       // 1: z, dz, sid of the slab live in shared memory
   int32_t n_struct;
   const uint8_t *sid;
+  const float *vt;         // per-voxel thresholds T_j (re-optimisation mode) or null
   const StructEntry *stab;
   double *mz;
   double *mdz;
@@ -339,6 +340,7 @@ struct MasterSmem {          // carved from dynamic shared memory by every threa
   uint64_t *full, *empty;    // [n_stages]
   double *zs, *dzs;          // [slab] (shared or this CTA's part of the global arrays)
   const uint8_t *sids;       // [slab]
+  const float *vts;          // [slab] or null
   StructEntry *stab;         // [n_struct]
   double *warp_part;         // [kNW][kpad]
 };
@@ -390,9 +392,11 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
     if (p.z_in_smem) {
       sm.zs = reinterpret_cast<double *>(q); q += (size_t)p.slab * 8;
       sm.dzs = reinterpret_cast<double *>(q); q += (size_t)p.slab * 8;
+      sm.vts = p.vt ? reinterpret_cast<const float *>(q) : nullptr; q += p.vt ? (size_t)p.slab * 4 : 0;
       sm.sids = q;
     } else {
       sm.zs = p.mz + v0; sm.dzs = p.mdz + v0; sm.sids = p.sid + v0;
+      sm.vts = p.vt ? p.vt + v0 : nullptr;
     }
   }
   if (tid == 0) {
@@ -454,8 +458,12 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
   if (tid < 4) free_prev_s[tid] = 0u;
   if (p.z_in_smem) {
     uint8_t *sids = const_cast<uint8_t *>(sm.sids);
-    for (int j = tid; j < slab_len; j += kMasterWorkers)      // j = position, see pos()
-      sids[j] = p.sid[v0 + (j & ~127) + (j & 31) * 4 + ((j >> 5) & 3)];
+    float *vts = const_cast<float *>(sm.vts);
+    for (int j = tid; j < slab_len; j += kMasterWorkers) {    // j = position, see pos()
+      const int i = v0 + (j & ~127) + (j & 31) * 4 + ((j >> 5) & 3);
+      sids[j] = p.sid[i];
+      if (vts) vts[j] = p.vt[i];
+    }
   }
   Reducer red{p.ll_part, p.ll_result, 0u};
   if (tid == 0) si[7] = (int)*p.epoch;
@@ -526,7 +534,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
               if (t_commit != 0.0) { z = fma(t_commit, out[i], z); sm.zs[i] = z; }
               const int s = sm.sids[i];
               if (s != kNoStruct) {
-                const StructEntry e = sm.stab[s];
+                StructEntry e = sm.stab[s];
+              if (sm.vts) e.tm = e.tp = (double)sm.vts[i];
                 const double c = (z < e.tm ? e.a : 0.0) + (z > e.tp ? e.b : 0.0);
                 h_acc = fma(2.0 * c * dd, dd, h_acc);
               }
@@ -585,7 +594,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
             const int i = pos(sb, u);
             const int s = sm.sids[i];
             if (s != kNoStruct) {
-              const StructEntry e = sm.stab[s];
+              StructEntry e = sm.stab[s];
+              if (sm.vts) e.tm = e.tp = (double)sm.vts[i];
               const double dz = sm.dzs[i];
               const double z = fma(t_trial, dz, sm.zs[i]);
               const double un = fmax(e.tm - z, 0.0), ov = fmax(z - e.tp, 0.0);
@@ -683,7 +693,8 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
           for (int i = tid; i < slab_len; i += kMasterWorkers) {
             const int s = sm.sids[i];
             if (s == kNoStruct) continue;
-            const StructEntry e = sm.stab[s];
+            StructEntry e = sm.stab[s];
+              if (sm.vts) e.tm = e.tp = (double)sm.vts[i];
             const double dz = sm.dzs[i];
             const double z = fma(t, dz, sm.zs[i]);
             const double u = fmax(e.tm - z, 0.0), o = fmax(z - e.tp, 0.0);
@@ -827,7 +838,7 @@ cudaError_t master_configure(Ctx *c) {
   e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device);
   if (e != cudaSuccess) return e;
   const size_t budget = (size_t)max_optin - fa.sharedSizeBytes - 1024;
-  const size_t slab_bytes = (size_t)slab * 17;
+  const size_t slab_bytes = (size_t)slab * (c->has_vt ? 21 : 17);
   // prefer z in shared memory with >= 4 stages; otherwise z stays in global memory (L2)
   c->master_z_in_smem = 0;
   int stages = 0;
@@ -860,6 +871,7 @@ cudaError_t launch_master(Ctx *c, bool add_candidate) {
   p.z_in_smem = c->master_z_in_smem;
   p.n_struct = std::max(c->n_struct, 1);
   p.sid = c->d.sid;
+  p.vt = c->has_vt ? c->d.vt : nullptr;
   p.stab = c->d.stab;
   p.mz = c->d.mz;
   p.mdz = c->d.mdz;

@@ -107,6 +107,7 @@ static void carve_workspace(Carver &cv, const Dims &dm, const HostLayout &L, Dev
   d->inv_perm = cv.take<int32_t>((size_t)dm.n_vox);
   d->sid = cv.take<uint8_t>(vp);
   d->stab = cv.take<StructEntry>(256);
+  d->vt = cv.take<float>(vp);
   d->t_ptr = cv.take<int32_t>((size_t)dm.n_bl + 2);
   d->t_row = cv.take<int32_t>((size_t)ntc * kTChunk + 64);
   d->t_val = cv.take<float>((size_t)ntc * kTChunk + 64);
@@ -151,7 +152,7 @@ static void carve_workspace(Carver &cv, const Dims &dm, const HostLayout &L, Dev
 // create-time scratch
 struct ScratchPtrs {
   int32_t *row_ptr, *col, *vs;
-  float *val;
+  float *val, *vt;
   int32_t *keyA, *rowA, *keyB, *rowB;
   float *valA, *valB;
   int32_t *tile_hist;
@@ -166,9 +167,10 @@ static void carve_scratch(Carver &cv, const Dims &dm, bool host_inputs, ScratchP
     s->col = cv.take<int32_t>(nz);
     s->val = cv.take<float>(nz);
     s->vs = cv.take<int32_t>((size_t)dm.n_vox);
+    s->vt = cv.take<float>((size_t)dm.n_vox);
   } else {
     s->row_ptr = s->col = s->vs = nullptr;
-    s->val = nullptr;
+    s->val = s->vt = nullptr;
   }
   s->keyA = cv.take<int32_t>(nz);
   s->rowA = cv.take<int32_t>(nz);
@@ -330,6 +332,17 @@ __global__ void k_fill_sell(int32_t n_vox_pad, const int32_t *__restrict__ perm,
     sell_col[dst] = k < n ? col[lo + k] : 0;
     sell_val[dst] = k < n ? val[lo + k] : 0.f;
   }
+}
+
+// per-voxel thresholds in the internal voxel order; flags non-finite values
+__global__ void k_fill_vt(int32_t n_vox_pad, const int32_t *__restrict__ perm, const float *__restrict__ vt_in,
+                          float *__restrict__ vt, int32_t *__restrict__ flags) {
+  const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_vox_pad) return;
+  const int32_t j = perm[i];
+  const float t = j >= 0 ? vt_in[j] : 0.f;
+  if (!isfinite(t)) atomicOr(flags, kErrVal);
+  vt[i] = t;
 }
 
 __global__ void k_fill_sid(int32_t n_vox_pad, const int32_t *__restrict__ perm, const int32_t *__restrict__ vs,
@@ -577,8 +590,9 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
     std::vector<StructEntry> tab(256, StructEntry{0.0, 0.0, 0.0, 0.0});
     for (int i = 0; i < s->n_struct; ++i) {
       const double n = (double)h_flags[1 + i];
-      tab[i].a = n > 0 ? (double)s->w_under[i] / n : 0.0;
-      tab[i].b = n > 0 ? (double)s->w_over[i] / n : 0.0;
+      const double div = s->per_voxel_weights ? 1.0 : n;       // eq. 3-4 as given, or eq. 9-10 per |v_s|
+      tab[i].a = n > 0 ? (double)s->w_under[i] / div : 0.0;
+      tab[i].b = n > 0 ? (double)s->w_over[i] / div : 0.0;
       tab[i].tm = (double)s->t_under[i];
       tab[i].tp = (double)s->t_over[i];
     }
@@ -595,6 +609,23 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   SETUP_CUDA(cudaGetLastError());
   k_fill_sid<<<grid_for(L.n_vox_pad, 256), 256, 0, q>>>(L.n_vox_pad, d.perm, d_vs, d.sid);
   SETUP_CUDA(cudaGetLastError());
+  c->has_vt = s->vox_threshold != nullptr;
+  if (c->has_vt) {
+    const float *d_vt = s->vox_threshold;
+    if (host_in) {
+      SETUP_CUDA(cudaMemcpyAsync(sp.vt, s->vox_threshold, (size_t)dm.n_vox * 4, cudaMemcpyHostToDevice, q));
+      d_vt = sp.vt;
+    }
+    SETUP_CUDA(cudaMemsetAsync(sp.flags, 0, sizeof(int32_t), q));
+    k_fill_vt<<<grid_for(L.n_vox_pad, 256), 256, 0, q>>>(L.n_vox_pad, d.perm, d_vt, d.vt, sp.flags);
+    SETUP_CUDA(cudaGetLastError());
+    int32_t f = 0;
+    SETUP_CUDA(cudaMemcpyAsync(&f, sp.flags, sizeof(f), cudaMemcpyDeviceToHost, q));
+    SETUP_CUDA(cudaStreamSynchronize(q));
+    if (f & kErrVal) { c->err = "vox_threshold must be finite"; return DAO_E_ARG; }
+  } else {
+    SETUP_CUDA(cudaMemsetAsync(d.vt, 0, (size_t)L.n_vox_pad * 4, q));
+  }
 
   // ---- CSR of D^T: expand, count columns, stable radix sort on the column index ----
   const int64_t ntc = tchunks_of(dm.nnz);

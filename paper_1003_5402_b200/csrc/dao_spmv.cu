@@ -63,6 +63,7 @@ struct SpmvParams {
   float *g;
   const uint8_t *sid;
   const StructEntry *stab;
+  const float *vt;           // per-voxel thresholds (re-optimisation mode) or null
   const int32_t *perm;
   double *f_part;
   DevState *st;
@@ -76,7 +77,8 @@ __device__ __forceinline__ void spmv_store(const SpmvParams &p, float *out, cons
     const int s = p.sid[i];
     double gv = 0.0;
     if (s != kNoStruct) {
-      const StructEntry e = stab_s[s];
+      StructEntry e = stab_s[s];
+      if (p.vt) e.tm = e.tp = (double)p.vt[i];       // T_j of eq. 3-4
       const double u = fmax(e.tm - acc, 0.0);
       const double o = fmax(acc - e.tp, 0.0);
       f_acc += e.a * u * u + e.b * o * o;
@@ -299,6 +301,7 @@ static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out) {
   p.out = out;
   p.g = c->d.g;
   p.sid = c->d.sid;
+  p.vt = c->has_vt ? c->d.vt : nullptr;
   p.stab = c->d.stab;
   p.perm = c->d.perm;
   p.f_part = c->d.f_part;

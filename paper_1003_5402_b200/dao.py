@@ -50,7 +50,8 @@ class CMlc(C.Structure):
 
 class CStructs(C.Structure):
     _fields_ = [("n_struct", C.c_int32), ("vox_struct", C.c_void_p), ("t_under", C.c_void_p),
-                ("w_under", C.c_void_p), ("t_over", C.c_void_p), ("w_over", C.c_void_p)]
+                ("w_under", C.c_void_p), ("t_over", C.c_void_p), ("w_over", C.c_void_p),
+                ("vox_threshold", C.c_void_p), ("per_voxel_weights", C.c_int32)]
 
 
 class COptions(C.Structure):
@@ -195,6 +196,20 @@ class Dao:
             csr.row_ptr, csr.col_idx, csr.val, csr.mem = _np_ptr(row_ptr), _np_ptr(col_idx), _np_ptr(val), MEM_HOST
             st.vox_struct = _np_ptr(vs)
         st.t_under, st.w_under, st.t_over, st.w_over = _np_ptr(tu), _np_ptr(wu), _np_ptr(to), _np_ptr(wo)
+        # re-optimisation mode: per-voxel thresholds T_j, weights not divided by |v_s|
+        vt = getattr(ph, "vox_threshold", None)
+        st.per_voxel_weights = 1 if getattr(ph, "per_voxel_weights", False) else 0
+        if vt is not None:
+            vt = np.ascontiguousarray(vt, dtype=np.float32)
+            if vt.size != self.n_vox:
+                raise ValueError("vox_threshold must have n_vox entries")
+            if device_inputs:
+                d_vt = torch.from_numpy(vt).cuda()
+                self._keep.append(d_vt)
+                st.vox_threshold = d_vt.data_ptr()
+            else:
+                self._keep.append(vt)
+                st.vox_threshold = _np_ptr(vt)
         mlc = CMlc(self.n_beams, self.n_rows, _np_ptr(brp), _np_ptr(rbp))
 
         sizes = CSizes()

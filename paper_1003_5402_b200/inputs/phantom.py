@@ -109,6 +109,10 @@ class Phantom:
     grid: Tuple[int, int, int] = (0, 0, 0)
     voxel_mm: float = 0.0
     prescription: float = 1.0                     # the largest target prescription
+    # re-optimisation mode: per-voxel threshold T_j replacing T_s^- and T_s^+, and
+    # weights used as they are (eq. 3-4) instead of divided by |v_s| (eq. 9-10)
+    vox_threshold: Optional[np.ndarray] = None    # float32 [n_vox] or None
+    per_voxel_weights: bool = False
 
     def summary(self) -> Dict[str, object]:
         rows = np.diff(self.row_bl_ptr)
@@ -423,7 +427,55 @@ CONFIGS = {
 
 
 def make(config: str, seed: int = 0) -> Phantom:
+    """``config`` is a key of CONFIGS, optionally followed by ``_reopt`` (re-optimisation mode)."""
+    if config.endswith("_reopt"):
+        return reoptimisation(generate(CONFIGS[config[:-6]](), seed), seed)
     return generate(CONFIGS[config](), seed)
+
+
+# --------------------------------------------------------------------------- re-optimisation inputs
+def reoptimisation(ph: Phantom, seed: int = 0, falloff_mm: float = 25.0, shift_mm: float = 4.0,
+                   ripple: float = 0.03) -> Phantom:
+    """The same geometry posed as the paper's re-optimisation problem: alpha_j =
+    beta_j = 1, T_j = "the dose distribution from the original plan, deformed to the daily image".
+
+    The clinical reference doses are not available, so T_j is a smooth synthetic stand-in with the
+    shape of a delivered plan: the prescription inside a target-sized ball around the (shifted)
+    target centroid, an exponential fall-off with distance outside it, and a seeded low-frequency
+    ripple (the "deformation").  Structures become 0 = target voxels (under- and over-dose
+    penalised, eq. 3-4) and 1 = all other voxels (over-dose only).  No method arithmetic here."""
+    rng = np.random.default_rng(seed + 7919)
+    nx, ny, nz = ph.grid
+    lin = ph.vox_grid_index
+    ix, iy, iz = lin % nx, (lin // nx) % ny, lin // (nx * ny)
+    h = ph.voxel_mm
+    x = (ix - (nx - 1) / 2.0) * h
+    y = (iy - (ny - 1) / 2.0) * h
+    z = (iz - (nz - 1) / 2.0) * h
+    is_target = np.zeros(ph.n_vox, dtype=bool)
+    for s in range(ph.n_struct):
+        if ph.w_under[s] > 0:
+            is_target |= ph.vox_struct == s
+    c = np.array([x[is_target].mean(), y[is_target].mean(), z[is_target].mean()])
+    c = c + rng.uniform(-shift_mm, shift_mm, size=3)
+    radius = (3.0 * is_target.sum() * h ** 3 / (4.0 * np.pi)) ** (1.0 / 3.0)
+    d = np.sqrt((x - c[0]) ** 2 + (y - c[1]) ** 2 + (z - c[2]) ** 2)
+    t = ph.prescription * np.exp(-np.maximum(d - radius, 0.0) / falloff_mm)
+    ph_x, ph_y, ph_z = rng.uniform(0.0, 2.0 * np.pi, size=3)
+    t = t * (1.0 + ripple * np.sin(x / 37.0 + ph_x) * np.sin(y / 41.0 + ph_y) * np.sin(z / 29.0 + ph_z))
+    import copy
+    q = copy.copy(ph)
+    q.name = ph.name + "_reopt"
+    q.n_struct = 2
+    q.vox_struct = np.where(is_target, 0, 1).astype(np.int32)
+    q.t_under = np.zeros(2, dtype=np.float32)
+    q.t_over = np.zeros(2, dtype=np.float32)
+    q.w_under = np.array([1.0, 0.0], dtype=np.float32)
+    q.w_over = np.array([1.0, 1.0], dtype=np.float32)
+    q.struct_names = ["target", "other"]
+    q.vox_threshold = t.astype(np.float32)
+    q.per_voxel_weights = True
+    return q
 
 
 # --------------------------------------------------------------------------- kernel-sweep inputs

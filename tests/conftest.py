@@ -61,3 +61,10 @@ def cfg0():
 def mini():
     from paper_1003_5402_b200.inputs import phantom
     return phantom.make("mini", seed=0)
+
+
+@pytest.fixture(scope="session")
+def mini_reopt():
+    """`mini` posed as the paper's re-optimisation problem: per-voxel T_j, alpha = beta = 1."""
+    from paper_1003_5402_b200.inputs import phantom
+    return phantom.make("mini_reopt", seed=0)

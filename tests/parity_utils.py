@@ -71,7 +71,7 @@ def check_beam(beam_price_gpu, best_gpu, beam_price_orc, rel_gap=1e-6):
 
 def oracle_state_from_plan(ph, beams, lefts, rights, y):
     """z, g, w of the oracle at the intensities (y over the given apertures)."""
-    vp = orc.voxel_params(ph.vox_struct, ph.t_under, ph.w_under, ph.t_over, ph.w_over)
+    vp = orc.voxel_params_of(ph)
     K = len(beams)
     max_rows = int(np.max(np.diff(ph.beam_row_ptr)))
     L = np.zeros((K, max_rows), np.int32); R = np.zeros_like(L)

@@ -86,10 +86,10 @@ def test_spmv_independent_of_sell_window(D, mini, sigma):
 
 
 # ----------------------------------------------------------------------------- step 3 (fused epilogue)
-@pytest.mark.parametrize("case", ["cfg0", "mini"])
-def test_objective_and_gradient_match_oracle(D, case, cfg0, mini):
-    ph = {"cfg0": cfg0, "mini": mini}[case]
-    vp = orc.voxel_params(ph.vox_struct, ph.t_under, ph.w_under, ph.t_over, ph.w_over)
+@pytest.mark.parametrize("case", ["cfg0", "mini", "mini_reopt"])
+def test_objective_and_gradient_match_oracle(D, case, cfg0, mini, mini_reopt):
+    ph = {"cfg0": cfg0, "mini": mini, "mini_reopt": mini_reopt}[case]
+    vp = orc.voxel_params_of(ph)
     rng = np.random.default_rng(11)
     with D.Dao(ph) as d:
         for scale in (0.0, 0.02, 0.05, 0.2):
@@ -101,8 +101,13 @@ def test_objective_and_gradient_match_oracle(D, case, cfg0, mini):
             assert abs(F - Fo) <= 1e-12 * max(Fo, 1e-30)
             assert np.abs(z - zo).max() <= REL_DOSE * ph.prescription
             assert np.abs(g - go).max() <= REL_DOSE * max(np.abs(go).max(), 1e-30)
-    # closed form: F(z = 0) = sum over targets of alpha_s (T_s^-)^2
-    assert abs(orc.objective(np.zeros(ph.n_vox), vp) - 10.0) < 1e-12
+    if case == "mini_reopt":
+        # closed form (PAPER.md:75-83 with alpha = beta = 1): F(z = 0) = sum over target voxels of T_j^2
+        t = ph.vox_threshold.astype(np.float64)
+        assert abs(orc.objective(np.zeros(ph.n_vox), vp) - float((t[ph.vox_struct == 0] ** 2).sum())) < 1e-9
+    else:
+        # closed form: F(z = 0) = sum over targets of alpha_s (T_s^-)^2
+        assert abs(orc.objective(np.zeros(ph.n_vox), vp) - 10.0) < 1e-12
 
 
 # ----------------------------------------------------------------------------- steps 5, 6
@@ -150,11 +155,11 @@ def test_pricing_on_own_tables(D, mini):
 
 
 # ----------------------------------------------------------------------------- lock-step protocol
-@pytest.mark.parametrize("case,n_ap", [("cfg0", 12), ("mini", 20)])
-def test_lockstep_against_oracle(D, case, n_ap, cfg0, mini):
+@pytest.mark.parametrize("case,n_ap", [("cfg0", 12), ("mini", 20), ("mini_reopt", 12)])
+def test_lockstep_against_oracle(D, case, n_ap, cfg0, mini, mini_reopt):
     """SURVEY 8(c) lock-step: at every column-generation iteration the oracle recomputes each step
     from the GPU's own state; isolates every step's error from trajectory divergence."""
-    ph = {"cfg0": cfg0, "mini": mini}[case]
+    ph = {"cfg0": cfg0, "mini": mini, "mini_reopt": mini_reopt}[case]
     with D.Dao(ph, k_max=n_ap) as d:
         for it in range(n_ap):
             info = d.price()
@@ -207,9 +212,9 @@ def test_master_on_oracle_pool(D, mini):
 
 
 # ----------------------------------------------------------------------------- free-running plans
-@pytest.mark.parametrize("case", ["cfg0", "mini"])
-def test_free_running_50_apertures(D, case, cfg0, mini):
-    ph = {"cfg0": cfg0, "mini": mini}[case]
+@pytest.mark.parametrize("case", ["cfg0", "mini", "mini_reopt"])
+def test_free_running_50_apertures(D, case, cfg0, mini, mini_reopt):
+    ph = {"cfg0": cfg0, "mini": mini, "mini_reopt": mini_reopt}[case]
     with D.Dao(ph) as d:
         info = d.run(50)
         plan = d.get_plan()
