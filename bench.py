@@ -92,6 +92,23 @@ def algorithmic_bytes(ph, sell_elems=None):
     }
 
 
+def reduce_max(x: float, world: int, device: str = "cuda") -> float:
+    """Max over ranks of a per-rank device time (torch.distributed all-reduce; NCCL on the GPU box,
+    gloo in the CPU tests).  The multi-rank path has no data-path collective: ranks are replicas."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_seconds_per_plan(elapsed_max: float, steps: int, world: int) -> float:
+    """Whole-job metric: `world` replicas each finish `steps` plans in `elapsed_max` seconds."""
+    return elapsed_max / (steps * world)
+
+
 def run_reference(args, rank, world):
     """The reference arm: the oracle, as it stands, on the host cores; bounded sample."""
     if rank != 0:
@@ -196,11 +213,8 @@ def main():
     barrier()
     clocks = sampler.stop()
     elapsed = ev0.elapsed_time(ev1) * 1e-3
-    if world > 1:
-        t = torch.tensor([elapsed], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        elapsed = float(t.item())
-    sec_per_plan = elapsed / (args.steps * world)          # whole job: N replicas produce N plans per step
+    elapsed = reduce_max(elapsed, world)
+    sec_per_plan = job_seconds_per_plan(elapsed, args.steps, world)   # N replicas produce N plans per step
     last = infos[-1]
     n_it = sum(i.n_iterations for i in infos)
 
@@ -258,10 +272,7 @@ def main():
             if i > 0:
                 ts.append(time.perf_counter() - t0)
         e = float(np.mean(ts))
-        if world > 1:
-            t = torch.tensor([e], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e = float(t.item())
+        e = reduce_max(e, world)
         e2e = {"value": e / world, "unit": "s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                "includes": "dao_create from pinned host CSR (H2D + sliced-ELL + transpose build), dao_run(50), dao_get_plan"}
 

@@ -1,0 +1,149 @@
+"""GPU parity at BASELINE.json's full size: configs[1] (the 9-field prostate phantom bench.py times),
+in the launch configuration of bench.py (default options, k_max = 50).
+
+The oracle's O(nnz) steps (dose, gradient, beamlet gradient, pricing) are cheap enough to be compared
+element by element at this size; the oracle's free-running 50-aperture plan takes ~2.5 min on one
+core, so its result is a stored fixture (tests/golden/oracle_plan_cfg1.json, written by
+tests/golden/make_oracle_plan.py from oracle/ only).  Tolerances: the north star's.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from oracle import dao_oracle as orc
+from paper_1003_5402_b200.inputs import phantom
+import parity_utils as pu
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+REL_DOSE = 1e-4
+REL_OBJ = 1e-3
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+@pytest.fixture(scope="module")
+def D():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1003_5402_b200 import dao
+    dao.load_library()
+    return dao
+
+
+@pytest.fixture(scope="module")
+def cfg1():
+    return phantom.make("cfg1", seed=0)
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _leaves(plan):
+    K = len(plan.beams)
+    return [plan.leaves(k)[0] for k in range(K)], [plan.leaves(k)[1] for k in range(K)]
+
+
+def test_cfg1_kernels_match_oracle(D, cfg1):
+    """Steps 2, 3, 4 on all 603,844 voxels / 4,337 beamlets / 47.2M non-zeros, element by element."""
+    ph = cfg1
+    rng = np.random.default_rng(21)
+    x = (0.05 * rng.random(ph.n_bl)).astype(np.float32)
+    gin = rng.standard_normal(ph.n_vox).astype(np.float32)
+    vp = orc.voxel_params_of(ph)
+    with D.Dao(ph, k_max=50) as d:
+        z = d.spmv(_dev(x)).cpu().numpy()
+        w = d.spmv_t(_dev(gin)).cpu().numpy()
+        F = d.eval_x(_dev(x))
+        zz, g = d.get_vector(D.VEC_Z), d.get_vector(D.VEC_G)
+    zo = orc.dose(ph.row_ptr, ph.col_idx, ph.val, x.astype(np.float64))
+    wo = orc.beamlet_gradient(ph.row_ptr, ph.col_idx, ph.val, gin.astype(np.float64), ph.n_bl)
+    Fo, go = orc.objective(zo, vp), orc.voxel_gradient(zo, vp)
+    assert np.abs(z - zo).max() <= REL_DOSE * ph.prescription
+    assert np.abs(zz - zo).max() <= REL_DOSE * ph.prescription
+    assert np.abs(w - wo).max() <= REL_DOSE * np.abs(wo).max()
+    assert np.abs(g - go).max() <= REL_DOSE * np.abs(go).max()
+    assert abs(F - Fo) <= 1e-10 * Fo
+    # adjoint identity at full size (independent of either implementation's own arithmetic)
+    lhs = float(np.dot(w.astype(np.float64), x.astype(np.float64)))
+    rhs = float(np.dot(gin.astype(np.float64), z.astype(np.float64)))
+    assert abs(lhs - rhs) <= 1e-5 * max(abs(lhs), abs(rhs), 1e-30)
+
+
+def test_cfg1_lockstep_first_iterations(D, cfg1):
+    """Lock-step protocol on the first 3 column-generation iterations at full size:
+    the oracle recomputes every step from the GPU's own state, prices the GPU's fp32 w, and solves
+    the master on the GPU's pool."""
+    ph = cfg1
+    with D.Dao(ph, k_max=50) as d:
+        for it in range(3):
+            info = d.price()
+            plan = d.get_plan()
+            K = len(plan.beams)
+            y = d.get_vector(D.VEC_Y)[:K]
+            lefts, rights = _leaves(plan)
+            vp, _, z_o, g_o, w_o, F_o = pu.oracle_state_from_plan(ph, plan.beams, lefts, rights, y)
+            z, g, w = d.get_vector(D.VEC_Z), d.get_vector(D.VEC_G), d.get_vector(D.VEC_W)
+            assert np.abs(z - z_o).max() <= REL_DOSE * ph.prescription
+            assert np.abs(g - g_o).max() <= REL_DOSE * np.abs(g_o).max()
+            assert np.abs(w - w_o).max() <= REL_DOSE * np.abs(w_o).max()
+            assert abs(info.objective - F_o) <= 1e-6 * F_o
+            le, ri, vs = d.get_vector(D.VEC_LEFT), d.get_vector(D.VEC_RIGHT), d.get_vector(D.VEC_VSTAR)
+            n_exact, n_band = pu.check_rows(w, ph.row_bl_ptr, le, ri, vs)
+            assert n_exact + n_band == ph.n_rows
+            pr = orc.price(w.astype(np.float64), ph.beam_row_ptr, ph.row_bl_ptr)
+            pu.check_beam(d.get_vector(D.VEC_BEAM_PRICE), info.beam, pr.beam_price)
+            assert not info.converged
+            m = d.solve_master()
+            assert m.n_apertures == it + 1 and not m.hit_max_iter
+            plan = d.get_plan()
+            lefts, rights = _leaves(plan)
+            A = pu.oracle_columns(ph, plan.beams, lefts, rights)
+            res = orc.master(A, np.zeros(len(plan.beams)), vp, tol=1e-10)
+            rel = (m.objective - res.objective) / res.objective
+            assert -1e-5 <= rel <= REL_OBJ, (it, m.objective, res.objective)
+
+
+def test_cfg1_plan_50_apertures(D, cfg1):
+    """The north-star target: a free-running 50-aperture plan of configs[1], run exactly as bench.py
+    runs it, against (i) the oracle's own free-running plan (stored fixture), (ii) the oracle's
+    recomputation of dose / objective / reduced costs from the GPU's plan."""
+    ph = cfg1
+    with open(os.path.join(GOLDEN, "oracle_plan_cfg1.json")) as f:
+        gold = json.load(f)
+    assert (gold["n_vox"], gold["n_bl"], gold["nnz"]) == (ph.n_vox, ph.n_bl, ph.nnz)
+    with D.Dao(ph, k_max=50) as d:
+        info = d.run(50)
+        plan = d.get_plan()
+        hist = d.get_vector(D.VEC_HISTORY)[:info.n_apertures]
+        z = d.get_vector(D.VEC_Z)
+        y = d.get_vector(D.VEC_Y)[:info.n_apertures]
+    assert info.n_apertures == 50 and not info.converged
+    # (i) free-running objective within 1e-3 of the oracle's (north star)
+    rel = abs(info.objective - gold["objective"]) / gold["objective"]
+    assert rel <= REL_OBJ, (info.objective, gold["objective"])
+    n_same = sum(int(a == b) for a, b in zip(plan.beams.tolist(), gold["beams"]))
+    # per-iteration master optimum follows the oracle's trajectory as long as both pick the same apertures
+    f_gpu, f_or = hist["objective"], np.asarray(gold["master_objective"])
+    assert (np.abs(f_gpu - f_or) <= REL_OBJ * f_or).all()
+    # (ii) the oracle at the GPU's plan
+    lefts, rights = _leaves(plan)
+    vp, _, z_o, g_o, w_o, F_o = pu.oracle_state_from_plan(ph, plan.beams, lefts, rights, y)
+    assert np.abs(z - z_o).max() <= REL_DOSE * ph.prescription
+    assert abs(info.objective - F_o) <= 1e-6 * F_o
+    # reduced cost of pool aperture k = sum of w over its open beamlets (eq. 2 and 8): KKT of the master
+    grad = np.zeros(50)
+    for k, b in enumerate(plan.beams):
+        m = orc.aperture_open_mask(ph.n_bl, int(b), lefts[k], rights[k], ph.beam_row_ptr, ph.row_bl_ptr)
+        grad[k] = w_o[m.astype(bool)].sum()
+    # first-order bound on the master's suboptimality (convexity): F(y) - F* <= grad.y - min(0, min grad) * |y*|_1,
+    # with |y*|_1 taken as 2 |y|_1
+    gap = float(grad @ y) + max(0.0, -grad.min()) * 2.0 * y.sum()
+    assert gap <= REL_OBJ * F_o, (gap, F_o)
+    f = np.r_[hist["objective_before"][:1], hist["objective"]]
+    assert (np.diff(f) <= 1e-9 * f[:-1]).all() and (hist["price"] < 0).all() and (plan.intensity >= 0).all()
+    print(f"cfg1: F_gpu={info.objective:.12g} F_oracle={gold['objective']:.12g} rel={rel:.2e} same beams {n_same}/50 "
+          f"pg iterations {info.n_pg_iter_total} kkt gap {gap:.2e}")
