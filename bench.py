@@ -92,6 +92,24 @@ def algorithmic_bytes(ph, sell_elems=None):
     }
 
 
+def ncu_traffic(kernel: str):
+    """DRAM bytes per launch of `kernel` from the newest profiles/*_traffic.csv (one `ncu --set full`
+    capture, see the .md beside it); None when no capture is committed."""
+    import csv
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv")))
+    if not files:
+        return None
+    try:
+        with open(files[-1]) as f:
+            for row in csv.DictReader(f):
+                if row["kernel"] == kernel:
+                    return int(row["dram_bytes_per_launch"])
+    except Exception:
+        pass
+    return None
+
+
 def reduce_max(x: float, world: int, device: str = "cuda") -> float:
     """Max over ranks of a per-rank device time (torch.distributed all-reduce; NCCL on the GPU box,
     gloo in the CPU tests).  The multi-rank path has no data-path collective: ranks are replicas."""
@@ -240,18 +258,13 @@ def main():
                               "note": "dense block A (4*V*K bytes <= L2) is L2-resident: GB/s is not an HBM figure"})
     plan_bytes = N_APERTURES * (ab["spmv"] + ab["spmv_t"] + ab["price"] + ab["column"]) + master_bytes_plan
     spmv = kernels["spmv"]
-    roofline = {"kernel": "k_spmv_sell (dose SpMV + fused objective/gradient)", "bound": "hbm",
+    roofline = {"kernel": "k_spmv_ring<0> (dose SpMV + fused objective/gradient)", "bound": "hbm",
                 "achieved": spmv.get("GBps"), "peak": peak, "unit": "GB/s", "frac": spmv.get("frac_of_hbm_peak"),
                 "traffic": None, "peak_source": peak_src, "alg_bytes_per_launch": ab["spmv"],
                 "avg_launch_us": spmv["avg_us"], "share_of_step": spmv["share"],
                 "dominant_by_time": max(kernels, key=lambda k: kernels[k]["share"] or 0),
                 "sell_padding": dims.sell_elems / max(1, ph.nnz)}
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(traffic_file):
-        try:
-            roofline["traffic"] = json.load(open(traffic_file)).get("k_spmv_sell")
-        except Exception:
-            pass
+    roofline["traffic"] = ncu_traffic("k_spmv_ring<0>")
 
     # ---- e2e: host (pinned) buffers -> dao_create -> dao_run -> dao_get_plan, wall clock ----
     e2e = None

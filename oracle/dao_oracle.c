@@ -439,3 +439,51 @@ double orc_master_gradient(int32_t n_vox, int32_t K, const double *A, const doub
     free(z); free(g);
     return f;
 }
+
+/* ------------------------------------------------------------------ FMO
+ * Fluence-map optimisation: the same objective with the beamlet intensities themselves as the
+ * decision variables, min_{x >= 0} F(D x) -- "Mathematically, the DAO model is the same as the FMO
+ * model ... in which the decision variables are the intensities of all beamlets", solved
+ * with "the same gradient projection method".  By eq. (7) every
+ * aperture plan is a beamlet plan, so F*_FMO is a lower bound of every DAO objective.
+ *
+ * Plain gradient projection on the sparse D, the statement of orc_master_pg with A = D^T: direction
+ * p_i = -w_i (w = D^T pi, eq. 8's inner sum) except p_i = 0 where x_i = 0 and w_i > 0; exact step along
+ * the feasible ray, capped at the first bound.  Stops when max_i |p_i| * max(1, max x) <= tol * F or
+ * after max_iter iterations.  Returns the iteration count; *f_out = F(D x), *kkt_out = KKT residual. */
+int32_t orc_fmo_pg(int32_t n_vox, int32_t n_bl, const int32_t *row_ptr, const int32_t *col_idx,
+                   const float *val, double *x, const double *a, const double *b, const double *tm,
+                   const double *tp, double tol, int32_t max_iter, double *f_out, double *kkt_out)
+{
+    double *z = (double *)malloc(sizeof(double) * (size_t)n_vox);
+    double *g = (double *)malloc(sizeof(double) * (size_t)n_vox);
+    double *dz = (double *)malloc(sizeof(double) * (size_t)n_vox);
+    double *w = (double *)malloc(sizeof(double) * (size_t)(n_bl > 0 ? n_bl : 1));
+    double *p = (double *)malloc(sizeof(double) * (size_t)(n_bl > 0 ? n_bl : 1));
+    int32_t it = 0;
+    double f = 0.0;
+    for (;;) {
+        orc_dose(n_vox, row_ptr, col_idx, val, x, z);
+        f = orc_objective(n_vox, z, a, b, tm, tp);
+        orc_voxel_gradient(n_vox, z, a, b, tm, tp, g);
+        orc_beamlet_gradient(n_vox, n_bl, row_ptr, col_idx, val, g, w);
+        double pmax = 0.0;
+        for (int32_t i = 0; i < n_bl; ++i) {
+            p[i] = (x[i] <= 0.0 && w[i] > 0.0) ? 0.0 : -w[i];
+            if (fabs(p[i]) > pmax) pmax = fabs(p[i]);
+        }
+        if (pmax * ymax1(n_bl, x) <= tol * (f > 1e-300 ? f : 1e-300) || it >= max_iter) break;
+        double t_max = INFINITY; int32_t ib = -1;
+        for (int32_t i = 0; i < n_bl; ++i)
+            if (p[i] < 0.0) { double t = x[i] / (-p[i]); if (t < t_max) { t_max = t; ib = i; } }
+        orc_dose(n_vox, row_ptr, col_idx, val, p, dz);
+        int hit = 0;
+        double t = exact_step(n_vox, z, dz, t_max, a, b, tm, tp, &hit);
+        for (int32_t i = 0; i < n_bl; ++i) { x[i] += t * p[i]; if (x[i] < 0.0) x[i] = 0.0; }
+        if (hit && ib >= 0) x[ib] = 0.0;
+        ++it;
+    }
+    *f_out = f; *kkt_out = kkt_residual(n_bl, x, w);
+    free(z); free(g); free(dz); free(w); free(p);
+    return it;
+}

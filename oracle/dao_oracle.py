@@ -40,6 +40,7 @@ def lib():
         _lib.orc_master_gradient.restype = C.c_double
         _lib.orc_master_pg.restype = C.c_int32
         _lib.orc_master_newton.restype = C.c_int32
+        _lib.orc_fmo_pg.restype = C.c_int32
     return _lib
 
 
@@ -226,6 +227,31 @@ def master_gradient(A, y, vp: VoxelParams):
     f = lib().orc_master_gradient(C.c_int32(n_vox), C.c_int32(K), _p(A), _p(y), _p(vp.a), _p(vp.b),
                                   _p(vp.tm), _p(vp.tp), _p(grad))
     return float(f), grad
+
+
+def dense_transpose(ph) -> np.ndarray:
+    """D^T as a dense [n_bl, n_vox] fp64 array (small instances only): the "aperture" block whose
+    columns are the single beamlets, i.e. the FMO model in the master's notation."""
+    A = np.zeros((ph.n_bl, ph.n_vox), dtype=np.float64)
+    rp = _i32(ph.row_ptr)
+    rows = np.repeat(np.arange(ph.n_vox), np.diff(rp))
+    A[_i32(ph.col_idx), rows] = _f32(ph.val).astype(np.float64)
+    return A
+
+
+def fmo(ph, x0=None, tol: float = 1e-10, max_iter: int = 20000, method: str = "newton") -> MasterResult:
+    """FMO: min_{x >= 0} F(D x) over the beamlet intensities.
+    method 'pg' = plain gradient projection on the sparse D (orc_fmo_pg, any size); 'newton' = the
+    master's projected Newton on the dense D^T (small instances; same optimum value by convexity)."""
+    vp = voxel_params_of(ph)
+    x = np.zeros(ph.n_bl) if x0 is None else _f64(x0).copy()
+    if method == "newton":
+        return master(dense_transpose(ph), x, vp, tol, max_iter, "newton")
+    rp, ci, v = _i32(ph.row_ptr), _i32(ph.col_idx), _f32(ph.val)
+    f = C.c_double(0.0); kkt = C.c_double(0.0)
+    it = lib().orc_fmo_pg(C.c_int32(ph.n_vox), C.c_int32(ph.n_bl), _p(rp), _p(ci), _p(v), _p(x), _p(vp.a), _p(vp.b),
+                          _p(vp.tm), _p(vp.tp), C.c_double(tol), C.c_int32(max_iter), C.byref(f), C.byref(kkt))
+    return MasterResult(x, f.value, int(it), kkt.value)
 
 
 # ----------------------------------------------------------------------------- driver (O9)
