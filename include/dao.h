@@ -273,6 +273,33 @@ dao_status dao_set_pool(dao_ctx *ctx, int32_t n_apertures, const int32_t *beam, 
 /* Solve the restricted master over the current pool without adding a column. */
 dao_status dao_resolve_master(dao_ctx *ctx, dao_master_info *out);
 
+/* ---- FMO workload ------------------------------------------------------------------
+ * Fluence-map optimisation: the same objective with the beamlet intensities as the decision
+ * variables, min_{x >= 0} F(D x).  "Mathematically, the DAO model is the same as the FMO model ...
+ * in which the decision variables are the intensities of all beamlets", solved by "the same gradient
+ * projection method".  By eq. (7) its optimum is a lower bound
+ * of every aperture plan's objective.  Runs steps 2-4 of the hot path (dose SpMV + fused objective /
+ * gradient, transposed SpMV) plus a projected-gradient update per iteration, entirely on the device;
+ * the host reads a small state block every `check_every` iterations. */
+typedef struct {
+  int32_t n_iter;            /* projected-gradient iterations done */
+  int32_t converged;         /* 2: F stopped decreasing beyond fp64 rounding (resolution of the fp32 gradient);
+                                1: max_i |x_i - max(0, x_i - t w_i)| / t * max(1, max x) <= tol * F, t = last step */
+  int32_t hit_max_iter;
+  int32_t n_restarts;        /* steepest-descent restarts of the conjugated direction */
+  int32_t n_ls_evals;        /* line-search evaluations of phi'(t) (passes over z, dz only) */
+  int32_t reserved;
+  double objective;          /* F(D x) at the returned x */
+  double kkt_residual;       /* that measure over x_i > 0, and max(0, -w_i) where x_i = 0 */
+  double pg_norm;            /* max_i |p_i| of the projected steepest-descent direction */
+  double seconds;            /* device time of the solve */
+} dao_fmo_info;
+/* Solve from x = 0 (warm_start = 0) or from the context's current DAO_VEC_X (warm_start = 1).
+ * tol <= 0 selects dao_options.master_tol; the conjugation follows dao_options.master_method.  On
+ * return DAO_VEC_X / DAO_VEC_Z / DAO_VEC_G / DAO_VEC_W describe the returned x.  The aperture pool of
+ * the context is not touched, but its last dose evaluation is overwritten. */
+dao_status dao_fmo_solve(dao_ctx *ctx, int32_t max_iter, double tol, int32_t warm_start, dao_fmo_info *out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -477,4 +477,12 @@ dao_status dao_set_pool(dao_ctx *ctx, int32_t n_apertures, const int32_t *beam, 
   return DAO_OK;
 }
 
+dao_status dao_fmo_solve(dao_ctx *ctx, int32_t max_iter, double tol, int32_t warm_start, dao_fmo_info *out) {
+  Ctx *c = reinterpret_cast<Ctx *>(ctx);
+  if (!c) return DAO_E_ARG;
+  if (max_iter < 0) return fail(c, DAO_E_ARG, "max_iter must be >= 0");
+  c->have_candidate = false;          // the pending candidate was priced at a dose that is being overwritten
+  return fmo_solve(c, max_iter, tol, warm_start != 0, out);
+}
+
 }  // extern "C"

@@ -30,6 +30,7 @@ constexpr int kMasterMaxGrid = 160;    // CTAs of the master kernel (one per SM,
 constexpr int kMasterProfSlots = 16;   // phase timers of the master (ns): 0 init, 1 G pass, 2 G reduce, 3 direction,
                                        // 4 D pass, 5 D reduce, 6 line search; 7 line-search evaluations,
                                        // 8 iterations, 9 calls, 10 publish
+constexpr int kFmoLsGridMax = 1024;   // CTAs of the FMO line-search kernels
 constexpr int kMaxStruct = 255;
 constexpr int kNoStruct = 255;         // sid value of a voxel without penalty
 constexpr int kMaxRedux = DAO_MAX_APERTURES + 8;   // doubles per grid reduction in the master
@@ -68,6 +69,32 @@ struct DevState {
   int64_t pg_iter_total;
   int32_t n_duplicates;
   int32_t pad_;
+};
+
+// Device state of the FMO solve (dao_fmo.cu); the host reads it every few iterations.
+struct FmoState {
+  double F;                // objective at the current x
+  double slope0;           // phi'(0) = p . w
+  double tmax;             // largest feasible step along p
+  double t;                // current trial / accepted step
+  double lo, slo, hi, shi; // bracket of the root of phi' (hi = inf: none yet)
+  double c1, c2;           // phi'(t), phi''(t) of the last evaluation
+  double pg_max, kkt, x_max;
+  double F_prev;           // objective of the previous iteration (stall detection)
+  double t_est;            // bending horizon of the next direction (2 x the last accepted step; 0: none)
+  int32_t done;            // 1: converged or iteration cap; every FMO kernel returns at once
+  int32_t converged;
+  int32_t hit_max;
+  int32_t iters;
+  int32_t ls_done;         // 1: the step t is accepted
+  int32_t at_bound;        // accepted step ends on the bound of variable ib
+  int32_t ib;
+  int32_t force_restart;
+  int32_t since_restart;
+  int32_t restarts;
+  int32_t ls_evals;
+  int32_t stall;           // consecutive iterations without a decrease of F beyond fp64 rounding
+  uint32_t ticket;
 };
 
 struct StructEntry {       // per-structure penalty parameters of eq. (9)-(10), already divided by |v_s|
@@ -129,6 +156,12 @@ struct DevPtrs {
   uint4 *ll_result;        // [2][kMaxRedux]
   uint32_t *m_epoch;       // reduction epoch (monotone over the life of the context)
   unsigned long long *m_prof;  // [kMasterProfSlots]
+  // FMO workload
+  float *fmo_p;            // [n_bl] search direction (fp32 values: x += t p and dz = D p stay consistent)
+  float *fmo_pgold;        // [n_bl] previous projected steepest-descent direction
+  float *fmo_dz;           // [n_vox_pad] dz = D p, internal order
+  double *fmo_part;        // [2 * kFmoLsGridMax] block partials of the line-search sums
+  FmoState *fmo_state;
   // history
   dao_iter_record *history;  // [k_max]
   DevState *state;
@@ -191,8 +224,9 @@ dao_status setup_sizes(const dao_csr *D, const dao_mlc *mlc, const dao_structs *
 
 // dao_spmv.cu
 enum SpmvMode { kSpmvObjective = 0, kSpmvPlain = 1, kSpmvColumn = 2, kSpmvPlainUserOrder = 3 };
-cudaError_t launch_spmv(Ctx *c, SpmvMode mode, const float *x, float *out);
-cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out);
+// `skip` (device, may be null): when *skip != 0 the kernels return at once (device-side loop control)
+cudaError_t launch_spmv(Ctx *c, SpmvMode mode, const float *x, float *out, const int32_t *skip = nullptr);
+cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out, const int32_t *skip = nullptr);
 cudaError_t launch_intensity(Ctx *c);
 void spmv_configure(Ctx *c);
 
@@ -202,6 +236,9 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
                            double *row_absmax, double *beam_price, double *beam_absmax, int32_t *best_out,
                            bool update_state);
 cudaError_t launch_append_candidate(Ctx *c);
+
+// dao_fmo.cu
+dao_status fmo_solve(Ctx *c, int32_t max_iter, double tol, bool warm_start, dao_fmo_info *out);
 
 // dao_master.cu
 cudaError_t master_configure(Ctx *c);

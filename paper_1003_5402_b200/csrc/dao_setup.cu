@@ -144,6 +144,11 @@ static void carve_workspace(Carver &cv, const Dims &dm, const HostLayout &L, Dev
   }
   d->m_epoch = cv.take<uint32_t>(64);
   d->m_prof = cv.take<unsigned long long>(kMasterProfSlots);
+  d->fmo_p = cv.take<float>((size_t)dm.n_bl);
+  d->fmo_pgold = cv.take<float>((size_t)dm.n_bl);
+  d->fmo_dz = cv.take<float>(vp);
+  d->fmo_part = cv.take<double>(2 * (size_t)kFmoLsGridMax);
+  d->fmo_state = cv.take<FmoState>(1);
   d->history = cv.take<dao_iter_record>((size_t)dm.k_max);
   d->state = cv.take<DevState>(1);
   d->io_scratch = cv.take<double>(std::max<size_t>(vp, (size_t)std::max(dm.n_bl, dm.n_rows)) + 64);

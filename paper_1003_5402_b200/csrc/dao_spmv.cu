@@ -67,6 +67,7 @@ struct SpmvParams {
   const int32_t *perm;
   double *f_part;
   DevState *st;
+  const int32_t *skip;       // device flag (may be null): non-zero -> the launch does nothing
 };
 
 // per-row epilogue: objective / gradient (step 3) or plain store
@@ -153,6 +154,7 @@ __global__ void __launch_bounds__(kSpmvRingThreads, 1) k_spmv_ring(SpmvParams p)
   __shared__ StructEntry stab_s[MODE == kSpmvObjective ? 256 : 1];
 
   float *out = p.out;
+  if (p.skip && *p.skip) return;
   if (MODE == kSpmvColumn) {
     if (!p.st->cand_valid) return;                       // nothing to add (converged or pool full)
     out += (size_t)p.st->K * (size_t)p.n_vox_pad;
@@ -241,6 +243,7 @@ __global__ void __launch_bounds__(kSpmvThreads, 2) k_spmv_sell(SpmvParams p) {
   __shared__ StructEntry stab_s[MODE == kSpmvObjective ? 256 : 1];
 
   float *out = p.out;
+  if (p.skip && *p.skip) return;
   if (MODE == kSpmvColumn) {
     if (!p.st->cand_valid) return;
     out += (size_t)p.st->K * (size_t)p.n_vox_pad;
@@ -289,7 +292,7 @@ __global__ void __launch_bounds__(kSpmvThreads, 2) k_spmv_sell(SpmvParams p) {
 }
 
 template <int MODE>
-static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out) {
+static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out, const int32_t *skip) {
   SpmvParams p{};
   p.col = c->d.sell_col;
   p.val = c->d.sell_val;
@@ -306,6 +309,7 @@ static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out) {
   p.perm = c->d.perm;
   p.f_part = c->d.f_part;
   p.st = c->d.state;
+  p.skip = skip;
   if (c->spmv_ring_warps > 0) {
     const int nw = c->spmv_ring_warps;
     const size_t smem = (size_t)nw * kRingStages * kRingStageBytes + align_up((size_t)nw * kRingStages * 8, 128) +
@@ -334,12 +338,12 @@ static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out) {
   return cudaGetLastError();
 }
 
-cudaError_t launch_spmv(Ctx *c, SpmvMode mode, const float *x, float *out) {
+cudaError_t launch_spmv(Ctx *c, SpmvMode mode, const float *x, float *out, const int32_t *skip) {
   switch (mode) {
-    case kSpmvObjective: return launch_spmv_mode<kSpmvObjective>(c, x, out);
-    case kSpmvPlain: return launch_spmv_mode<kSpmvPlain>(c, x, out);
-    case kSpmvColumn: return launch_spmv_mode<kSpmvColumn>(c, x, out);
-    default: return launch_spmv_mode<kSpmvPlainUserOrder>(c, x, out);
+    case kSpmvObjective: return launch_spmv_mode<kSpmvObjective>(c, x, out, skip);
+    case kSpmvPlain: return launch_spmv_mode<kSpmvPlain>(c, x, out, skip);
+    case kSpmvColumn: return launch_spmv_mode<kSpmvColumn>(c, x, out, skip);
+    default: return launch_spmv_mode<kSpmvPlainUserOrder>(c, x, out, skip);
   }
 }
 

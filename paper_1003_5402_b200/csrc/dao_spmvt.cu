@@ -20,8 +20,10 @@ __global__ void __launch_bounds__(kTThreads) k_spmvt(const int32_t *__restrict__
                                                      const int32_t *__restrict__ first_row,
                                                      const int32_t *__restrict__ seg_base,
                                                      const float *__restrict__ g, double *__restrict__ segsum,
-                                                     uint32_t *__restrict__ ticket) {
+                                                     uint32_t *__restrict__ ticket,
+                                                     const int32_t *__restrict__ skip) {
   const int lane = threadIdx.x & 31;
+  if (skip && *skip) return;
   constexpr int kRound = 512;                       // entries per warp round: 4 x (int4 + float4) per lane
   for (;;) {
     int c = 0;
@@ -86,8 +88,9 @@ __global__ void __launch_bounds__(kTThreads) k_spmvt(const int32_t *__restrict__
 __global__ void k_spmvt_finish(int32_t n_bl, const int32_t *__restrict__ t_ptr,
                                const int32_t *__restrict__ first_row, const int32_t *__restrict__ seg_base,
                                const double *__restrict__ segsum, float *__restrict__ w,
-                               uint32_t *__restrict__ ticket) {
+                               uint32_t *__restrict__ ticket, const int32_t *__restrict__ skip) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (skip && *skip) return;
   if (i == 0) *ticket = 0u;                         // re-arm the span counter for the next launch
   if (i >= n_bl) return;
   const int64_t lo = t_ptr[i], hi = t_ptr[i + 1];
@@ -99,21 +102,21 @@ __global__ void k_spmvt_finish(int32_t n_bl, const int32_t *__restrict__ t_ptr,
   w[i] = (float)s;
 }
 
-cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out) {
+cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out, const int32_t *skip) {
   if (c->n_tchunks > 0) {
     int grid = c->n_sm * kTCtasPerSm;
     const int need = (c->n_tchunks + kTThreads / 32 - 1) / (kTThreads / 32);
     if (grid > need) grid = need;
     k_spmvt<<<grid, kTThreads, 0, c->stream>>>(c->d.t_ptr, c->d.t_row, c->d.t_val, c->nnz, c->n_tchunks,
                                                c->d.t_first_row, c->d.t_seg_base, g, c->d.t_segsum,
-                                               &c->d.state->ticket_misc);
+                                               &c->d.state->ticket_misc, skip);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }
   const int t = 128;
   k_spmvt_finish<<<(c->n_bl + t - 1) / t, t, 0, c->stream>>>(c->n_bl, c->d.t_ptr, c->d.t_first_row,
                                                              c->d.t_seg_base, c->d.t_segsum, w_out,
-                                                             &c->d.state->ticket_misc);
+                                                             &c->d.state->ticket_misc, skip);
   return cudaGetLastError();
 }
 

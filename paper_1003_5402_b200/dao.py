@@ -28,7 +28,7 @@ MAX_APERTURES = 128
 EXPORTS = ["dao_default_options", "dao_workspace_bytes", "dao_create", "dao_price", "dao_solve_master",
            "dao_run", "dao_get_plan", "dao_reset", "dao_destroy", "dao_last_error", "dao_get_vector",
            "dao_get_dims", "dao_spmv", "dao_spmv_t", "dao_eval_x", "dao_price_from_w", "dao_set_pool",
-           "dao_resolve_master"]
+           "dao_resolve_master", "dao_fmo_solve"]
 
 
 class DaoError(RuntimeError):
@@ -87,6 +87,12 @@ class CIterRecord(C.Structure):
     _fields_ = [("k", C.c_int32), ("beam", C.c_int32), ("n_pg_iter", C.c_int32), ("duplicate", C.c_int32),
                 ("price", C.c_double), ("objective_before", C.c_double), ("objective", C.c_double),
                 ("kkt_residual", C.c_double)]
+
+
+class CFmoInfo(C.Structure):
+    _fields_ = [("n_iter", C.c_int32), ("converged", C.c_int32), ("hit_max_iter", C.c_int32), ("n_restarts", C.c_int32),
+                ("n_ls_evals", C.c_int32), ("reserved", C.c_int32), ("objective", C.c_double),
+                ("kkt_residual", C.c_double), ("pg_norm", C.c_double), ("seconds", C.c_double)]
 
 
 class CPlan(C.Structure):
@@ -274,6 +280,13 @@ class Dao:
     def run(self, max_apertures: int) -> CRunInfo:
         info = CRunInfo()
         self._check(self.lib.dao_run(self._ctx, C.c_int32(max_apertures), C.byref(info)))
+        return info
+
+    def fmo_solve(self, max_iter: int = 2000, tol: float = 0.0, warm_start: bool = False) -> CFmoInfo:
+        """FMO workload: min_{x >= 0} F(D x) by projected gradient on the device."""
+        info = CFmoInfo()
+        self._check(self.lib.dao_fmo_solve(self._ctx, C.c_int32(max_iter), C.c_double(tol),
+                                           C.c_int32(1 if warm_start else 0), C.byref(info)))
         return info
 
     def get_plan(self) -> Plan:

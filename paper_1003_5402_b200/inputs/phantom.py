@@ -419,7 +419,8 @@ CONFIGS = {
     "cfg0": spec_tiny,
     "cfg1": lambda: spec_prostate(2.0),
     "cfg1_literal": lambda: spec_prostate(1.0),
-    "cfg2": lambda: spec_headneck(1.0),
+    "cfg2": lambda: spec_headneck(1.8),          # fields of about 40x30 beamlets, as configs[2] states
+    "cfg2_literal": lambda: spec_headneck(1.0),
     "cfg4": lambda: spec_stress(2.2),
     "cfg4_literal": lambda: spec_stress(1.0),
     "mini": spec_mini,

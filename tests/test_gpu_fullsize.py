@@ -147,3 +147,49 @@ def test_cfg1_plan_50_apertures(D, cfg1):
     assert (np.diff(f) <= 1e-9 * f[:-1]).all() and (hist["price"] < 0).all() and (plan.intensity >= 0).all()
     print(f"cfg1: F_gpu={info.objective:.12g} F_oracle={gold['objective']:.12g} rel={rel:.2e} same beams {n_same}/50 "
           f"pg iterations {info.n_pg_iter_total} kkt gap {gap:.2e}")
+
+
+@pytest.mark.parametrize("config,n_ap", [("cfg2", 50), ("cfg4", 100)])
+def test_other_full_size_configs(D, config, n_ap):
+    """BASELINE.json configs[2] (5-field head-and-neck shape, 50 apertures) and configs[4] (7-field stress
+    case at 2 mm voxels, 100 apertures) at full size: kernels element by element, then the free-running
+    plan checked by the oracle at the GPU's plan (dose, objective, master optimality).  Prints the
+    per-kernel-class time split configs[4] asks for."""
+    ph = phantom.make(config, seed=0)
+    rng = np.random.default_rng(5)
+    x = (0.05 * rng.random(ph.n_bl)).astype(np.float32)
+    gin = rng.standard_normal(ph.n_vox).astype(np.float32)
+    with D.Dao(ph, k_max=n_ap) as d:
+        z = d.spmv(_dev(x)).cpu().numpy()
+        w = d.spmv_t(_dev(gin)).cpu().numpy()
+        zo = orc.dose(ph.row_ptr, ph.col_idx, ph.val, x.astype(np.float64))
+        wo = orc.beamlet_gradient(ph.row_ptr, ph.col_idx, ph.val, gin.astype(np.float64), ph.n_bl)
+        assert np.abs(z - zo).max() <= REL_DOSE * ph.prescription
+        assert np.abs(w - wo).max() <= REL_DOSE * np.abs(wo).max()
+        del zo, wo
+        d.run(n_ap); d.reset()                       # warm-up plan
+        info = d.run(n_ap)
+        plan = d.get_plan()
+        hist = d.get_vector(D.VEC_HISTORY)[:info.n_apertures]
+        z = d.get_vector(D.VEC_Z)
+        y = d.get_vector(D.VEC_Y)[:info.n_apertures]
+    assert info.n_apertures == n_ap
+    lefts, rights = _leaves(plan)
+    vp, _, z_o, g_o, w_o, F_o = pu.oracle_state_from_plan(ph, plan.beams, lefts, rights, y)
+    assert np.abs(z - z_o).max() <= REL_DOSE * ph.prescription
+    assert abs(info.objective - F_o) <= 1e-6 * F_o
+    grad = np.zeros(n_ap)
+    for k, b in enumerate(plan.beams):
+        m = orc.aperture_open_mask(ph.n_bl, int(b), lefts[k], rights[k], ph.beam_row_ptr, ph.row_bl_ptr)
+        grad[k] = w_o[m.astype(bool)].sum()
+    gap = float(grad @ y) + max(0.0, -grad.min()) * 2.0 * y.sum()
+    assert gap <= REL_OBJ * F_o, (gap, F_o)
+    f = np.r_[hist["objective_before"][:1], hist["objective"]]
+    assert (np.diff(f) <= 1e-9 * f[:-1]).all() and (hist["price"] < 0).all() and (plan.intensity >= 0).all()
+    n_it = max(1, info.n_iterations)
+    split = {k: getattr(info, "seconds_" + k) for k in ("intensity", "spmv", "spmv_t", "price", "column", "master")}
+    tot = sum(split.values())
+    print(f"{config}: {ph.name} V={ph.n_vox} N={ph.n_bl} nnz={ph.nnz} rows={ph.n_rows}; {n_ap} apertures in "
+          f"{info.seconds_total:.4f} s, F={info.objective:.8g}, pg iterations {info.n_pg_iter_total}, kkt gap {gap:.1e}; "
+          "per-iteration split: " + ", ".join(f"{k} {1e6 * v / n_it:.1f} us ({v / tot:.1%})" for k, v in split.items())
+          + f"; SpMV {8e-9 * ph.nnz / (split['spmv'] / n_it):.0f} GB/s, SpMV^T {8e-9 * ph.nnz / (split['spmv_t'] / n_it):.0f} GB/s (8 nnz bytes)")
