@@ -257,14 +257,33 @@ def main():
                               "GBps": master_bytes_plan * args.steps / tot["master"] * 1e-9 if tot["master"] > 0 else None,
                               "note": "dense block A (4*V*K bytes <= L2) is L2-resident: GB/s is not an HBM figure"})
     plan_bytes = N_APERTURES * (ab["spmv"] + ab["spmv_t"] + ab["price"] + ab["column"]) + master_bytes_plan
-    spmv = kernels["spmv"]
-    roofline = {"kernel": "k_spmv_ring<0> (dose SpMV + fused objective/gradient)", "bound": "hbm",
-                "achieved": spmv.get("GBps"), "peak": peak, "unit": "GB/s", "frac": spmv.get("frac_of_hbm_peak"),
-                "traffic": None, "peak_source": peak_src, "alg_bytes_per_launch": ab["spmv"],
-                "avg_launch_us": spmv["avg_us"], "share_of_step": spmv["share"],
-                "dominant_by_time": max(kernels, key=lambda k: kernels[k]["share"] or 0),
-                "sell_padding": dims.sell_elems / max(1, ph.nnz)}
-    roofline["traffic"] = ncu_traffic("k_spmv_ring<0>")
+    # `roofline` describes the kernel that dominates the step (k_master, ~90 % of a plan); the SpMV-class kernels the
+    # metric names are in `roofline_kernels`.  achieved = algorithmic bytes per launch / average launch duration
+    # (CUDA events on the launching stream inside dao_run); peak = measured HBM copy bandwidth.
+    n_master = max(1, n_it)
+    master_alg_per_launch = master_bytes_plan * args.steps / n_master
+    master_avg = tot["master"] / n_master
+    master_gbs = master_alg_per_launch / master_avg * 1e-9 if master_avg > 0 else None
+    roofline = {"kernel": "k_master (restricted master problem: projected gradient over the dense block A)",
+                "bound": "hbm", "achieved": master_gbs, "peak": peak, "unit": "GB/s",
+                "frac": master_gbs / peak if master_gbs else None, "traffic": ncu_traffic("k_master"),
+                "peak_source": peak_src, "alg_bytes_per_launch": master_alg_per_launch,
+                "alg_bytes_model": "per projected-gradient iteration 2 passes over A (2*4*V*K) + 3 passes over z, dz, sid (3*17*V)",
+                "avg_launch_us": 1e6 * master_avg, "share_of_step": kernels["master"]["share"],
+                "note": "A (4*V*K bytes, 121 MB at K = 50) stays L2-resident on this workload, so DRAM traffic is far below "
+                        "the algorithmic bytes; the fraction is of the HBM roof the same bytes would face from DRAM"}
+
+    def class_roofline(key, kernel_name, label):
+        k = kernels[key]
+        return {"kernel": label, "bound": "hbm", "achieved": k.get("GBps"), "peak": peak, "unit": "GB/s",
+                "frac": k.get("frac_of_hbm_peak"), "traffic": ncu_traffic(kernel_name), "alg_bytes_per_launch": ab[key],
+                "avg_launch_us": k["avg_us"], "share_of_step": k["share"]}
+
+    roofline_kernels = {
+        "spmv": class_roofline("spmv", "k_spmv_ring<0>", "k_spmv_ring<0> (dose SpMV + fused objective/gradient)"),
+        "spmv_t": class_roofline("spmv_t", "k_spmvt", "k_spmvt + k_spmvt_finish (w = D^T pi)"),
+        "column": class_roofline("column", "k_spmv_ring<2>", "k_spmv_ring<2> (aperture column a_K = D 1_A)"),
+        "sell_padding": dims.sell_elems / max(1, ph.nnz)}
 
     # ---- e2e: host (pinned) buffers -> dao_create -> dao_run -> dao_get_plan, wall clock ----
     e2e = None
@@ -308,7 +327,7 @@ def main():
                "warmup": args.warmup, "ms_per_step": 1e3 * elapsed / args.steps, "higher_is_better": False,
                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "storage_dtype": "f32/int32", "data": "synthetic",
                "config": workload_config(ph, args), "clocks": clocks, "e2e": e2e,
-               "gpu_launches": int(launches_per_plan * args.steps), "roofline": roofline, "cpu_baseline": cpu,
+               "gpu_launches": int(launches_per_plan * args.steps), "roofline": roofline, "roofline_kernels": roofline_kernels, "cpu_baseline": cpu,
                "kernels": kernels,
                "plan": {"objective": last.objective, "apertures": last.n_apertures, "cg_iterations_per_s": n_it / elapsed,
                         "pg_iterations": int(last.n_pg_iter_total), "converged": int(last.converged),

@@ -84,7 +84,8 @@ __global__ void __launch_bounds__(kFmoDirThreads) k_fmo_direction(FmoState *__re
   const int iters = fs->iters;
   // w is an fp32 vector: once F stops decreasing beyond fp64 rounding for 4 iterations in a row the
   // iterate sits at the resolution of the arithmetic and counts as converged (converged = 2)
-  const bool flat = iters > 0 && fabs(fs->F_prev - F) <= 1e-13 * fabs(F);
+  // (a step that was cut at a bound does not count: it can be arbitrarily short)
+  const bool flat = iters > 0 && !fs->force_restart && fabs(fs->F_prev - F) <= 1e-13 * fabs(F);
   const int stall = flat ? fs->stall + 1 : 0;
   const bool conv = pg_max * x_max <= tol * fmax(F, 1e-300) || stall >= 4;
   const bool stop = conv || iters >= max_iter;
@@ -273,6 +274,11 @@ __global__ void k_fmo_update(FmoState *__restrict__ fs, int32_t n_bl, float *__r
     x[i] = (float)v;
   }
 }
+__global__ void k_fmo_reset(FmoState *fs, int keep_horizon) {
+  const double te = keep_horizon ? fs->t_est : 0.0;      // a warm start keeps the step scale of the last solve
+  *fs = FmoState{};
+  fs->t_est = te;
+}
 __global__ void k_fmo_advance(FmoState *fs) {
   if (fs->done) return;
   fs->iters += 1;
@@ -296,7 +302,8 @@ constexpr int kFmoCheckEvery = 8;     // iterations between two host looks at th
 dao_status fmo_solve(Ctx *c, int32_t max_iter, double tol, bool warm_start, dao_fmo_info *out) {
   FmoState *fs = c->d.fmo_state;
   const int32_t *skip = &fs->done;
-  FMO_CUDA(cudaMemsetAsync(fs, 0, sizeof(FmoState), c->stream));
+  k_fmo_reset<<<1, 1, 0, c->stream>>>(fs, warm_start ? 1 : 0);
+  FMO_CUDA(cudaGetLastError());
   FMO_CUDA(cudaMemsetAsync(c->d.fmo_p, 0, (size_t)c->n_bl * 4, c->stream));
   FMO_CUDA(cudaMemsetAsync(c->d.fmo_pgold, 0, (size_t)c->n_bl * 4, c->stream));
   if (!warm_start) FMO_CUDA(cudaMemsetAsync(c->d.x, 0, (size_t)c->n_bl * 4, c->stream));

@@ -501,25 +501,32 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
       const int tn = min(kMasterTileVox, slab_len - t0);
       const bool a0 = l0 < tn, a1 = l1 < tn;
       double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-      for (int k = 0; k < K; ++k) {
-        const double ck = coef[k];
-        mbar_wait(&sm.full[cp.stage], cp.phase);
-        if (ck != 0.0) {
-          const unsigned char *st = sm.ring + (size_t)cp.stage * kMasterStageBytes;
-          if (a0) {
-            const float4 a = *reinterpret_cast<const float4 *>(st + (size_t)l0 * 4);
-            acc[0] = fma(ck, (double)a.x, acc[0]); acc[1] = fma(ck, (double)a.y, acc[1]);
-            acc[2] = fma(ck, (double)a.z, acc[2]); acc[3] = fma(ck, (double)a.w, acc[3]);
-          }
-          if (a1) {
-            const float4 a = *reinterpret_cast<const float4 *>(st + (size_t)l1 * 4);
-            acc[4] = fma(ck, (double)a.x, acc[4]); acc[5] = fma(ck, (double)a.y, acc[5]);
-            acc[6] = fma(ck, (double)a.z, acc[6]); acc[7] = fma(ck, (double)a.w, acc[7]);
-          }
-        }
+      // two stages per step: both waits first, then all loads, then the arithmetic (more independent
+      // work per warp between two barrier round trips)
+      for (int k = 0; k < K; k += 2) {
+        const bool two = k + 1 < K;
+        const double c0 = coef[k], c1 = two ? coef[k + 1] : 0.0;
+        RingPos q0 = cp, q1 = cp;
+        q1.advance(NS);
+        mbar_wait(&sm.full[q0.stage], q0.phase);
+        if (two) mbar_wait(&sm.full[q1.stage], q1.phase);
+        const unsigned char *s0 = sm.ring + (size_t)q0.stage * kMasterStageBytes;
+        const unsigned char *s1 = sm.ring + (size_t)q1.stage * kMasterStageBytes;
+        float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0, y0 = x0, y1 = x0;
+        if (a0) { x0 = *reinterpret_cast<const float4 *>(s0 + (size_t)l0 * 4); if (two) y0 = *reinterpret_cast<const float4 *>(s1 + (size_t)l0 * 4); }
+        if (a1) { x1 = *reinterpret_cast<const float4 *>(s0 + (size_t)l1 * 4); if (two) y1 = *reinterpret_cast<const float4 *>(s1 + (size_t)l1 * 4); }
+        acc[0] = fma(c0, (double)x0.x, acc[0]); acc[1] = fma(c0, (double)x0.y, acc[1]);
+        acc[2] = fma(c0, (double)x0.z, acc[2]); acc[3] = fma(c0, (double)x0.w, acc[3]);
+        acc[4] = fma(c0, (double)x1.x, acc[4]); acc[5] = fma(c0, (double)x1.y, acc[5]);
+        acc[6] = fma(c0, (double)x1.z, acc[6]); acc[7] = fma(c0, (double)x1.w, acc[7]);
+        acc[0] = fma(c1, (double)y0.x, acc[0]); acc[1] = fma(c1, (double)y0.y, acc[1]);
+        acc[2] = fma(c1, (double)y0.z, acc[2]); acc[3] = fma(c1, (double)y0.w, acc[3]);
+        acc[4] = fma(c1, (double)y1.x, acc[4]); acc[5] = fma(c1, (double)y1.y, acc[5]);
+        acc[6] = fma(c1, (double)y1.z, acc[6]); acc[7] = fma(c1, (double)y1.w, acc[7]);
         __syncwarp();
-        if (lane == 0) mbar_arrive(&sm.empty[cp.stage]);
+        if (lane == 0) { mbar_arrive(&sm.empty[q0.stage]); if (two) mbar_arrive(&sm.empty[q1.stage]); }
         cp.advance(NS);
+        if (two) cp.advance(NS);
       }
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
@@ -612,26 +619,38 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
       for (int kb8 = 0; kb8 < K; kb8 += 8) {
         double d[8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
+        for (int j = 0; j < 8; j += 2) {
           d[j] = 0.0;
-          if (kb8 + j < K) {
-            mbar_wait(&sm.full[cp.stage], cp.phase);
-            const unsigned char *st = sm.ring + (size_t)cp.stage * kMasterStageBytes;
-            if (a0) {
-              const float4 a = *reinterpret_cast<const float4 *>(st + (size_t)l0 * 4);
-              double q = (double)a.x * g[0];
-              q = fma((double)a.y, g[1], q); q = fma((double)a.z, g[2], q); q = fma((double)a.w, g[3], q);
-              d[j] = q;
+          d[j + 1] = 0.0;
+          if (kb8 + j < K) {                       // two stages per step: waits, then loads, then arithmetic
+            const bool two = kb8 + j + 1 < K;
+            RingPos q0 = cp, q1 = cp;
+            q1.advance(NS);
+            mbar_wait(&sm.full[q0.stage], q0.phase);
+            if (two) mbar_wait(&sm.full[q1.stage], q1.phase);
+            const unsigned char *s0 = sm.ring + (size_t)q0.stage * kMasterStageBytes;
+            const unsigned char *s1 = sm.ring + (size_t)q1.stage * kMasterStageBytes;
+            float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0, y0 = x0, y1 = x0;
+            if (a0) { x0 = *reinterpret_cast<const float4 *>(s0 + (size_t)l0 * 4); if (two) y0 = *reinterpret_cast<const float4 *>(s1 + (size_t)l0 * 4); }
+            if (a1) { x1 = *reinterpret_cast<const float4 *>(s0 + (size_t)l1 * 4); if (two) y1 = *reinterpret_cast<const float4 *>(s1 + (size_t)l1 * 4); }
+            {
+              double q = (double)x0.x * g[0];
+              q = fma((double)x0.y, g[1], q); q = fma((double)x0.z, g[2], q); q = fma((double)x0.w, g[3], q);
+              double r = (double)x1.x * g[4];
+              r = fma((double)x1.y, g[5], r); r = fma((double)x1.z, g[6], r); r = fma((double)x1.w, g[7], r);
+              d[j] = a0 ? (a1 ? q + r : q) : (a1 ? 0.0 + r : 0.0);
             }
-            if (a1) {
-              const float4 a = *reinterpret_cast<const float4 *>(st + (size_t)l1 * 4);
-              double q = (double)a.x * g[4];
-              q = fma((double)a.y, g[5], q); q = fma((double)a.z, g[6], q); q = fma((double)a.w, g[7], q);
-              d[j] += q;
+            {
+              double q = (double)y0.x * g[0];
+              q = fma((double)y0.y, g[1], q); q = fma((double)y0.z, g[2], q); q = fma((double)y0.w, g[3], q);
+              double r = (double)y1.x * g[4];
+              r = fma((double)y1.y, g[5], r); r = fma((double)y1.z, g[6], r); r = fma((double)y1.w, g[7], r);
+              d[j + 1] = a0 ? (a1 ? q + r : q) : (a1 ? 0.0 + r : 0.0);
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(&sm.empty[cp.stage]);
+            if (lane == 0) { mbar_arrive(&sm.empty[q0.stage]); if (two) mbar_arrive(&sm.empty[q1.stage]); }
             cp.advance(NS);
+            if (two) cp.advance(NS);
           }
         }
         const double r = butterfly8(d, lane);

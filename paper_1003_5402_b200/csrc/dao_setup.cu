@@ -707,6 +707,7 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   // ---- zero the state ----
   const size_t vp = (size_t)L.n_vox_pad;
   SETUP_CUDA(cudaMemsetAsync(d.state, 0, sizeof(DevState), q));
+  SETUP_CUDA(cudaMemsetAsync(d.fmo_state, 0, sizeof(FmoState), q));
   SETUP_CUDA(cudaMemsetAsync(d.x, 0, (size_t)dm.n_bl * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.xmask, 0, (size_t)dm.n_bl * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.z, 0, vp * 4, q));
