@@ -175,6 +175,82 @@ def pinned_phantom(ph, torch):
     return q
 
 
+SWEEP_MATRICES = ["sweep_1m", "sweep_3m", "cfg1_literal", "cfg4_literal", "cfg2", "cfg1", "sweep_100m", "cfg4", "sweep_200m"]
+
+
+def run_sweep(args):
+    """BASELINE.json configs[3]: isolated SpMV / SpMV^T on pencil-beam matrices of 1M-200M non-zeros and the
+    pricing kernels on 1k-100k leaf rows, GB/s against the measured HBM peak, each checked against the oracle
+    (full vectors).  Prints a markdown table; every timing is per launch with CUDA events on the launching
+    stream, cold = a 512 MB buffer is rewritten between launches (L2 flushed), warm = back to back."""
+    import torch
+    from oracle import dao_oracle as orc
+    from paper_1003_5402_b200 import build, dao
+    from paper_1003_5402_b200.inputs import phantom
+    build.build()
+    orc.build()
+    peak, peak_src = load_peaks()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+
+    def timed(fn, reps, cold):
+        ts = []
+        for _ in range(3):
+            fn()
+        for _ in range(reps):
+            if cold:
+                flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e-3)
+        return float(np.median(ts))
+
+    print(f"HBM peak {peak:.0f} GB/s, {peak_src}; bytes = SURVEY 8(d) algorithmic bytes; median of {args.sweep_reps} launches\n")
+    print("| matrix | V | N | V:N | nnz | 8 nnz (MB) | SpMV cold us | GB/s | frac | SpMV warm GB/s | SpMV^T cold us | GB/s | frac | SpMV^T warm GB/s | max err z, w vs oracle |")
+    print("|---|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---:|---|")
+    names = args.sweep_only.split(",") if args.sweep_only else SWEEP_MATRICES
+    for name in names:
+        ph = phantom.make(name, 0)
+        rng = np.random.default_rng(1)
+        x = rng.random(ph.n_bl).astype(np.float32)
+        g = rng.standard_normal(ph.n_vox).astype(np.float32)
+        xd, gd = torch.from_numpy(x).cuda(), torch.from_numpy(g).cuda()
+        with dao.Dao(ph, k_max=1) as d:
+            zd = torch.empty(ph.n_vox, dtype=torch.float32, device="cuda")
+            wd = torch.empty(ph.n_bl, dtype=torch.float32, device="cuda")
+            res = {}
+            for cold in (True, False):
+                res["spmv", cold] = timed(lambda: d.spmv(xd, zd), args.sweep_reps, cold)
+                res["spmvt", cold] = timed(lambda: d.spmv_t(gd, wd), args.sweep_reps, cold)
+            z, w = zd.cpu().numpy(), wd.cpu().numpy()
+        zo = orc.dose(ph.row_ptr, ph.col_idx, ph.val, x.astype(np.float64))
+        wo = orc.beamlet_gradient(ph.row_ptr, ph.col_idx, ph.val, g.astype(np.float64), ph.n_bl)
+        ez, ew = np.abs(z - zo).max() / np.abs(zo).max(), np.abs(w - wo).max() / np.abs(wo).max()
+        b_spmv = 8 * ph.nnz + 4 * (ph.n_vox + 1) + 4 * ph.n_bl + 4 * ph.n_vox
+        b_t = 8 * ph.nnz + 4 * (ph.n_bl + 1) + 4 * ph.n_vox + 4 * ph.n_bl
+        c1, w1, c2, w2 = res["spmv", True], res["spmv", False], res["spmvt", True], res["spmvt", False]
+        print(f"| {name} ({ph.name}) | {ph.n_vox} | {ph.n_bl} | {ph.n_vox / ph.n_bl:.0f} | {ph.nnz} | {8e-6 * ph.nnz:.0f} | "
+              f"{1e6 * c1:.1f} | {1e-9 * b_spmv / c1:.0f} | {1e-9 * b_spmv / c1 / peak:.2f} | {1e-9 * b_spmv / w1:.0f} | "
+              f"{1e6 * c2:.1f} | {1e-9 * b_t / c2:.0f} | {1e-9 * b_t / c2 / peak:.2f} | {1e-9 * b_t / w2:.0f} | {ez:.1e}, {ew:.1e} |", flush=True)
+        del ph, zo, wo
+    print("\n| leaf rows R | beamlets per row | N | pricing cold us | GB/s (4N + 4(R+1) + 20R bytes) | frac | warm us | rows bit-exact vs oracle | best beam |")
+    print("|---:|---:|---:|---:|---:|---:|---:|---|---|")
+    ph = phantom.make("cfg1_literal", 0)
+    with dao.Dao(ph, k_max=1) as d:
+        for n_rows in (1000, 10000, 100000):
+            for row_len in (20, 40, 80):
+                w, brp, rbp = phantom.pricing_rows(n_rows, row_len, rows_per_beam=40, seed=n_rows % 3)
+                wd, rd, bd = (torch.from_numpy(a).cuda() for a in (w, rbp, brp))
+                tc = timed(lambda: d.price_from_w(wd, rd, bd), args.sweep_reps, True)
+                tw = timed(lambda: d.price_from_w(wd, rd, bd), args.sweep_reps, False)
+                le, ri, vs, bp, best = (t.cpu().numpy() for t in d.price_from_w(wd, rd, bd))
+                pr = orc.price(w.astype(np.float64), brp, rbp)
+                same = int(((le == pr.left) & (ri == pr.right)).sum())
+                nbytes = 4 * w.size + 4 * (n_rows + 1) + 20 * n_rows
+                print(f"| {n_rows} | {row_len} | {w.size} | {1e6 * tc:.1f} | {1e-9 * nbytes / tc:.0f} | {1e-9 * nbytes / tc / peak:.3f} | "
+                      f"{1e6 * tw:.1f} | {same}/{n_rows} | {'same' if int(best[0]) == pr.best_beam else 'differs'} |", flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -185,12 +261,19 @@ def main():
     ap.add_argument("--ref-apertures", type=int, default=3, help="apertures per step of the reference arm / cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[3] kernel sweep (markdown table)")
+    ap.add_argument("--sweep-reps", type=int, default=15)
+    ap.add_argument("--sweep-only", default="", help="comma-separated subset of the sweep matrices")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+        return
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args)
         return
     args.warmup = max(args.warmup, 3)
 

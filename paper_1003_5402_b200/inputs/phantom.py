@@ -424,6 +424,11 @@ CONFIGS = {
     "cfg4": lambda: spec_stress(2.2),
     "cfg4_literal": lambda: spec_stress(1.0),
     "mini": spec_mini,
+    # BASELINE.json configs[3] (kernel sweep): pencil-beam matrices from ~1M to ~200M non-zeros
+    "sweep_1m": lambda: spec_prostate(1.0, n_beams=5, voxel_mm=4.0, grid=(126, 126, 76), name="sweep_1m"),
+    "sweep_3m": lambda: spec_prostate(1.0, n_beams=9, voxel_mm=4.0, grid=(126, 126, 76), name="sweep_3m"),
+    "sweep_100m": lambda: spec_stress(1.7),
+    "sweep_200m": lambda: spec_stress(2.4),
 }
 
 
