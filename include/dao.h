@@ -115,7 +115,8 @@ typedef struct {
                                 caller's voxel order; 0 = library default */
   int32_t timers;            /* non-zero: CUDA-event timers per kernel class in dao_run (default 1) */
   int32_t reserved;          /* test/bench hooks, 0 in production: bit 0 forces the direct-load SpMV variant,
-                                bit 1 turns on the master's phase timers (DAO_VEC_MASTER_PHASES) */
+                                bit 1 turns on the master's phase timers (DAO_VEC_MASTER_PHASES), bit 2 forces the span variant
+                                of the transposed SpMV even for short beamlet rows */
 } dao_options;
 
 typedef struct {
