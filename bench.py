@@ -28,7 +28,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "50-aperture DAO plan time"
-N_APERTURES = 50
+N_APERTURES = 50          # BASELINE.json configs[1]; --apertures overrides it for the other configs (configs[4]: 100)
 
 
 def load_peaks():
@@ -252,12 +252,14 @@ def run_sweep(args):
 
 
 def main():
+    global N_APERTURES, METRIC
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="cfg1")
     ap.add_argument("--impl", default="dao", choices=["dao", "reference"])
+    ap.add_argument("--apertures", type=int, default=N_APERTURES, help="apertures per plan (50; configs[4] asks for 100)")
     ap.add_argument("--ref-apertures", type=int, default=3, help="apertures per step of the reference arm / cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -265,6 +267,8 @@ def main():
     ap.add_argument("--sweep-reps", type=int, default=15)
     ap.add_argument("--sweep-only", default="", help="comma-separated subset of the sweep matrices")
     args = ap.parse_args()
+    N_APERTURES = args.apertures
+    METRIC = f"{N_APERTURES}-aperture DAO plan time"
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -359,7 +363,8 @@ def main():
     def class_roofline(key, kernel_name, label):
         k = kernels[key]
         return {"kernel": label, "bound": "hbm", "achieved": k.get("GBps"), "peak": peak, "unit": "GB/s",
-                "frac": k.get("frac_of_hbm_peak"), "traffic": ncu_traffic(kernel_name), "alg_bytes_per_launch": ab[key],
+                "frac": k.get("frac_of_hbm_peak"), "frac_of_nominal_8000": (k.get("GBps") or 0.0) / 8000.0,
+                "traffic": ncu_traffic(kernel_name), "alg_bytes_per_launch": ab[key],
                 "avg_launch_us": k["avg_us"], "share_of_step": k["share"]}
 
     roofline_kernels = {

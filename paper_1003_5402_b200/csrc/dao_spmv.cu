@@ -164,11 +164,7 @@ __global__ void __launch_bounds__(kSpmvRingThreads, 1) k_spmv_ring(SpmvParams p)
     for (int s = 0; s < kRingStages; ++s) mbar_init(&bars[warp * kRingStages + s], 1);
   }
   fence_mbar_init();
-  for (int i = threadIdx.x; i < p.n_bl; i += blockDim.x) xs[i] = p.x[i];
-  if (MODE == kSpmvObjective) {
-    for (int i = threadIdx.x; i < 256; i += blockDim.x) stab_s[i] = p.stab[i];
-  }
-  __syncthreads();
+  __syncwarp();                 // the ring is warp-private: its first copies go out before x is staged
 
   const int stride = gridDim.x * nw;
   const int first = blockIdx.x * nw + warp;
@@ -207,6 +203,13 @@ __global__ void __launch_bounds__(kSpmvRingThreads, 1) k_spmv_ring(SpmvParams p)
   };
 #pragma unroll
   for (int s = 0; s < kRingStages; ++s) issue();
+
+  // x and the penalty table are staged while the first chunks are in flight
+  for (int i = threadIdx.x; i < p.n_bl; i += blockDim.x) xs[i] = p.x[i];
+  if (MODE == kSpmvObjective) {
+    for (int i = threadIdx.x; i < 256; i += blockDim.x) stab_s[i] = p.stab[i];
+  }
+  __syncthreads();
 
   double f_acc = 0.0;
   for (int slice = first; slice < p.n_slices; slice += stride) {
