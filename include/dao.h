@@ -194,7 +194,8 @@ typedef enum {               /* dao_get_vector selectors; lengths in elements */
                                 dao_options.reserved has bit 1 (value 2) set, else zeros.  Nanoseconds of CTA 0 in:
                                 0 set-up and z = A y, 1 gradient pass over A, 2 gradient reduction, 3 direction,
                                 4 dz = A p pass, 5 curvature reduction, 6 line search, 10 publish; counts:
-                                7 line-search evaluations, 8 projected-gradient iterations, 9 calls */
+                                7 line-search evaluations, 8 projected-gradient iterations, 9 calls; SM clock cycles thread 0 of
+                                CTA 0 spent waiting for stages of A: 12 in gradient passes, 13 in dz passes */
 } dao_vector;
 
 void dao_default_options(dao_options *opt);

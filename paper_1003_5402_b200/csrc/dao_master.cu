@@ -502,14 +502,16 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
       const bool a0 = l0 < tn, a1 = l1 < tn;
       double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
       // two stages per step: both waits first, then all loads, then the arithmetic (more independent
-      // work per warp between two barrier round trips)
+      // work per warp between two barrier round trips; four stages per step measured slower: registers)
       for (int k = 0; k < K; k += 2) {
         const bool two = k + 1 < K;
         const double c0 = coef[k], c1 = two ? coef[k + 1] : 0.0;
         RingPos q0 = cp, q1 = cp;
         q1.advance(NS);
+        const long long tw = prof ? clock64() : 0ll;
         mbar_wait(&sm.full[q0.stage], q0.phase);
         if (two) mbar_wait(&sm.full[q1.stage], q1.phase);
+        if (prof) prof_s[13] += (unsigned long long)(clock64() - tw);                 // time this thread waited for A in D passes
         const unsigned char *s0 = sm.ring + (size_t)q0.stage * kMasterStageBytes;
         const unsigned char *s1 = sm.ring + (size_t)q1.stage * kMasterStageBytes;
         float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0, y0 = x0, y1 = x0;
@@ -626,8 +628,10 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
             const bool two = kb8 + j + 1 < K;
             RingPos q0 = cp, q1 = cp;
             q1.advance(NS);
+            const long long tw = prof ? clock64() : 0ll;
             mbar_wait(&sm.full[q0.stage], q0.phase);
             if (two) mbar_wait(&sm.full[q1.stage], q1.phase);
+            if (prof) prof_s[12] += (unsigned long long)(clock64() - tw);             // time this thread waited for A in G passes
             const unsigned char *s0 = sm.ring + (size_t)q0.stage * kMasterStageBytes;
             const unsigned char *s1 = sm.ring + (size_t)q1.stage * kMasterStageBytes;
             float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0, y0 = x0, y1 = x0;
