@@ -487,3 +487,61 @@ int32_t orc_fmo_pg(int32_t n_vox, int32_t n_bl, const int32_t *row_ptr, const in
     free(z); free(g); free(dz); free(w); free(p);
     return it;
 }
+
+/* ------------------------------------------------------------------ jaws-only pricing
+ * "we are able to handle various MLC hardware constraints ... including standard consecutiveness,
+ * interdigitation, connectedness and jaws-only delivery": the paper names the constraint and
+ * prints no algorithm.  Reading J1: with jaws only, an aperture of beam b is a RECTANGLE --
+ * consecutive leaf rows m1..m2 all opened over the same lateral range [c1, c2), measured in beamlet widths from
+ * the beam's leftmost beamlet (row r starts at row_col0[r]), every other row closed; a cell of the rectangle
+ * where a row has no beamlet contributes nothing.  The sub-problem (8) becomes: over all rectangles of all
+ * beams, minimise the sum of w over the rectangle's beamlets.  Plain definition written out: every rectangle
+ * is enumerated in the order c1, c2, m1, m2 (ascending) and replaces the incumbent only when strictly smaller,
+ * so the closed aperture (value 0) wins ties at 0 and equal negative values keep the first in that order.
+ * Outputs as orc_price: per row the half-open leaves inside the row (closed = (0,0)) and vstar[r] = sum of w
+ * over the row's open beamlets; beam_price[b] = value of the best rectangle of beam b. */
+void orc_price_jaws(const double *w, int32_t n_beams, const int32_t *beam_row_ptr, const int32_t *row_bl_ptr,
+                    const int32_t *row_col0, double *vstar, int32_t *left, int32_t *right, double *beam_price,
+                    int32_t *best_beam)
+{
+    int32_t bb = -1; double bbv = 0.0;
+    for (int32_t b = 0; b < n_beams; ++b) {
+        const int32_t r0 = beam_row_ptr[b], r1 = beam_row_ptr[b + 1], R = r1 - r0;
+        int32_t C = 0;
+        for (int32_t r = r0; r < r1; ++r) {
+            const int32_t c0 = row_col0 ? row_col0[r] : 0, e = c0 + (row_bl_ptr[r + 1] - row_bl_ptr[r]);
+            if (e > C) C = e;
+        }
+        double best = 0.0; int32_t bc1 = 0, bc2 = 0, bm1 = 0, bm2 = -1;          /* closed */
+        double *S = (double *)malloc(sizeof(double) * (size_t)(R > 0 ? R : 1));
+        for (int32_t c1 = 0; c1 < C; ++c1)
+            for (int32_t c2 = c1 + 1; c2 <= C; ++c2) {
+                for (int32_t m = 0; m < R; ++m) {                                /* row sums over [c1, c2) */
+                    const int32_t r = r0 + m, c0 = row_col0 ? row_col0[r] : 0, n = row_bl_ptr[r + 1] - row_bl_ptr[r];
+                    const int32_t lo = c1 > c0 ? c1 : c0, hi = c2 < c0 + n ? c2 : c0 + n;
+                    double s = 0.0;
+                    for (int32_t c = lo; c < hi; ++c) s += w[row_bl_ptr[r] + (c - c0)];
+                    S[m] = s;
+                }
+                for (int32_t m1 = 0; m1 < R; ++m1) {
+                    double s = 0.0;
+                    for (int32_t m2 = m1; m2 < R; ++m2) {
+                        s += S[m2];
+                        if (s < best) { best = s; bc1 = c1; bc2 = c2; bm1 = m1; bm2 = m2; }
+                    }
+                }
+            }
+        free(S);
+        beam_price[b] = best;
+        for (int32_t m = 0; m < R; ++m) {
+            const int32_t r = r0 + m, c0 = row_col0 ? row_col0[r] : 0, n = row_bl_ptr[r + 1] - row_bl_ptr[r];
+            int32_t lo = bc1 > c0 ? bc1 : c0, hi = bc2 < c0 + n ? bc2 : c0 + n;
+            double s = 0.0;
+            if (m < bm1 || m > bm2 || hi <= lo) { lo = c0; hi = c0; }
+            for (int32_t c = lo; c < hi; ++c) s += w[row_bl_ptr[r] + (c - c0)];
+            left[r] = hi > lo ? lo - c0 : 0; right[r] = hi > lo ? hi - c0 : 0; vstar[r] = s;
+        }
+        if (bb < 0 || best < bbv) { bb = b; bbv = best; }
+    }
+    *best_beam = bb;
+}

@@ -168,6 +168,21 @@ def price(w, beam_row_ptr, row_bl_ptr) -> Pricing:
     return Pricing(vs, le, ri, bp, bb.value)
 
 
+def price_jaws(w, beam_row_ptr, row_bl_ptr, row_col0=None) -> Pricing:
+    """Jaws-only sub-problem (reading J1): the best RECTANGLE per beam (consecutive rows, one
+    common lateral range), all rectangles enumerated.  row_col0[r] = lateral position of row r's first beamlet."""
+    w, brp, rbp = _f64(w), _i32(beam_row_ptr), _i32(row_bl_ptr)
+    n_beams, n_rows = brp.size - 1, rbp.size - 1
+    rc0 = _i32(np.zeros(n_rows) if row_col0 is None else row_col0)
+    vs = np.zeros(n_rows, dtype=np.float64)
+    le = np.zeros(n_rows, dtype=np.int32)
+    ri = np.zeros(n_rows, dtype=np.int32)
+    bp = np.zeros(n_beams, dtype=np.float64)
+    bb = C.c_int32(-1)
+    lib().orc_price_jaws(_p(w), C.c_int32(n_beams), _p(brp), _p(rbp), _p(rc0), _p(vs), _p(le), _p(ri), _p(bp), C.byref(bb))
+    return Pricing(vs, le, ri, bp, bb.value)
+
+
 def aperture_open_mask(n_bl, beam, left, right, beam_row_ptr, row_bl_ptr):
     """0/1 mask over beamlets of an aperture in `beam` with per-row half-open leaves (rows of that beam)."""
     m = np.zeros(n_bl, dtype=np.uint8)
@@ -287,8 +302,9 @@ def price_converged(pr: Pricing, w, beam_row_ptr, price_tol: float) -> bool:
 
 
 def run(ph, max_apertures: int, master_tol: float = 1e-10, master_max_iter: int = 20000,
-        price_tol: float = 1e-9, method: str = "newton", keep_A: bool = False) -> Plan:
-    """O9: the column-generation loop.  `ph` is any object with the Phantom fields."""
+        price_tol: float = 1e-9, method: str = "newton", keep_A: bool = False, mlc: str = "consecutive") -> Plan:
+    """O9: the column-generation loop.  `ph` is any object with the Phantom fields.  mlc = "consecutive"
+    (the paper's experiments) or "jaws" (jaws-only delivery, reading J1)."""
     vp = voxel_params_of(ph)
     n_vox, n_bl = ph.n_vox, ph.n_bl
     A = np.zeros((max_apertures, n_vox), dtype=np.float64)
@@ -299,7 +315,10 @@ def run(ph, max_apertures: int, master_tol: float = 1e-10, master_max_iter: int 
     for it in range(max_apertures):
         g = voxel_gradient(z, vp)
         w = beamlet_gradient(ph.row_ptr, ph.col_idx, ph.val, g, n_bl)
-        pr = price(w, ph.beam_row_ptr, ph.row_bl_ptr)
+        if mlc == "jaws":
+            pr = price_jaws(w, ph.beam_row_ptr, ph.row_bl_ptr, getattr(ph, "row_col0", None))
+        else:
+            pr = price(w, ph.beam_row_ptr, ph.row_bl_ptr)
         if price_converged(pr, w, ph.beam_row_ptr, price_tol):
             plan.converged = True
             break

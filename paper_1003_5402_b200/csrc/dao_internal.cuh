@@ -23,10 +23,16 @@ constexpr int kTThreads = 256;
 constexpr int kTCtasPerSm = 6;         // persistent CTAs per SM of the transposed SpMV
 constexpr int kMasterWorkers = 512;    // worker threads of the persistent master kernel (one CTA per SM)
 constexpr int kMasterThreads = kMasterWorkers + 32;   // + the producer warp that streams A through the ring
-constexpr int kMasterTileVox = 4096;   // voxels per ring stage: 16 worker warps x 2 strips x 128
+#ifndef DAO_MASTER_CTAS_PER_SM
+#define DAO_MASTER_CTAS_PER_SM 1
+#endif
+constexpr int kMasterCtasPerSm = DAO_MASTER_CTAS_PER_SM;   // resident CTAs of the master per SM.  2 (34 warps per SM, one strip per warp) was measured on cfg1: the passes
+                                       // take the same time (L2-side limit, not warp latency) and the grid reductions over 296 CTAs double: slower
+constexpr int kMasterStrips = kMasterCtasPerSm == 1 ? 2 : 1;   // 128-voxel strips per worker warp and stage
+constexpr int kMasterTileVox = 16 * 128 * kMasterStrips;   // voxels per ring stage: 16 worker warps x strips x 128
 constexpr int kMasterStageBytes = kMasterTileVox * 4;
 constexpr int kMasterMaxStages = 10;
-constexpr int kMasterMaxGrid = 160;    // CTAs of the master kernel (one per SM, capped)
+constexpr int kMasterMaxGrid = 160 * kMasterCtasPerSm;    // CTAs of the master kernel (capped)
 constexpr int kMasterProfSlots = 16;   // phase timers of the master (ns): 0 init, 1 G pass, 2 G reduce, 3 direction,
                                        // 4 D pass, 5 D reduce, 6 line search; 7 line-search evaluations,
                                        // 8 iterations, 9 calls, 10 publish

@@ -345,7 +345,7 @@ struct MasterSmem {          // carved from dynamic shared memory by every threa
   double *warp_part;         // [kNW][kpad]
 };
 
-__global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
+__global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(MasterParams p) {
   extern __shared__ __align__(128) unsigned char dyn_smem[];
   // ---- shared state (replicated in every CTA, evolves identically everywhere) ----
   __shared__ double y_s[DAO_MAX_APERTURES];
@@ -499,7 +499,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
     for (int tile = 0; tile < n_tiles; ++tile) {
       const int t0 = tile * kMasterTileVox;
       const int tn = min(kMasterTileVox, slab_len - t0);
-      const bool a0 = l0 < tn, a1 = l1 < tn;
+      const bool a0 = l0 < tn, a1 = (kMasterStrips > 1) && l1 < tn;
       double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
       // two stages per step: both waits first, then all loads, then the arithmetic (more independent
       // work per warp between two barrier round trips; four stages per step measured slower: registers)
@@ -590,7 +590,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master(MasterParams p) {
     for (int tile = 0; tile < n_tiles; ++tile) {
       const int t0 = tile * kMasterTileVox;
       const int tn = min(kMasterTileVox, slab_len - t0);
-      const bool a0 = l0 < tn, a1 = l1 < tn;
+      const bool a0 = l0 < tn, a1 = (kMasterStrips > 1) && l1 < tn;
       double g[8];
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
@@ -850,7 +850,7 @@ static size_t master_fixed_smem(const Ctx *c, int n_stages) {
 }
 
 cudaError_t master_configure(Ctx *c) {
-  c->master_grid = std::min(c->n_sm, kMasterMaxGrid);      // one CTA per SM
+  c->master_grid = std::min(c->n_sm * kMasterCtasPerSm, kMasterMaxGrid);
   int slab = (c->n_vox_pad + c->master_grid - 1) / c->master_grid;
   slab = (slab + 127) / 128 * 128;
   c->master_slab = slab;
@@ -860,7 +860,10 @@ cudaError_t master_configure(Ctx *c) {
   int max_optin = 0;
   e = cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device);
   if (e != cudaSuccess) return e;
-  const size_t budget = (size_t)max_optin - fa.sharedSizeBytes - 1024;
+  // shared memory per CTA: the opt-in maximum for one CTA per SM; with more, an equal share of the SM's
+  // 228 KB (1 KB per resident CTA is reserved by the system)
+  size_t budget = (size_t)max_optin - fa.sharedSizeBytes - 1024;
+  if (kMasterCtasPerSm > 1) budget = (size_t)(228 * 1024) / kMasterCtasPerSm - 1024 - fa.sharedSizeBytes - 512;
   const size_t slab_bytes = (size_t)slab * (c->has_vt ? 21 : 17);
   // prefer z in shared memory with >= 4 stages; otherwise z stays in global memory (L2)
   c->master_z_in_smem = 0;
@@ -881,7 +884,7 @@ cudaError_t master_configure(Ctx *c) {
   int nb = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_master, kMasterThreads, c->master_smem);
   if (e != cudaSuccess) return e;
-  if (nb < 1) return cudaErrorLaunchOutOfResources;
+  if (nb < kMasterCtasPerSm) return cudaErrorLaunchOutOfResources;
   return cudaSuccess;
 }
 

@@ -138,7 +138,7 @@ static void carve_workspace(Carver &cv, const Dims &dm, const HostLayout &L, Dev
   d->mz = cv.take<double>(vp);
   d->mdz = cv.take<double>(vp);
   {
-    const size_t g = (size_t)std::min(n_sm, kMasterMaxGrid);
+    const size_t g = (size_t)std::min(n_sm * kMasterCtasPerSm, kMasterMaxGrid);
     d->ll_part = cv.take<uint4>(2 * g * kMaxRedux);
     d->ll_result = cv.take<uint4>(2 * kMaxRedux);
   }
@@ -717,7 +717,7 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   SETUP_CUDA(cudaMemsetAsync(d.mz, 0, vp * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.mdz, 0, vp * 8, q));
   {
-    const size_t g = (size_t)std::min(c->n_sm, kMasterMaxGrid);
+    const size_t g = (size_t)std::min(c->n_sm * kMasterCtasPerSm, kMasterMaxGrid);
     SETUP_CUDA(cudaMemsetAsync(d.ll_part, 0, 2 * g * kMaxRedux * sizeof(uint4), q));
     SETUP_CUDA(cudaMemsetAsync(d.ll_result, 0, 2 * kMaxRedux * sizeof(uint4), q));
   }

@@ -113,6 +113,10 @@ class Phantom:
     # weights used as they are (eq. 3-4) instead of divided by |v_s| (eq. 9-10)
     vox_threshold: Optional[np.ndarray] = None    # float32 [n_vox] or None
     per_voxel_weights: bool = False
+    # lateral position (in beamlet widths, relative to the beam's leftmost beamlet) of the first beamlet of
+    # every leaf row: rows are contiguous hulls that need not start at the same place.  Needed by the MLC
+    # constraints that couple neighbouring rows (jaws-only delivery)
+    row_col0: Optional[np.ndarray] = None         # int32 [n_rows] or None (= all zero)
 
     def summary(self) -> Dict[str, object]:
         rows = np.diff(self.row_bl_ptr)
@@ -197,6 +201,8 @@ def _beam_cells(spec: PhantomSpec, u, zc, target_mask):
                 keep[iz[ok], iu[ok]] = True
     cell_to_bl = np.full((ncz, ncu), -1, dtype=np.int64)
     row_len = []
+    row_lo = []                                       # lateral cell index of each row's first beamlet
+    row_z = []
     nb = 0
     for m_ in range(ncz):
         cols = np.nonzero(keep[m_])[0]
@@ -206,7 +212,12 @@ def _beam_cells(spec: PhantomSpec, u, zc, target_mask):
         n = hi - lo + 1
         cell_to_bl[m_, lo:hi + 1] = nb + np.arange(n)
         row_len.append(n)
+        row_lo.append(lo)
+        row_z.append(m_)
         nb += n
+    if row_z and row_z[-1] - row_z[0] + 1 != len(row_z):
+        raise ValueError("leaf rows of a beam are not physically adjacent (a row without beamlets in between)")
+    _beam_cells.last_row_lo = row_lo                  # picked up by generate() (row_col0)
     return cell_to_bl, row_len, u0, z0
 
 
@@ -288,6 +299,7 @@ def generate(spec: PhantomSpec, seed: int = 0) -> Phantom:
     per_beam = []
     beam_row_ptr = [0]
     row_bl_ptr = [0]
+    row_col0 = []
     bl_base = 0
     total = np.zeros(n_in, dtype=np.int64)
     for th in gantry:
@@ -296,6 +308,8 @@ def generate(spec: PhantomSpec, seed: int = 0) -> Phantom:
         total[sel] += counts
         for n in row_len:
             row_bl_ptr.append(row_bl_ptr[-1] + n)
+        lo0 = min(_beam_cells.last_row_lo)
+        row_col0.extend(int(v - lo0) for v in _beam_cells.last_row_lo)
         beam_row_ptr.append(len(row_bl_ptr) - 1)
         bl_base += int(sum(row_len))
     n_bl = bl_base
@@ -332,6 +346,7 @@ def generate(spec: PhantomSpec, seed: int = 0) -> Phantom:
         n_beams=spec.n_beams, n_rows=len(row_bl_ptr) - 1,
         beam_row_ptr=np.asarray(beam_row_ptr, dtype=np.int32),
         row_bl_ptr=np.asarray(row_bl_ptr, dtype=np.int32),
+        row_col0=np.asarray(row_col0, dtype=np.int32),
         n_struct=len(names), vox_struct=sid[keep_vox].astype(np.int32),
         t_under=tu, w_under=wu, t_over=to, w_over=wo, struct_names=names,
         gantry_deg=gantry, vox_grid_index=lin[keep_vox], grid=spec.grid, voxel_mm=spec.voxel_mm,
