@@ -80,7 +80,21 @@ typedef struct {
   int32_t n_beams, n_rows;
   const int32_t *beam_row_ptr;   /* [n_beams+1] host, into leaf rows; beam_row_ptr[n_beams] = n_rows */
   const int32_t *row_bl_ptr;     /* [n_rows+1]  host, into beamlets;  row_bl_ptr[n_rows] = n_bl */
+  const int32_t *row_col0;       /* optional [n_rows] host (NULL = all 0): lateral position, in beamlet widths, of
+                                    the first beamlet of every leaf row (rows are contiguous hulls that need not
+                                    start at the same place; consecutive rows of a beam are physically adjacent).
+                                    >= 0.  Only read by MLC modes that couple rows (DAO_MLC_JAWS_ONLY) */
 } dao_mlc;
+
+/* MLC deliverability rule of the pricing sub-problem ("standard consecutiveness, interdigitation,
+ * connectedness and jaws-only delivery"; the paper shows results, and prints an algorithm, for the first only). */
+typedef enum {
+  DAO_MLC_CONSECUTIVE = 0,   /* every leaf row opens one contiguous interval, rows independent */
+  DAO_MLC_JAWS_ONLY = 1      /* reading J1 of DESIGN.md: the aperture is a rectangle -- consecutive leaf rows m1..m2
+                                of the beam all opened over the same lateral range [c1, c2) (positions as in
+                                row_col0), the other rows closed; per beam the rectangle with the most negative sum
+                                of w; ties: closed aperture at 0, else smallest (c1, c2, m1, m2) */
+} dao_mlc_mode;
 
 /* Structures, thresholds and weights of eq. (9)-(10).  One structure per voxel. */
 typedef struct {
@@ -114,9 +128,11 @@ typedef struct {
   int32_t sell_sigma;        /* sorting window (rows) of the internal sliced-ELL layout of D; 1 = keep the
                                 caller's voxel order; 0 = library default */
   int32_t timers;            /* non-zero: CUDA-event timers per kernel class in dao_run (default 1) */
+  int32_t mlc_mode;          /* dao_mlc_mode (default DAO_MLC_CONSECUTIVE) */
   int32_t reserved;          /* test/bench hooks, 0 in production: bit 0 forces the direct-load SpMV variant,
                                 bit 1 turns on the master's phase timers (DAO_VEC_MASTER_PHASES), bit 2 forces the span variant
                                 of the transposed SpMV even for short beamlet rows */
+  int32_t pad_;              /* keep 0 */
 } dao_options;
 
 typedef struct {

@@ -105,6 +105,7 @@ void dao_default_options(dao_options *opt) {
   opt->master_ls_tol = 0.01;
   opt->sell_sigma = 0;
   opt->timers = 1;
+  opt->mlc_mode = DAO_MLC_CONSECUTIVE;
 }
 
 dao_status dao_workspace_bytes(const dao_csr *D, const dao_mlc *mlc, const dao_structs *s, const dao_options *opt,
@@ -410,6 +411,8 @@ dao_status dao_price_from_w(dao_ctx *ctx, const float *w_dev, const int32_t *row
   Ctx *c = reinterpret_cast<Ctx *>(ctx);
   if (!c || !w_dev || !left_dev || !right_dev || !vstar_dev || !beam_price_dev || !best_dev) return DAO_E_ARG;
   const bool own = row_bl_ptr_dev == nullptr;
+  if (!own && c->opt.mlc_mode != DAO_MLC_CONSECUTIVE)
+    return fail(c, DAO_E_UNSUPPORTED, "caller-provided MLC tables are only supported with DAO_MLC_CONSECUTIVE");
   if (own) {
     if (beam_row_ptr_dev != nullptr) return fail(c, DAO_E_ARG, "pass both MLC tables or neither");
     row_bl_ptr_dev = c->d.row_bl_ptr; beam_row_ptr_dev = c->d.beam_row_ptr;

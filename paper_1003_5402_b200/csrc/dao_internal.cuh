@@ -136,6 +136,7 @@ struct DevPtrs {
   int32_t *row_bl_ptr;     // [n_rows+1]
   int32_t *bl_row;         // [n_bl]
   int32_t *row_beam;       // [n_rows]
+  int32_t *row_col0;       // [n_rows] lateral position of the first beamlet of every row
   // vectors
   float *x;                // [n_bl]
   float *xmask;            // [n_bl]
@@ -180,12 +181,13 @@ struct Ctx {
   int64_t nnz = 0;
   int32_t n_vox_pad = 0;        // n_vox rounded up to a multiple of 128
   int32_t max_rows_per_beam = 0;
+  int32_t max_beam_width = 0;   // widest beam in lateral positions (max over rows of row_col0 + row length)
   int32_t n_slices = 0;
   int64_t sell_elems = 0;
   int32_t n_tchunks = 0, n_tsegs = 0;
   dao_options opt{};
   // host copies of small tables
-  std::vector<int32_t> beam_row_ptr, row_bl_ptr;
+  std::vector<int32_t> beam_row_ptr, row_bl_ptr, row_col0;
   // device
   DevPtrs d{};
   cudaStream_t stream = nullptr;

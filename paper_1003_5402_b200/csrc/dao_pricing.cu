@@ -116,6 +116,86 @@ __global__ void __launch_bounds__(256) k_price_beams(const double *__restrict__ 
   }
 }
 
+// ------------------------------------------------------------------------------------------
+// Jaws-only pricing (PAPER.md:260 names the constraint; reading J1 of DESIGN.md): per beam the rectangle
+// (consecutive leaf rows m1..m2, one common lateral range [c1, c2)) with the most negative sum of w.
+// One CTA per beam.  Prefix sums of every row over lateral positions (fp64, zero where the row has no
+// beamlet) go to shared memory; every thread takes column pairs (c1, c2) in ascending order and runs the
+// paper's one-pass scan over the ROWS on the row sums P[m][c2] - P[m][c1]; a block
+// argmin with the key (value, c1, c2) picks the winner.  Strict comparisons everywhere: the closed aperture
+// wins ties at 0, equal negative values keep the smallest (c1, c2, m1, m2) -- the oracle's enumeration order.
+// Outputs per row: the rectangle clipped to the row's beamlets as half-open leaves inside the row, and the
+// sum of w over them.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_price_jaws(const float *__restrict__ w, const int32_t *__restrict__ beam_row_ptr,
+                                                    const int32_t *__restrict__ row_bl_ptr,
+                                                    const int32_t *__restrict__ row_col0, int32_t width,
+                                                    double *__restrict__ vstar, int32_t *__restrict__ left,
+                                                    int32_t *__restrict__ right, double *__restrict__ beam_price,
+                                                    double *__restrict__ beam_absmax) {
+  extern __shared__ double P[];                     // [R][width + 1]
+  __shared__ double s_val[256];
+  __shared__ int32_t s_c1[256], s_c2[256], s_m1[256], s_m2[256];
+  __shared__ double s_abs[256];
+  const int t = threadIdx.x, b = blockIdx.x;
+  const int32_t r0 = beam_row_ptr[b], R = beam_row_ptr[b + 1] - r0;
+  const int ld = width + 1;
+  double amax = 0.0;
+  for (int m = t; m < R; m += 256) {                // one thread per row: sequential prefix sum, left to right
+    const int32_t r = r0 + m, c0 = row_col0 ? row_col0[r] : 0, b0 = row_bl_ptr[r], n = row_bl_ptr[r + 1] - b0;
+    double s = 0.0;
+    P[m * ld] = 0.0;
+    for (int c = 0; c < width; ++c) {
+      if (c >= c0 && c < c0 + n) {
+        const double wv = (double)w[b0 + (c - c0)];
+        s += wv;
+        amax = fmax(amax, fabs(wv));
+      }
+      P[m * ld + c + 1] = s;
+    }
+  }
+  __syncthreads();
+  double best = 0.0;
+  int32_t bc1 = 0, bc2 = 0, bm1 = 0, bm2 = 0;       // closed: m2 exclusive, empty range
+  for (int c1 = 0; c1 < width; ++c1) {
+    for (int c2 = c1 + 1 + t; c2 <= width; c2 += 256) {
+      double v = 0.0, vbar = 0.0;
+      int32_t l = 0;
+      for (int m = 0; m < R; ++m) {
+        v += P[m * ld + c2] - P[m * ld + c1];
+        if (v - vbar < best) { best = v - vbar; bc1 = c1; bc2 = c2; bm1 = l; bm2 = m + 1; }
+        if (v > vbar) { vbar = v; l = m + 1; }
+      }
+    }
+  }
+  s_val[t] = best; s_c1[t] = bc1; s_c2[t] = bc2; s_m1[t] = bm1; s_m2[t] = bm2; s_abs[t] = amax;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (t < o) {
+      const double ov = s_val[t + o];
+      const bool take = ov < s_val[t] ||
+                        (ov == s_val[t] && ov < 0.0 &&
+                         (s_c1[t + o] < s_c1[t] || (s_c1[t + o] == s_c1[t] && s_c2[t + o] < s_c2[t])));
+      if (take) { s_val[t] = ov; s_c1[t] = s_c1[t + o]; s_c2[t] = s_c2[t + o]; s_m1[t] = s_m1[t + o]; s_m2[t] = s_m2[t + o]; }
+      s_abs[t] = fmax(s_abs[t], s_abs[t + o]);
+    }
+    __syncthreads();
+  }
+  const int32_t c1 = s_c1[0], c2 = s_c2[0], m1 = s_m1[0], m2 = s_m2[0];
+  for (int m = t; m < R; m += 256) {
+    const int32_t r = r0 + m, c0 = row_col0 ? row_col0[r] : 0, n = row_bl_ptr[r + 1] - row_bl_ptr[r];
+    int32_t lo = max(c1, c0), hi = min(c2, c0 + n);
+    if (m < m1 || m >= m2 || hi <= lo) { lo = c0; hi = c0; }
+    left[r] = hi > lo ? lo - c0 : 0;
+    right[r] = hi > lo ? hi - c0 : 0;
+    vstar[r] = P[m * ld + hi] - P[m * ld + lo];
+  }
+  if (t == 0) {
+    beam_price[b] = s_val[0];
+    beam_absmax[b] = s_abs[0];
+  }
+}
+
 // step 6b: b* = argmin_b price_b (ties: smallest b), optimality test (reading S3), candidate
 // bookkeeping.  One CTA.
 __global__ void __launch_bounds__(256) k_price_select(const double *__restrict__ beam_price,
@@ -203,16 +283,27 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
                            double *row_absmax, double *beam_price, double *beam_absmax, int32_t *best_out,
                            bool update_state) {
   const int wpb = 8;
-  if (n_rows > 0) {
-    k_price_rows<<<(n_rows + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(w, row_bl_ptr, n_rows, vstar, left,
-                                                                      right, row_absmax);
+  if (c->opt.mlc_mode == DAO_MLC_JAWS_ONLY) {
+    // the context's own MLC tables only (dao_price_from_w refuses caller tables in this mode)
+    const size_t smem = (size_t)c->max_rows_per_beam * (size_t)(c->max_beam_width + 1) * sizeof(double);
+    cudaError_t e = cudaFuncSetAttribute(k_price_jaws, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_price_jaws<<<n_beams, 256, smem, c->stream>>>(w, beam_row_ptr, row_bl_ptr, c->d.row_col0, c->max_beam_width, vstar,
+                                                    left, right, beam_price, beam_absmax);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  } else {
+    if (n_rows > 0) {
+      k_price_rows<<<(n_rows + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(w, row_bl_ptr, n_rows, vstar, left,
+                                                                        right, row_absmax);
+      cudaError_t e = cudaGetLastError();
+      if (e != cudaSuccess) return e;
+    }
+    k_price_beams<<<(n_beams + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(vstar, row_absmax, beam_row_ptr, n_beams,
+                                                                         beam_price, beam_absmax);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }
-  k_price_beams<<<(n_beams + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(vstar, row_absmax, beam_row_ptr, n_beams,
-                                                                       beam_price, beam_absmax);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
   k_price_select<<<1, 256, 0, c->stream>>>(beam_price, beam_absmax, n_beams, beam_row_ptr, left, right, best_out,
                                            update_state ? c->d.state : nullptr, c->opt.price_tol, c->opt.k_max,
                                            c->max_rows_per_beam, c->d.ap_beam, c->d.ap_left, c->d.ap_right);

@@ -118,6 +118,7 @@ static void carve_workspace(Carver &cv, const Dims &dm, const HostLayout &L, Dev
   d->row_bl_ptr = cv.take<int32_t>((size_t)dm.n_rows + 1);
   d->bl_row = cv.take<int32_t>((size_t)dm.n_bl);
   d->row_beam = cv.take<int32_t>((size_t)dm.n_rows);
+  d->row_col0 = cv.take<int32_t>((size_t)dm.n_rows);
   d->x = cv.take<float>((size_t)dm.n_bl);
   d->xmask = cv.take<float>((size_t)dm.n_bl);
   d->z = cv.take<float>(vp);
@@ -216,7 +217,8 @@ static dao_status check_args(const dao_csr *D, const dao_mlc *mlc, const dao_str
   if (opt->k_max > DAO_MAX_APERTURES) { *err = "k_max > DAO_MAX_APERTURES"; return DAO_E_UNSUPPORTED; }
   if (opt->master_max_iter < 0 || !(opt->master_tol >= 0.0) || !(opt->price_tol >= 0.0) ||
       (opt->master_method != 0 && opt->master_method != 1) || opt->sell_sigma < 0 ||
-      !(opt->master_ls_tol > 0.0) || !(opt->master_ls_tol < 1.0)) {
+      !(opt->master_ls_tol > 0.0) || !(opt->master_ls_tol < 1.0) ||
+      (opt->mlc_mode != DAO_MLC_CONSECUTIVE && opt->mlc_mode != DAO_MLC_JAWS_ONLY)) {
     *err = "bad option value"; return DAO_E_ARG;
   }
   // MLC tables (host)
@@ -234,6 +236,9 @@ static dao_status check_args(const dao_csr *D, const dao_mlc *mlc, const dao_str
   }
   for (int r = 0; r < mlc->n_rows; ++r)
     if (mlc->row_bl_ptr[r + 1] < mlc->row_bl_ptr[r]) { *err = "row_bl_ptr not monotone"; return DAO_E_SHAPE; }
+  if (mlc->row_col0)
+    for (int r = 0; r < mlc->n_rows; ++r)
+      if (mlc->row_col0[r] < 0 || mlc->row_col0[r] > (1 << 20)) { *err = "row_col0 out of range"; return DAO_E_SHAPE; }
   dm->n_vox = D->n_vox; dm->n_bl = D->n_bl; dm->nnz = D->nnz;
   dm->n_beams = mlc->n_beams; dm->n_rows = mlc->n_rows; dm->k_max = opt->k_max;
   dm->max_rows = std::max(max_rows, 1);
@@ -559,6 +564,16 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   c->max_rows_per_beam = dm.max_rows;
   c->beam_row_ptr.assign(mlc->beam_row_ptr, mlc->beam_row_ptr + dm.n_beams + 1);
   c->row_bl_ptr.assign(mlc->row_bl_ptr, mlc->row_bl_ptr + dm.n_rows + 1);
+  c->row_col0.assign((size_t)dm.n_rows, 0);
+  if (mlc->row_col0) c->row_col0.assign(mlc->row_col0, mlc->row_col0 + dm.n_rows);
+  c->max_beam_width = 0;
+  for (int r = 0; r < dm.n_rows; ++r)
+    c->max_beam_width = std::max(c->max_beam_width, c->row_col0[r] + (c->row_bl_ptr[r + 1] - c->row_bl_ptr[r]));
+  if (c->opt.mlc_mode == DAO_MLC_JAWS_ONLY &&
+      (size_t)dm.max_rows * (size_t)(c->max_beam_width + 1) * sizeof(double) > (size_t)200 * 1024) {
+    c->err = "jaws-only pricing: rows x lateral width of a beam exceeds the shared-memory table (200 KB)";
+    return DAO_E_UNSUPPORTED;
+  }
   cudaStream_t q = c->stream;
   DevPtrs &d = c->d;
 
@@ -701,6 +716,7 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
     SETUP_CUDA(cudaMemcpyAsync(d.row_bl_ptr, c->row_bl_ptr.data(), ((size_t)dm.n_rows + 1) * 4, cudaMemcpyHostToDevice, q));
     SETUP_CUDA(cudaMemcpyAsync(d.bl_row, bl_row.data(), (size_t)dm.n_bl * 4, cudaMemcpyHostToDevice, q));
     SETUP_CUDA(cudaMemcpyAsync(d.row_beam, row_beam.data(), (size_t)dm.n_rows * 4, cudaMemcpyHostToDevice, q));
+    SETUP_CUDA(cudaMemcpyAsync(d.row_col0, c->row_col0.data(), (size_t)dm.n_rows * 4, cudaMemcpyHostToDevice, q));
     SETUP_CUDA(cudaStreamSynchronize(q));
   }
 

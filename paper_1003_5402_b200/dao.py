@@ -21,6 +21,7 @@ DAO_OK = 0
 STATUS_NAMES = {0: "DAO_OK", 1: "DAO_E_ARG", 2: "DAO_E_SHAPE", 3: "DAO_E_CUDA", 4: "DAO_E_ALLOC",
                 5: "DAO_E_STATE", 6: "DAO_E_UNSUPPORTED"}
 MEM_HOST, MEM_DEVICE = 0, 1
+MLC_CONSECUTIVE, MLC_JAWS_ONLY = 0, 1
 MAX_APERTURES = 128
 (VEC_Z, VEC_G, VEC_W, VEC_X, VEC_Y, VEC_VSTAR, VEC_LEFT, VEC_RIGHT, VEC_BEAM_PRICE, VEC_HISTORY,
  VEC_MASTER_Z, VEC_MASTER_PHASES) = range(12)
@@ -45,7 +46,7 @@ class CCsr(C.Structure):
 
 class CMlc(C.Structure):
     _fields_ = [("n_beams", C.c_int32), ("n_rows", C.c_int32), ("beam_row_ptr", C.c_void_p),
-                ("row_bl_ptr", C.c_void_p)]
+                ("row_bl_ptr", C.c_void_p), ("row_col0", C.c_void_p)]
 
 
 class CStructs(C.Structure):
@@ -57,7 +58,7 @@ class CStructs(C.Structure):
 class COptions(C.Structure):
     _fields_ = [("k_max", C.c_int32), ("master_max_iter", C.c_int32), ("master_tol", C.c_double),
                 ("price_tol", C.c_double), ("master_ls_tol", C.c_double), ("master_method", C.c_int32), ("sell_sigma", C.c_int32),
-                ("timers", C.c_int32), ("reserved", C.c_int32)]
+                ("timers", C.c_int32), ("mlc_mode", C.c_int32), ("reserved", C.c_int32), ("pad_", C.c_int32)]
 
 
 class CSizes(C.Structure):
@@ -217,6 +218,13 @@ class Dao:
                 self._keep.append(vt)
                 st.vox_threshold = _np_ptr(vt)
         mlc = CMlc(self.n_beams, self.n_rows, _np_ptr(brp), _np_ptr(rbp))
+        rc0 = getattr(ph, "row_col0", None)
+        if rc0 is not None:
+            rc0 = np.ascontiguousarray(rc0, dtype=np.int32)
+            if rc0.size != self.n_rows:
+                raise ValueError("row_col0 must have n_rows entries")
+            self._keep.append(rc0)
+            mlc.row_col0 = _np_ptr(rc0)
 
         sizes = CSizes()
         rc = self.lib.dao_workspace_bytes(C.byref(csr), C.byref(mlc), C.byref(st), C.byref(self.opt), C.byref(sizes))

@@ -1,0 +1,114 @@
+"""GPU parity of the jaws-only pricing mode (reading J1 of DESIGN.md: apertures are
+rectangles) against the oracle's enumeration of every rectangle, fed the same fp32 w."""
+import numpy as np
+import pytest
+
+from oracle import dao_oracle as orc
+import parity_utils as pu
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def D():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1003_5402_b200 import dao
+    dao.load_library()
+    return dao
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _check_against_oracle(ph, w32, le, ri, vs, bp, best, exact):
+    pr = orc.price_jaws(w32.astype(np.float64), ph.beam_row_ptr, ph.row_bl_ptr, ph.row_col0)
+    scale = max(float(np.abs(pr.beam_price).max()), float(np.abs(w32).max()), 1e-300)
+    np.testing.assert_allclose(bp, pr.beam_price, rtol=0, atol=1e-9 * scale)
+    if exact:
+        assert np.array_equal(le, pr.left) and np.array_equal(ri, pr.right) and np.array_equal(vs, pr.vstar)
+        assert int(best) == pr.best_beam
+    else:
+        # the GPU's rectangle must reach the oracle's optimum per beam (north-star band rule: 1e-6 relative) ...
+        for b in range(ph.n_beams):
+            rows = range(ph.beam_row_ptr[b], ph.beam_row_ptr[b + 1])
+            got = sum(float(w32[ph.row_bl_ptr[r] + le[r]: ph.row_bl_ptr[r] + ri[r]].astype(np.float64).sum()) for r in rows)
+            assert abs(got - pr.beam_price[b]) <= 1e-6 * scale
+        # ... and be the same rectangle wherever no other rectangle comes that close (checked through the leaves)
+        same = np.array_equal(le, pr.left) and np.array_equal(ri, pr.right)
+        assert same or _has_near_tie(ph, w32, pr, scale)
+        pu.check_beam(bp, best, pr.beam_price)
+
+
+def _has_near_tie(ph, w32, pr, scale):
+    """True when some beam has two different rectangles within 1e-6 relative of its optimum."""
+    w = w32.astype(np.float64)
+    for b in range(ph.n_beams):
+        r0, r1 = int(ph.beam_row_ptr[b]), int(ph.beam_row_ptr[b + 1])
+        C = max(int(ph.row_col0[r] + ph.row_bl_ptr[r + 1] - ph.row_bl_ptr[r]) for r in range(r0, r1))
+        W = np.zeros((r1 - r0, C))
+        for r in range(r0, r1):
+            n = int(ph.row_bl_ptr[r + 1] - ph.row_bl_ptr[r])
+            W[r - r0, ph.row_col0[r]: ph.row_col0[r] + n] = w[ph.row_bl_ptr[r]: ph.row_bl_ptr[r] + n]
+        P = np.zeros((r1 - r0 + 1, C + 1)); P[1:, 1:] = W.cumsum(0).cumsum(1)
+        vals = []
+        for c1 in range(C):
+            for c2 in range(c1 + 1, C + 1):
+                col = P[:, c2] - P[:, c1]
+                d = col[None, :] - col[:, None]
+                vals.append(d[np.triu_indices(r1 - r0 + 1, 1)])
+        v = np.sort(np.concatenate(vals))
+        if v[1] - v[0] <= 1e-6 * scale:
+            return True
+    return False
+
+
+@pytest.mark.parametrize("case", ["cfg0", "mini"])
+def test_jaws_pricing_matches_oracle(D, case, cfg0, mini):
+    ph = {"cfg0": cfg0, "mini": mini}[case]
+    rng = np.random.default_rng(3)
+    with D.Dao(ph, mlc_mode=D.MLC_JAWS_ONLY) as d:
+        # the method's own first-iteration w (all w_i <= 0: the whole field of the best beam opens)
+        info = d.price()
+        w = d.get_vector(D.VEC_W)
+        le, ri, vs = d.get_vector(D.VEC_LEFT), d.get_vector(D.VEC_RIGHT), d.get_vector(D.VEC_VSTAR)
+        _check_against_oracle(ph, w, le, ri, vs, d.get_vector(D.VEC_BEAM_PRICE), info.beam, exact=False)
+        # random and integer-valued (exact ties) beamlet gradients through the hook
+        for trial in range(4):
+            wr = rng.standard_normal(ph.n_bl).astype(np.float32)
+            if trial >= 2:
+                wr = np.round(2 * wr).astype(np.float32)
+            le, ri, vs, bp, best = (t.cpu().numpy() for t in d.price_from_w(_dev(wr)))
+            _check_against_oracle(ph, wr, le, ri, vs, bp, best[0], exact=trial >= 2)
+        with pytest.raises(D.DaoError):                     # caller tables carry no lateral offsets
+            d.price_from_w(_dev(wr), _dev(ph.row_bl_ptr), _dev(ph.beam_row_ptr))
+
+
+@pytest.mark.parametrize("case,n_ap", [("cfg0", 10), ("mini", 25)])
+def test_jaws_plan_matches_oracle(D, case, n_ap, cfg0, mini):
+    ph = {"cfg0": cfg0, "mini": mini}[case]
+    ref = orc.run(ph, n_ap, mlc="jaws")
+    with D.Dao(ph, k_max=n_ap, mlc_mode=D.MLC_JAWS_ONLY) as d:
+        info = d.run(n_ap)
+        plan = d.get_plan()
+    assert abs(info.objective - ref.objective) <= 1e-3 * ref.objective, (info.objective, ref.objective)
+    assert info.n_apertures == len(ref.beams)
+    for k, b in enumerate(plan.beams):                       # every aperture is a rectangle in lateral positions
+        r0 = int(ph.beam_row_ptr[b])
+        le, ri = plan.leaves(k)
+        rows = [m for m in range(le.size) if ri[m] > le[m]]
+        assert rows and rows == list(range(rows[0], rows[-1] + 1))
+        c1 = min(int(ph.row_col0[r0 + m] + le[m]) for m in rows)
+        c2 = max(int(ph.row_col0[r0 + m] + ri[m]) for m in rows)
+        for m in rows:
+            c0 = int(ph.row_col0[r0 + m]); n = int(ph.row_bl_ptr[r0 + m + 1] - ph.row_bl_ptr[r0 + m])
+            assert (c0 + le[m], c0 + ri[m]) == (max(c1, c0), min(c2, c0 + n))
+    n_same = sum(1 for k in range(len(ref.beams)) if plan.beams[k] == ref.beams[k]
+                 and np.array_equal(plan.leaves(k)[0], ref.lefts[k]) and np.array_equal(plan.leaves(k)[1], ref.rights[k]))
+    cons = orc.run(ph, n_ap)
+    assert info.objective >= cons.objective * (1 - 1e-6)      # rectangles are a subset of the consecutive apertures
+    print(f"{case} jaws-only: F_gpu={info.objective:.10g} F_oracle={ref.objective:.10g} same apertures {n_same}/{len(ref.beams)}; "
+          f"consecutive-leaves oracle F={cons.objective:.10g}")
