@@ -545,3 +545,87 @@ void orc_price_jaws(const double *w, int32_t n_beams, const int32_t *beam_row_pt
     }
     *best_beam = bb;
 }
+
+/* ------------------------------------------------------------------ interdigitation / connectedness pricing
+ * The other two MLC constraints PAPER.md:260 names without an algorithm.  Leaf positions are lateral
+ * positions in beamlet widths (row r's beamlets occupy [c0_r, c0_r + n_r)); the state of a row is (a, b),
+ * 0 <= a <= b <= W: left leaf tip at a, right leaf tip at b, open cells [a, b), closed when a == b.  An open
+ * row stays inside its own beamlets (c0_r <= a < b <= c0_r + n_r); a closed leaf pair may park anywhere.
+ *   Reading J2 (mode 2, interdigitation forbidden): for physically adjacent rows m, m+1 a leaf may not pass
+ *   the opposing leaf of the neighbouring row:  a_m <= b_{m+1}  and  a_{m+1} <= b_m.
+ *   Reading J3 (mode 3, connectedness): the open rows are consecutive and the open intervals of adjacent open
+ *   rows share at least one lateral position: max(a_m, a_{m+1}) < min(b_m, b_{m+1}); closed rows are free.
+ * The sub-problem minimises the sum of w over the open beamlets of a beam.  The feasible sets are chains over
+ * the rows, so the minimum is a shortest path through the layered graph rows x states (the construction of
+ * Romeijn et al. 2005 that the paper cites); it is written out as the plain dynamic programme
+ *   f_m(s) = val_m(s) + min { f_{m-1}(s') : s' compatible with s },  O(rows x states^2),
+ * and pinned against exhaustive enumeration of every aperture on tiny beams.  Several apertures can attain
+ * the minimum (closed rows park anywhere; exact ties), so only the VALUE is unique; the aperture returned is
+ * the first minimiser in state order and callers compare values and check feasibility. */
+static int mlc_compatible(int mode, int a0, int b0, int a1, int b1)
+{   /* states of two adjacent rows */
+    if (mode == 2) return a0 <= b1 && a1 <= b0;
+    /* mode 3: both open -> overlap; otherwise handled by the phase logic of the caller */
+    return (a0 > a1 ? a0 : a1) < (b0 < b1 ? b0 : b1);
+}
+
+void orc_price_chain(int32_t mode, const double *w, int32_t n_beams, const int32_t *beam_row_ptr,
+                     const int32_t *row_bl_ptr, const int32_t *row_col0, double *vstar, int32_t *left,
+                     int32_t *right, double *beam_price, int32_t *best_beam)
+{
+    int32_t bb = -1; double bbv = 0.0;
+    for (int32_t bm = 0; bm < n_beams; ++bm) {
+        const int32_t r0 = beam_row_ptr[bm], R = beam_row_ptr[bm + 1] - r0;
+        int32_t W = 0;
+        for (int32_t r = r0; r < r0 + R; ++r) {
+            const int32_t e = (row_col0 ? row_col0[r] : 0) + (row_bl_ptr[r + 1] - row_bl_ptr[r]);
+            if (e > W) W = e;
+        }
+        const int32_t S = (W + 1) * (W + 2) / 2;                 /* states (a, b), a <= b, in the order a, then b */
+        int32_t *sa = (int32_t *)malloc(sizeof(int32_t) * (size_t)S), *sb = (int32_t *)malloc(sizeof(int32_t) * (size_t)S);
+        { int32_t k = 0; for (int32_t a = 0; a <= W; ++a) for (int32_t b = a; b <= W; ++b) { sa[k] = a; sb[k] = b; ++k; } }
+        double *f = (double *)malloc(sizeof(double) * (size_t)S * (size_t)(R > 0 ? R : 1));
+        int32_t *from = (int32_t *)malloc(sizeof(int32_t) * (size_t)S * (size_t)(R > 0 ? R : 1));
+        double best = 0.0; int32_t best_m = -1, best_s = -1;     /* connectedness: best end of an open run */
+        for (int32_t m = 0; m < R; ++m) {
+            const int32_t r = r0 + m, c0 = row_col0 ? row_col0[r] : 0, n = row_bl_ptr[r + 1] - row_bl_ptr[r];
+            for (int32_t s = 0; s < S; ++s) {
+                const int32_t a = sa[s], b = sb[s];
+                double val = 0.0, prev = 0.0; int32_t arg = -1;
+                f[(size_t)m * S + s] = INFINITY; from[(size_t)m * S + s] = -1;
+                if (a < b) {                                      /* open: inside the row's own beamlets */
+                    if (a < c0 || b > c0 + n) continue;
+                    for (int32_t c = a; c < b; ++c) val += w[row_bl_ptr[r] + (c - c0)];
+                } else if (mode == 3) continue;                   /* connectedness tracks open states only */
+                if (m > 0) {
+                    prev = (mode == 3) ? 0.0 : INFINITY;          /* mode 3: the run may start at this row */
+                    for (int32_t q = 0; q < S; ++q) {
+                        const double fq = f[(size_t)(m - 1) * S + q];
+                        if (fq == INFINITY || !mlc_compatible(mode, sa[q], sb[q], a, b)) continue;
+                        if (fq < prev) { prev = fq; arg = q; }
+                    }
+                    if (prev == INFINITY) continue;
+                }
+                f[(size_t)m * S + s] = val + prev; from[(size_t)m * S + s] = arg;
+                if (mode == 3 && val + prev < best) { best = val + prev; best_m = m; best_s = s; }
+            }
+        }
+        if (mode == 2) {                                          /* best state of the last row */
+            best = INFINITY; best_m = R - 1;
+            for (int32_t s = 0; s < S; ++s) if (f[(size_t)(R - 1) * S + s] < best) { best = f[(size_t)(R - 1) * S + s]; best_s = s; }
+        }
+        for (int32_t r = r0; r < r0 + R; ++r) { left[r] = 0; right[r] = 0; vstar[r] = 0.0; }
+        for (int32_t m = best_m, s = best_s; m >= 0 && s >= 0; s = from[(size_t)m * S + s], --m) {
+            const int32_t r = r0 + m, c0 = row_col0 ? row_col0[r] : 0;
+            if (sa[s] < sb[s]) {
+                double val = 0.0;
+                for (int32_t c = sa[s]; c < sb[s]; ++c) val += w[row_bl_ptr[r] + (c - c0)];
+                left[r] = sa[s] - c0; right[r] = sb[s] - c0; vstar[r] = val;
+            }
+        }
+        beam_price[bm] = best;
+        free(sa); free(sb); free(f); free(from);
+        if (bb < 0 || best < bbv) { bb = bm; bbv = best; }
+    }
+    *best_beam = bb;
+}

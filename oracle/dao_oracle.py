@@ -183,6 +183,25 @@ def price_jaws(w, beam_row_ptr, row_bl_ptr, row_col0=None) -> Pricing:
     return Pricing(vs, le, ri, bp, bb.value)
 
 
+MLC_MODES = {"consecutive": 0, "jaws": 1, "interdigitation": 2, "connected": 3}
+
+
+def price_chain(w, beam_row_ptr, row_bl_ptr, row_col0=None, mlc: str = "interdigitation") -> Pricing:
+    """Sub-problem under the interdigitation (reading J2) or connectedness (reading J3) constraint
+    (PAPER.md:260): dynamic programme over the leaf rows of every beam.  Only the value is unique."""
+    w, brp, rbp = _f64(w), _i32(beam_row_ptr), _i32(row_bl_ptr)
+    n_beams, n_rows = brp.size - 1, rbp.size - 1
+    rc0 = _i32(np.zeros(n_rows) if row_col0 is None else row_col0)
+    vs = np.zeros(n_rows, dtype=np.float64)
+    le = np.zeros(n_rows, dtype=np.int32)
+    ri = np.zeros(n_rows, dtype=np.int32)
+    bp = np.zeros(n_beams, dtype=np.float64)
+    bb = C.c_int32(-1)
+    lib().orc_price_chain(C.c_int32(MLC_MODES[mlc]), _p(w), C.c_int32(n_beams), _p(brp), _p(rbp), _p(rc0), _p(vs),
+                          _p(le), _p(ri), _p(bp), C.byref(bb))
+    return Pricing(vs, le, ri, bp, bb.value)
+
+
 def aperture_open_mask(n_bl, beam, left, right, beam_row_ptr, row_bl_ptr):
     """0/1 mask over beamlets of an aperture in `beam` with per-row half-open leaves (rows of that beam)."""
     m = np.zeros(n_bl, dtype=np.uint8)
@@ -317,6 +336,8 @@ def run(ph, max_apertures: int, master_tol: float = 1e-10, master_max_iter: int 
         w = beamlet_gradient(ph.row_ptr, ph.col_idx, ph.val, g, n_bl)
         if mlc == "jaws":
             pr = price_jaws(w, ph.beam_row_ptr, ph.row_bl_ptr, getattr(ph, "row_col0", None))
+        elif mlc in ("interdigitation", "connected"):
+            pr = price_chain(w, ph.beam_row_ptr, ph.row_bl_ptr, getattr(ph, "row_col0", None), mlc)
         else:
             pr = price(w, ph.beam_row_ptr, ph.row_bl_ptr)
         if price_converged(pr, w, ph.beam_row_ptr, price_tol):
