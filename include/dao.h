@@ -90,6 +90,13 @@ typedef struct {
  * connectedness and jaws-only delivery"; the paper shows results, and prints an algorithm, for the first only). */
 typedef enum {
   DAO_MLC_CONSECUTIVE = 0,   /* every leaf row opens one contiguous interval, rows independent */
+  DAO_MLC_INTERDIGITATION = 2,  /* reading J2: leaf states (a, b) = lateral tip positions of the left and right leaf
+                                of a row (open cells [a, b), closed when a == b, an open row stays inside its own
+                                beamlets, a closed pair parks anywhere); for physically adjacent rows m, m+1 no leaf
+                                passes the opposing leaf of the neighbour: a_m <= b_{m+1} and a_{m+1} <= b_m */
+  DAO_MLC_CONNECTED = 3,     /* reading J3: the open rows are consecutive and the open intervals of adjacent open
+                                rows share at least one lateral position; closed rows are free.  Modes 2 and 3 are
+                                solved by a dynamic programme over the rows; only the optimal VALUE is unique */
   DAO_MLC_JAWS_ONLY = 1      /* reading J1 of DESIGN.md: the aperture is a rectangle -- consecutive leaf rows m1..m2
                                 of the beam all opened over the same lateral range [c1, c2) (positions as in
                                 row_col0), the other rows closed; per beam the rectangle with the most negative sum

@@ -244,6 +244,7 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
                            double *row_absmax, double *beam_price, double *beam_absmax, int32_t *best_out,
                            bool update_state);
 cudaError_t launch_append_candidate(Ctx *c);
+size_t chain_pricing_smem(int32_t max_rows, int32_t width);   // shared memory of k_price_chain
 
 // dao_fmo.cu
 dao_status fmo_solve(Ctx *c, int32_t max_iter, double tol, bool warm_start, dao_fmo_info *out);

@@ -196,6 +196,132 @@ __global__ void __launch_bounds__(256) k_price_jaws(const float *__restrict__ w,
   }
 }
 
+// ------------------------------------------------------------------------------------------
+// Interdigitation (reading J2) and connectedness (reading J3) pricing (PAPER.md:260 names the constraints):
+// the feasible apertures of a beam are chains over its leaf rows, so the best one is a shortest path through
+// the layered graph rows x leaf states (a, b) (lateral tip positions, 0 <= a <= b <= W; closed when a == b):
+//   f_m(s) = val_m(s) + min { f_{m-1}(s') : s' compatible with s }.
+// One CTA per beam; the row prefix sums, two layers of f and the back-pointers live in shared memory; a thread
+// owns states s = t, t + 256, ... of the current row and scans the previous layer in state order with strict
+// comparisons, which reproduces the oracle's choice among equal minima.  Thread 0 walks the back-pointers.
+//   J2: a_m <= b_{m+1} and a_{m+1} <= b_m for adjacent rows (a closed pair may park anywhere in [0, W]);
+//   J3: the open rows are consecutive and adjacent open intervals share a lateral position.
+// An open row stays inside its own beamlets.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_price_chain(int32_t mode, const float *__restrict__ w,
+                                                     const int32_t *__restrict__ beam_row_ptr,
+                                                     const int32_t *__restrict__ row_bl_ptr,
+                                                     const int32_t *__restrict__ row_col0, int32_t width, int32_t max_rows,
+                                                     double *__restrict__ vstar, int32_t *__restrict__ left,
+                                                     int32_t *__restrict__ right, double *__restrict__ beam_price,
+                                                     double *__restrict__ beam_absmax) {
+  extern __shared__ double sm_d[];
+  const int ld = width + 1;
+  const int S = (width + 1) * (width + 2) / 2;
+  double *P = sm_d;                                         // [max_rows][ld]
+  double *f0 = P + (size_t)max_rows * ld;                   // [S]
+  double *f1 = f0 + S;                                      // [S]
+  int16_t *sa = reinterpret_cast<int16_t *>(f1 + S);        // [S]
+  int16_t *sb = sa + S;                                     // [S]
+  int16_t *from = sb + S;                                   // [max_rows][S]
+  __shared__ double s_val[256];
+  __shared__ int32_t s_m[256], s_s[256];
+  __shared__ double s_abs[256];
+  const int t = threadIdx.x, b = blockIdx.x;
+  const int32_t r0 = beam_row_ptr[b], R = beam_row_ptr[b + 1] - r0;
+  double amax = 0.0;
+  for (int m = t; m < R; m += 256) {
+    const int32_t r = r0 + m, c0 = row_col0 ? row_col0[r] : 0, b0 = row_bl_ptr[r], n = row_bl_ptr[r + 1] - b0;
+    double s = 0.0;
+    P[m * ld] = 0.0;
+    for (int c = 0; c < width; ++c) {
+      if (c >= c0 && c < c0 + n) {
+        const double wv = (double)w[b0 + (c - c0)];
+        s += wv;
+        amax = fmax(amax, fabs(wv));
+      }
+      P[m * ld + c + 1] = s;
+    }
+  }
+  for (int a = t; a <= width; a += 256) {                   // states in the order a, then b
+    int k = a * (width + 1) - a * (a - 1) / 2;
+    for (int bb = a; bb <= width; ++bb, ++k) { sa[k] = (int16_t)a; sb[k] = (int16_t)bb; }
+  }
+  __syncthreads();
+  double best = CUDART_INF;                                 // J3: best end of an open run seen by this thread
+  int32_t best_m = -1, best_s = -1;
+  if (mode == 3) best = 0.0;
+  double *fp = f0, *fc = f1;
+  for (int m = 0; m < R; ++m) {
+    const int32_t r = r0 + m, c0 = row_col0 ? row_col0[r] : 0, n = row_bl_ptr[r + 1] - row_bl_ptr[r];
+    for (int s = t; s < S; s += 256) {
+      const int a = sa[s], bb = sb[s];
+      double out = CUDART_INF;
+      int arg = -1;
+      const bool open = a < bb;
+      const bool valid = open ? (a >= c0 && bb <= c0 + n) : (mode != 3);
+      if (valid) {
+        const double val = open ? P[m * ld + bb] - P[m * ld + a] : 0.0;
+        double prev = 0.0;
+        if (m > 0) {
+          prev = (mode == 3) ? 0.0 : CUDART_INF;            // J3: the run may start at this row
+          for (int q = 0; q < S; ++q) {
+            const double fq = fp[q];
+            if (fq == CUDART_INF) continue;
+            const int a0 = sa[q], b0 = sb[q];
+            const bool ok = (mode == 2) ? (a0 <= bb && a <= b0) : (max(a0, a) < min(b0, bb));
+            if (ok && fq < prev) { prev = fq; arg = q; }
+          }
+        }
+        if (prev != CUDART_INF) {
+          out = val + prev;
+          if (mode == 3 && out < best) { best = out; best_m = m; best_s = s; }
+        }
+      }
+      fc[s] = out;
+      from[(size_t)m * S + s] = (int16_t)arg;
+    }
+    __syncthreads();
+    double *tmp = fp; fp = fc; fc = tmp;
+  }
+  if (mode == 2) {                                          // best state of the last row (fp = last layer)
+    best = CUDART_INF; best_m = R - 1; best_s = -1;
+    for (int s = t; s < S; s += 256)
+      if (fp[s] < best) { best = fp[s]; best_s = s; }
+  }
+  s_val[t] = best; s_m[t] = best_m; s_s[t] = best_s; s_abs[t] = amax;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (t < o) {
+      const double ov = s_val[t + o];
+      const int om = s_m[t + o], os = s_s[t + o];
+      // key (value, m, s); an entry without a state (s < 0) only carries the neutral value
+      const bool take = os >= 0 && (s_s[t] < 0 || ov < s_val[t] ||
+                                    (ov == s_val[t] && (om < s_m[t] || (om == s_m[t] && os < s_s[t]))));
+      if (take) { s_val[t] = ov; s_m[t] = om; s_s[t] = os; }
+      s_abs[t] = fmax(s_abs[t], s_abs[t + o]);
+    }
+    __syncthreads();
+  }
+  for (int m = t; m < R; m += 256) { left[r0 + m] = 0; right[r0 + m] = 0; vstar[r0 + m] = 0.0; }
+  __syncthreads();
+  if (t == 0) {
+    double price = s_val[0];
+    int m = s_m[0], s = s_s[0];
+    if (s < 0) { price = 0.0; m = -1; }                     // nothing improves: closed aperture
+    for (; m >= 0 && s >= 0; s = from[(size_t)m * S + s], --m) {
+      const int a = sa[s], bb = sb[s];
+      if (a < bb) {
+        const int32_t r = r0 + m, c0 = row_col0 ? row_col0[r] : 0;
+        left[r] = a - c0; right[r] = bb - c0;
+        vstar[r] = P[m * ld + bb] - P[m * ld + a];
+      }
+    }
+    beam_price[b] = price;
+    beam_absmax[b] = s_abs[0];
+  }
+}
+
 // step 6b: b* = argmin_b price_b (ties: smallest b), optimality test (reading S3), candidate
 // bookkeeping.  One CTA.
 __global__ void __launch_bounds__(256) k_price_select(const double *__restrict__ beam_price,
@@ -278,6 +404,11 @@ __global__ void __launch_bounds__(256) k_price_select(const double *__restrict__
   }
 }
 
+size_t chain_pricing_smem(int32_t max_rows, int32_t width) {
+  const size_t S = (size_t)(width + 1) * (size_t)(width + 2) / 2;
+  return align_up((size_t)max_rows * (size_t)(width + 1) * 8 + 2 * S * 8 + 2 * S * 2 + (size_t)max_rows * S * 2, 16);
+}
+
 cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, const int32_t *beam_row_ptr,
                            int32_t n_rows, int32_t n_beams, int32_t *left, int32_t *right, double *vstar,
                            double *row_absmax, double *beam_price, double *beam_absmax, int32_t *best_out,
@@ -290,6 +421,15 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
     if (e != cudaSuccess) return e;
     k_price_jaws<<<n_beams, 256, smem, c->stream>>>(w, beam_row_ptr, row_bl_ptr, c->d.row_col0, c->max_beam_width, vstar,
                                                     left, right, beam_price, beam_absmax);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  } else if (c->opt.mlc_mode == DAO_MLC_INTERDIGITATION || c->opt.mlc_mode == DAO_MLC_CONNECTED) {
+    const size_t smem = chain_pricing_smem(c->max_rows_per_beam, c->max_beam_width);
+    cudaError_t e = cudaFuncSetAttribute(k_price_chain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_price_chain<<<n_beams, 256, smem, c->stream>>>(c->opt.mlc_mode, w, beam_row_ptr, row_bl_ptr, c->d.row_col0,
+                                                     c->max_beam_width, c->max_rows_per_beam, vstar, left, right,
+                                                     beam_price, beam_absmax);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   } else {

@@ -218,7 +218,7 @@ static dao_status check_args(const dao_csr *D, const dao_mlc *mlc, const dao_str
   if (opt->master_max_iter < 0 || !(opt->master_tol >= 0.0) || !(opt->price_tol >= 0.0) ||
       (opt->master_method != 0 && opt->master_method != 1) || opt->sell_sigma < 0 ||
       !(opt->master_ls_tol > 0.0) || !(opt->master_ls_tol < 1.0) ||
-      (opt->mlc_mode != DAO_MLC_CONSECUTIVE && opt->mlc_mode != DAO_MLC_JAWS_ONLY)) {
+      (opt->mlc_mode < DAO_MLC_CONSECUTIVE || opt->mlc_mode > DAO_MLC_CONNECTED)) {
     *err = "bad option value"; return DAO_E_ARG;
   }
   // MLC tables (host)
@@ -572,6 +572,11 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   if (c->opt.mlc_mode == DAO_MLC_JAWS_ONLY &&
       (size_t)dm.max_rows * (size_t)(c->max_beam_width + 1) * sizeof(double) > (size_t)200 * 1024) {
     c->err = "jaws-only pricing: rows x lateral width of a beam exceeds the shared-memory table (200 KB)";
+    return DAO_E_UNSUPPORTED;
+  }
+  if ((c->opt.mlc_mode == DAO_MLC_INTERDIGITATION || c->opt.mlc_mode == DAO_MLC_CONNECTED) &&
+      (chain_pricing_smem(dm.max_rows, c->max_beam_width) > (size_t)200 * 1024 || c->max_beam_width > 30000)) {
+    c->err = "interdigitation / connectedness pricing: rows x leaf states of a beam exceed the shared-memory tables (200 KB)";
     return DAO_E_UNSUPPORTED;
   }
   cudaStream_t q = c->stream;

@@ -21,7 +21,7 @@ DAO_OK = 0
 STATUS_NAMES = {0: "DAO_OK", 1: "DAO_E_ARG", 2: "DAO_E_SHAPE", 3: "DAO_E_CUDA", 4: "DAO_E_ALLOC",
                 5: "DAO_E_STATE", 6: "DAO_E_UNSUPPORTED"}
 MEM_HOST, MEM_DEVICE = 0, 1
-MLC_CONSECUTIVE, MLC_JAWS_ONLY = 0, 1
+MLC_CONSECUTIVE, MLC_JAWS_ONLY, MLC_INTERDIGITATION, MLC_CONNECTED = 0, 1, 2, 3
 MAX_APERTURES = 128
 (VEC_Z, VEC_G, VEC_W, VEC_X, VEC_Y, VEC_VSTAR, VEC_LEFT, VEC_RIGHT, VEC_BEAM_PRICE, VEC_HISTORY,
  VEC_MASTER_Z, VEC_MASTER_PHASES) = range(12)

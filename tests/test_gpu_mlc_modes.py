@@ -1,5 +1,5 @@
-"""GPU parity of the jaws-only pricing mode (reading J1 of DESIGN.md: apertures are
-rectangles) against the oracle's enumeration of every rectangle, fed the same fp32 w."""
+"""GPU parity of the alternative MLC deliverability rules of the pricing sub-problem (
+readings J1-J3 of DESIGN.md): jaws-only (rectangles), interdigitation, connectedness -- against the oracle, fed the same fp32 w."""
 import numpy as np
 import pytest
 
@@ -112,3 +112,75 @@ def test_jaws_plan_matches_oracle(D, case, n_ap, cfg0, mini):
     assert info.objective >= cons.objective * (1 - 1e-6)      # rectangles are a subset of the consecutive apertures
     print(f"{case} jaws-only: F_gpu={info.objective:.10g} F_oracle={ref.objective:.10g} same apertures {n_same}/{len(ref.beams)}; "
           f"consecutive-leaves oracle F={cons.objective:.10g}")
+
+
+# ----------------------------------------------------------------------------- interdigitation / connectedness
+def _chain_feasible(mode, ph, b, le, ri):
+    r0, r1 = int(ph.beam_row_ptr[b]), int(ph.beam_row_ptr[b + 1])
+    conf = [(int(ph.row_col0[r] + le[r]), int(ph.row_col0[r] + ri[r])) for r in range(r0, r1)]
+    opens = [(m, c) for m, c in enumerate(conf) if c[0] < c[1]]
+    if mode == "connected":
+        rows = [m for m, _ in opens]
+        if rows and rows != list(range(rows[0], rows[-1] + 1)):
+            return False
+        return all(max(c0[0], c1[0]) < min(c0[1], c1[1]) for (_, c0), (_, c1) in zip(opens[:-1], opens[1:]))
+    # interdigitation: a closed row between two open ones must find a parking position p with
+    # a_up <= p <= b_up and a_down <= p <= b_down, i.e. the chain of constraints is checked through closed rows
+    lo, hi = -10 ** 9, 10 ** 9          # feasible parking range propagated through closed rows
+    prev = None
+    for m, (a, b_) in enumerate(conf):
+        if a < b_:
+            if prev is not None:
+                if prev[0] == m - 1:
+                    if not (prev[1][0] <= b_ and a <= prev[1][1]):
+                        return False
+                else:                   # closed rows in between: park them in [max(a's), min(b's)] of both neighbours
+                    if max(prev[1][0], a) > min(prev[1][1], b_):
+                        return False
+            prev = (m, (a, b_))
+    return True
+
+
+@pytest.mark.parametrize("mode", ["interdigitation", "connected"])
+@pytest.mark.parametrize("case", ["cfg0", "mini"])
+def test_chain_pricing_matches_oracle(D, mode, case, cfg0, mini):
+    ph = {"cfg0": cfg0, "mini": mini}[case]
+    code = {"interdigitation": D.MLC_INTERDIGITATION, "connected": D.MLC_CONNECTED}[mode]
+    rng = np.random.default_rng(11)
+    with D.Dao(ph, mlc_mode=code) as d:
+        for trial in range(5):
+            wr = rng.standard_normal(ph.n_bl).astype(np.float32)
+            if trial >= 3:
+                wr = np.round(2 * wr).astype(np.float32)              # exact arithmetic, exact ties
+            le, ri, vs, bp, best = (t.cpu().numpy() for t in d.price_from_w(_dev(wr)))
+            pr = orc.price_chain(wr.astype(np.float64), ph.beam_row_ptr, ph.row_bl_ptr, ph.row_col0, mode)
+            scale = max(float(np.abs(pr.beam_price).max()), 1e-300)
+            np.testing.assert_allclose(bp, pr.beam_price, rtol=0, atol=1e-9 * scale)       # the value is unique
+            pu.check_beam(bp, best[0], pr.beam_price)
+            for b in range(ph.n_beams):                                                     # the aperture: valid + attains it
+                rows = range(ph.beam_row_ptr[b], ph.beam_row_ptr[b + 1])
+                got = sum(float(wr[ph.row_bl_ptr[r] + le[r]: ph.row_bl_ptr[r] + ri[r]].astype(np.float64).sum()) for r in rows)
+                assert abs(got - pr.beam_price[b]) <= 1e-9 * scale
+                assert _chain_feasible(mode, ph, b, le, ri)
+                for r in rows:
+                    assert 0 <= le[r] <= ri[r] <= ph.row_bl_ptr[r + 1] - ph.row_bl_ptr[r]
+            if trial >= 3:                                            # same scan order -> same aperture even on ties
+                assert np.array_equal(le, pr.left) and np.array_equal(ri, pr.right)
+
+
+@pytest.mark.parametrize("mode", ["interdigitation", "connected"])
+def test_chain_plan_matches_oracle(D, mode, mini):
+    code = {"interdigitation": D.MLC_INTERDIGITATION, "connected": D.MLC_CONNECTED}[mode]
+    ref = orc.run(mini, 20, mlc=mode)
+    with D.Dao(mini, k_max=20, mlc_mode=code) as d:
+        info = d.run(20)
+        plan = d.get_plan()
+    assert abs(info.objective - ref.objective) <= 1e-3 * ref.objective, (info.objective, ref.objective)
+    for k, b in enumerate(plan.beams):
+        le = np.zeros(mini.n_rows, np.int32); ri = np.zeros(mini.n_rows, np.int32)
+        r0 = int(mini.beam_row_ptr[b]); l, r = plan.leaves(k)
+        le[r0:r0 + l.size] = l; ri[r0:r0 + r.size] = r
+        assert _chain_feasible(mode, mini, int(b), le, ri)
+    n_same = sum(1 for k in range(min(len(ref.beams), len(plan.beams))) if plan.beams[k] == ref.beams[k]
+                 and np.array_equal(plan.leaves(k)[0], ref.lefts[k]) and np.array_equal(plan.leaves(k)[1], ref.rights[k]))
+    print(f"mini {mode}: F_gpu={info.objective:.10g} F_oracle={ref.objective:.10g} same apertures {n_same}/{len(ref.beams)}")
