@@ -357,8 +357,10 @@ def main():
                 "peak_source": peak_src, "alg_bytes_per_launch": master_alg_per_launch,
                 "alg_bytes_model": "per projected-gradient iteration 2 passes over A (2*4*V*K) + 3 passes over z, dz, sid (3*17*V)",
                 "avg_launch_us": 1e6 * master_avg, "share_of_step": kernels["master"]["share"],
-                "note": "A (4*V*K bytes, 121 MB at K = 50) stays L2-resident on this workload, so DRAM traffic is far below "
-                        "the algorithmic bytes; the fraction is of the HBM roof the same bytes would face from DRAM"}
+                "note": "alg_bytes_per_launch is the average over the solves of a plan (K = 1..50); traffic is the ncu DRAM "
+                        "figure of ONE late solve (K = 47, profiles/r01d_ncu_full.md).  While 4*V*K is well below the 126 MB L2 "
+                        "(K <~ 40 here) the block is L2-resident and a solve reads ~70 MB from DRAM; late in the plan it "
+                        "streams from HBM and DRAM traffic equals the algorithmic bytes"}
 
     def class_roofline(key, kernel_name, label):
         k = kernels[key]

@@ -413,12 +413,18 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
       RingPos pp{0, 0u};
       bool first_round = true;
       bool stop = slab_len == 0;
-      while (!stop) {
-        for (int tile = 0; tile < n_tiles && !stop; ++tile) {
+      // Pass i walks the block forwards (tiles and columns ascending) when i is even and backwards when
+      // it is odd: what the previous pass read last is read first, so an LRU-like L2 keeps serving the
+      // most recent part of A when 4 V K bytes no longer fit it (cyclic order would miss everywhere).
+      for (unsigned pass = 0; !stop; ++pass) {
+        const bool rev = (pass & 1u) != 0u;
+        for (int ti = 0; ti < n_tiles && !stop; ++ti) {
+          const int tile = rev ? n_tiles - 1 - ti : ti;
           const int t0 = tile * kMasterTileVox;
           const uint32_t bytes = (uint32_t)min(kMasterTileVox, slab_len - t0) * 4u;
           const float *src = p.A + (size_t)v0 + (size_t)t0;
-          for (int k = 0; k < K; ++k) {
+          for (int kj = 0; kj < K; ++kj) {
+            const int k = rev ? K - 1 - kj : kj;
             if (!first_round) {
               while (!mbar_try_wait(&sm.empty[pp.stage], pp.phase ^ 1u)) {
                 if (s_stop) { stop = true; break; }
@@ -482,6 +488,7 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
   } while (0)
 
   RingPos cp{0, 0u};                       // consumer position in the A stream
+  unsigned pass_no = 0;                    // passes consumed so far: the parity gives the traversal direction
   // strips of this warp inside a tile: warp and warp + kNW (128 voxels each, 4 per lane)
   const int l0 = warp * 128 + lane * 4, l1 = (warp + kNW) * 128 + lane * 4;
 
@@ -491,12 +498,14 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
   const bool permuted = p.z_in_smem != 0;
   auto pos = [&](int strip_base, int u) { return permuted ? strip_base + u * 32 + lane : strip_base + lane * 4 + u; };
 
-  // one D-type pass: out[i] = sum_k coef[k] A[k][i] on the slab (fp64, k ascending).  With
+  // one D-type pass: out[i] = sum_k coef[k] A[k][i] on the slab (fp64, k in the order of the pass).  With
   // t_commit != 0 the pending step is committed first: z += t_commit * out_old (same thread, same
   // voxels).  With curv, returns this thread's part of phi''(0) = sum 2 c_j out_j^2.
   auto pass_d = [&](const double *coef, double *out, double t_commit, bool curv) -> double {
     double h_acc = 0.0;
-    for (int tile = 0; tile < n_tiles; ++tile) {
+    const bool rev = (pass_no++ & 1u) != 0u;
+    for (int ti = 0; ti < n_tiles; ++ti) {
+      const int tile = rev ? n_tiles - 1 - ti : ti;
       const int t0 = tile * kMasterTileVox;
       const int tn = min(kMasterTileVox, slab_len - t0);
       const bool a0 = l0 < tn, a1 = (kMasterStrips > 1) && l1 < tn;
@@ -505,7 +514,7 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
       // work per warp between two barrier round trips; four stages per step measured slower: registers)
       for (int k = 0; k < K; k += 2) {
         const bool two = k + 1 < K;
-        const double c0 = coef[k], c1 = two ? coef[k + 1] : 0.0;
+        const double c0 = coef[rev ? K - 1 - k : k], c1 = two ? coef[rev ? K - 2 - k : k + 1] : 0.0;
         RingPos q0 = cp, q1 = cp;
         q1.advance(NS);
         const long long tw = prof ? clock64() : 0ll;
@@ -587,7 +596,9 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
   for (;;) {
     // ============ phase G: g(z + t dz), grad = A^T g, F, phi'(t), phi''(t) ================
     double f_acc = 0.0, s1_acc = 0.0, s2_acc = 0.0;
-    for (int tile = 0; tile < n_tiles; ++tile) {
+    const bool rev = (pass_no++ & 1u) != 0u;
+    for (int ti = 0; ti < n_tiles; ++ti) {
+      const int tile = rev ? n_tiles - 1 - ti : ti;
       const int t0 = tile * kMasterTileVox;
       const int tn = min(kMasterTileVox, slab_len - t0);
       const bool a0 = l0 < tn, a1 = (kMasterStrips > 1) && l1 < tn;
@@ -658,10 +669,11 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
           }
         }
         const double r = butterfly8(d, lane);
-        const int kk = kb8 + butterfly8_index(lane);
-        if ((lane & 3) == 0) {
+        const int kj = kb8 + butterfly8_index(lane);       // position in the pass; column k = kj or K - 1 - kj
+        const int kk = rev ? K - 1 - kj : kj;
+        if ((lane & 3) == 0 && kj < K) {
           double *slot = sm.warp_part + warp * DAO_MAX_APERTURES + kk;
-          *slot = (tile == 0) ? r : (*slot + r);
+          *slot = (ti == 0) ? r : (*slot + r);
         }
       }
     }
