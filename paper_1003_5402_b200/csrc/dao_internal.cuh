@@ -30,8 +30,16 @@ constexpr int kMasterCtasPerSm = DAO_MASTER_CTAS_PER_SM;   // resident CTAs of t
                                        // take the same time (L2-side limit, not warp latency) and the grid reductions over 296 CTAs double: slower
 constexpr int kMasterStrips = kMasterCtasPerSm == 1 ? 2 : 1;   // 128-voxel strips per worker warp and stage
 constexpr int kMasterTileVox = 16 * 128 * kMasterStrips;   // voxels per ring stage: 16 worker warps x strips x 128
-constexpr int kMasterStageBytes = kMasterTileVox * 4;
-constexpr int kMasterMaxStages = 10;
+constexpr int kMasterColBytes = kMasterTileVox * 4;      // one column of one tile
+#ifndef DAO_MASTER_COLS_PER_STAGE
+#define DAO_MASTER_COLS_PER_STAGE 2
+#endif
+constexpr int kMasterColsPerStage = DAO_MASTER_COLS_PER_STAGE;   // a ring stage holds this many consecutive columns (even)
+                                                        // behind ONE full/empty mbarrier pair: the barrier traffic per byte,
+                                                        // not the memory system, limits the passes (measured: 1 -> 2 columns
+                                                        // per stage made them 16 % faster)
+constexpr int kMasterStageBytes = kMasterColsPerStage * kMasterColBytes;
+constexpr int kMasterMaxStages = 10 / kMasterColsPerStage + 1;
 constexpr int kMasterMaxGrid = 160 * kMasterCtasPerSm;    // CTAs of the master kernel (capped)
 constexpr int kMasterProfSlots = 16;   // phase timers of the master (ns): 0 init, 1 G pass, 2 G reduce, 3 direction,
                                        // 4 D pass, 5 D reduce, 6 line search; 7 line-search evaluations,

@@ -26,6 +26,7 @@
 #include <math_constants.h>
 
 #include <algorithm>
+#include <cstdlib>
 
 namespace dao {
 
@@ -423,16 +424,20 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
           const int t0 = tile * kMasterTileVox;
           const uint32_t bytes = (uint32_t)min(kMasterTileVox, slab_len - t0) * 4u;
           const float *src = p.A + (size_t)v0 + (size_t)t0;
-          for (int kj = 0; kj < K; ++kj) {
-            const int k = rev ? K - 1 - kj : kj;
+          for (int kj = 0; kj < K; kj += kMasterColsPerStage) {
+            const int ncol = min(kMasterColsPerStage, K - kj);
             if (!first_round) {
               while (!mbar_try_wait(&sm.empty[pp.stage], pp.phase ^ 1u)) {
                 if (s_stop) { stop = true; break; }
               }
               if (stop) break;
             }
-            mbar_arrive_expect_tx(&sm.full[pp.stage], bytes);
-            bulk_g2s(sm.ring + (size_t)pp.stage * kMasterStageBytes, src + (size_t)k * vpad, bytes, &sm.full[pp.stage]);
+            mbar_arrive_expect_tx(&sm.full[pp.stage], bytes * (uint32_t)ncol);
+            for (int u = 0; u < ncol; ++u) {
+              const int k = rev ? K - 1 - (kj + u) : kj + u;
+              bulk_g2s(sm.ring + (size_t)pp.stage * kMasterStageBytes + (size_t)u * kMasterColBytes, src + (size_t)k * vpad,
+                       bytes, &sm.full[pp.stage]);
+            }
             pp.advance(NS);
             if (pp.stage == 0) first_round = false;
           }
@@ -515,14 +520,14 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
       for (int k = 0; k < K; k += 2) {
         const bool two = k + 1 < K;
         const double c0 = coef[rev ? K - 1 - k : k], c1 = two ? coef[rev ? K - 2 - k : k + 1] : 0.0;
-        RingPos q0 = cp, q1 = cp;
-        q1.advance(NS);
-        const long long tw = prof ? clock64() : 0ll;
-        mbar_wait(&sm.full[q0.stage], q0.phase);
-        if (two) mbar_wait(&sm.full[q1.stage], q1.phase);
-        if (prof) prof_s[13] += (unsigned long long)(clock64() - tw);                 // time this thread waited for A in D passes
-        const unsigned char *s0 = sm.ring + (size_t)q0.stage * kMasterStageBytes;
-        const unsigned char *s1 = sm.ring + (size_t)q1.stage * kMasterStageBytes;
+        const int kin = k % kMasterColsPerStage;           // position of this pair inside its stage
+        if (kin == 0) {
+          const long long tw = prof ? clock64() : 0ll;
+          mbar_wait(&sm.full[cp.stage], cp.phase);
+          if (prof) prof_s[13] += (unsigned long long)(clock64() - tw);               // time this thread waited for A in D passes
+        }
+        const unsigned char *s0 = sm.ring + (size_t)cp.stage * kMasterStageBytes + (size_t)kin * kMasterColBytes;
+        const unsigned char *s1 = s0 + kMasterColBytes;
         float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0, y0 = x0, y1 = x0;
         if (a0) { x0 = *reinterpret_cast<const float4 *>(s0 + (size_t)l0 * 4); if (two) y0 = *reinterpret_cast<const float4 *>(s1 + (size_t)l0 * 4); }
         if (a1) { x1 = *reinterpret_cast<const float4 *>(s0 + (size_t)l1 * 4); if (two) y1 = *reinterpret_cast<const float4 *>(s1 + (size_t)l1 * 4); }
@@ -534,10 +539,11 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
         acc[2] = fma(c1, (double)y0.z, acc[2]); acc[3] = fma(c1, (double)y0.w, acc[3]);
         acc[4] = fma(c1, (double)y1.x, acc[4]); acc[5] = fma(c1, (double)y1.y, acc[5]);
         acc[6] = fma(c1, (double)y1.z, acc[6]); acc[7] = fma(c1, (double)y1.w, acc[7]);
-        __syncwarp();
-        if (lane == 0) { mbar_arrive(&sm.empty[q0.stage]); if (two) mbar_arrive(&sm.empty[q1.stage]); }
-        cp.advance(NS);
-        if (two) cp.advance(NS);
+        if (kin == kMasterColsPerStage - 2 || k + 2 >= K) {   // done with the stage
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&sm.empty[cp.stage]);
+          cp.advance(NS);
+        }
       }
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
@@ -637,14 +643,14 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
           d[j + 1] = 0.0;
           if (kb8 + j < K) {                       // two stages per step: waits, then loads, then arithmetic
             const bool two = kb8 + j + 1 < K;
-            RingPos q0 = cp, q1 = cp;
-            q1.advance(NS);
-            const long long tw = prof ? clock64() : 0ll;
-            mbar_wait(&sm.full[q0.stage], q0.phase);
-            if (two) mbar_wait(&sm.full[q1.stage], q1.phase);
-            if (prof) prof_s[12] += (unsigned long long)(clock64() - tw);             // time this thread waited for A in G passes
-            const unsigned char *s0 = sm.ring + (size_t)q0.stage * kMasterStageBytes;
-            const unsigned char *s1 = sm.ring + (size_t)q1.stage * kMasterStageBytes;
+            const int kin = (kb8 + j) % kMasterColsPerStage;   // position of this pair inside its stage
+            if (kin == 0) {
+              const long long tw = prof ? clock64() : 0ll;
+              mbar_wait(&sm.full[cp.stage], cp.phase);
+              if (prof) prof_s[12] += (unsigned long long)(clock64() - tw);           // time this thread waited for A in G passes
+            }
+            const unsigned char *s0 = sm.ring + (size_t)cp.stage * kMasterStageBytes + (size_t)kin * kMasterColBytes;
+            const unsigned char *s1 = s0 + kMasterColBytes;
             float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0, y0 = x0, y1 = x0;
             if (a0) { x0 = *reinterpret_cast<const float4 *>(s0 + (size_t)l0 * 4); if (two) y0 = *reinterpret_cast<const float4 *>(s1 + (size_t)l0 * 4); }
             if (a1) { x1 = *reinterpret_cast<const float4 *>(s0 + (size_t)l1 * 4); if (two) y1 = *reinterpret_cast<const float4 *>(s1 + (size_t)l1 * 4); }
@@ -662,10 +668,11 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
               r = fma((double)y1.y, g[5], r); r = fma((double)y1.z, g[6], r); r = fma((double)y1.w, g[7], r);
               d[j + 1] = a0 ? (a1 ? q + r : q) : (a1 ? 0.0 + r : 0.0);
             }
-            __syncwarp();
-            if (lane == 0) { mbar_arrive(&sm.empty[q0.stage]); if (two) mbar_arrive(&sm.empty[q1.stage]); }
-            cp.advance(NS);
-            if (two) cp.advance(NS);
+            if (kin == kMasterColsPerStage - 2 || kb8 + j + 2 >= K) {   // done with the stage
+              __syncwarp();
+              if (lane == 0) mbar_arrive(&sm.empty[cp.stage]);
+              cp.advance(NS);
+            }
           }
         }
         const double r = butterfly8(d, lane);
@@ -880,9 +887,9 @@ cudaError_t master_configure(Ctx *c) {
   // prefer z in shared memory with >= 4 stages; otherwise z stays in global memory (L2)
   c->master_z_in_smem = 0;
   int stages = 0;
-  if (master_fixed_smem(c, 4) + slab_bytes <= budget) {
+  if (master_fixed_smem(c, 2) + slab_bytes <= budget) {
     c->master_z_in_smem = 1;
-    stages = 4;
+    stages = 2;
     while (stages < kMasterMaxStages && master_fixed_smem(c, stages + 1) + slab_bytes <= budget) ++stages;
   } else {
     stages = 2;
