@@ -260,7 +260,7 @@ def main():
     ap.add_argument("--config", default="cfg1")
     ap.add_argument("--impl", default="dao", choices=["dao", "reference"])
     ap.add_argument("--apertures", type=int, default=N_APERTURES, help="apertures per plan (50; configs[4] asks for 100)")
-    ap.add_argument("--ref-apertures", type=int, default=3, help="apertures per step of the reference arm / cpu_baseline")
+    ap.add_argument("--ref-apertures", type=int, default=12, help="apertures per step of the reference arm / cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[3] kernel sweep (markdown table)")
