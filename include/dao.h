@@ -216,7 +216,8 @@ typedef enum {               /* dao_get_vector selectors; lengths in elements */
   DAO_VEC_MASTER_PHASES = 11 /* uint64 [16]     phase timers of the master kernel, accumulated since dao_create when
                                 dao_options.reserved has bit 1 (value 2) set, else zeros.  Nanoseconds of CTA 0 in:
                                 0 set-up and z = A y, 1 gradient pass over A, 2 gradient reduction, 3 direction,
-                                4 dz = A p pass, 5 curvature reduction, 6 line search, 10 publish; counts:
+                                4 dz = A p pass, 5 curvature reduction, 6 line search, 10 publish, 14 accept / refine decision (split off
+                                slot 3); counts:
                                 7 line-search evaluations, 8 projected-gradient iterations, 9 calls; SM clock cycles thread 0 of
                                 CTA 0 spent waiting for stages of A: 12 in gradient passes, 13 in dz passes */
 } dao_vector;

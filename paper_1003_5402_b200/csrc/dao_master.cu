@@ -768,6 +768,7 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
       ++iters;
       wsync();
     }
+    PROF_MARK(14);                       // accept / refine decision and the y update
     F = F_trial;
 
     // ================= phase P: direction (warp 0, identical in every CTA) ================
