@@ -108,38 +108,71 @@ __global__ void k_spmvt_finish(int32_t n_bl, const int32_t *__restrict__ t_ptr,
 // entries per beamlet): one warp per row of D^T, lanes stride over the row with 4
 // independent accumulators, shuffle tree, w written directly -- no span tables, no second kernel.  Fixed
 // order per row: bit-reproducible.
+template <int WPR>   // warps per row: 1, 2, 4 or 8 (few rows -> more warps per row, so that the GPU is filled)
 __global__ void __launch_bounds__(kTThreads) k_spmvt_rows(int32_t n_bl, const int32_t *__restrict__ t_ptr,
                                                           const int32_t *__restrict__ t_row,
                                                           const float *__restrict__ t_val, const float *__restrict__ g,
                                                           float *__restrict__ w, const int32_t *__restrict__ skip) {
+  __shared__ double part[kTThreads / 32];
   if (skip && *skip) return;
-  const int lane = threadIdx.x & 31;
-  const int nw = (gridDim.x * blockDim.x) >> 5;
-  for (int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; row < n_bl; row += nw) {
-    const int lo = t_ptr[row], hi = t_ptr[row + 1];
-    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-    int e = lo + lane;
-    for (; e + 96 < hi; e += 128) {
-      const int r0 = ld_stream_i32(t_row + e), r1 = ld_stream_i32(t_row + e + 32);
-      const int r2 = ld_stream_i32(t_row + e + 64), r3 = ld_stream_i32(t_row + e + 96);
-      const float v0 = ld_stream_f32(t_val + e), v1 = ld_stream_f32(t_val + e + 32);
-      const float v2 = ld_stream_f32(t_val + e + 64), v3 = ld_stream_f32(t_val + e + 96);
-      a0 = fma((double)v0, (double)ld_gather_f32(g + r0), a0);
-      a1 = fma((double)v1, (double)ld_gather_f32(g + r1), a1);
-      a2 = fma((double)v2, (double)ld_gather_f32(g + r2), a2);
-      a3 = fma((double)v3, (double)ld_gather_f32(g + r3), a3);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int kRowsPerCta = (kTThreads / 32) / WPR;
+  const int sub = warp % WPR;                         // this warp's share of the row
+  for (int row0 = blockIdx.x * kRowsPerCta; row0 < n_bl; row0 += gridDim.x * kRowsPerCta) {
+    const int row = row0 + warp / WPR;
+    double acc = 0.0;
+    if (row < n_bl) {
+      const int lo = t_ptr[row], hi = t_ptr[row + 1];
+      double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+      // the warps of a row interleave rounds of 128 entries
+      for (int base = lo + 128 * sub; base < hi; base += 128 * WPR) {
+        const int e = base + lane;
+        if (base + 128 <= hi) {
+          const int r0 = ld_stream_i32(t_row + e), r1 = ld_stream_i32(t_row + e + 32);
+          const int r2 = ld_stream_i32(t_row + e + 64), r3 = ld_stream_i32(t_row + e + 96);
+          const float v0 = ld_stream_f32(t_val + e), v1 = ld_stream_f32(t_val + e + 32);
+          const float v2 = ld_stream_f32(t_val + e + 64), v3 = ld_stream_f32(t_val + e + 96);
+          a0 = fma((double)v0, (double)ld_gather_f32(g + r0), a0);
+          a1 = fma((double)v1, (double)ld_gather_f32(g + r1), a1);
+          a2 = fma((double)v2, (double)ld_gather_f32(g + r2), a2);
+          a3 = fma((double)v3, (double)ld_gather_f32(g + r3), a3);
+        } else {
+          for (int q = e; q < hi; q += 32)
+            a0 = fma((double)ld_stream_f32(t_val + q), (double)ld_gather_f32(g + ld_stream_i32(t_row + q)), a0);
+        }
+      }
+      acc = warp_sum_f64((a0 + a1) + (a2 + a3));
     }
-    for (; e < hi; e += 32) a0 = fma((double)ld_stream_f32(t_val + e), (double)ld_gather_f32(g + ld_stream_i32(t_row + e)), a0);
-    const double acc = warp_sum_f64((a0 + a1) + (a2 + a3));
-    if (lane == 0) w[row] = (float)acc;
+    if (WPR == 1) {
+      if (lane == 0 && row < n_bl) w[row] = (float)acc;
+    } else {
+      __syncthreads();
+      if (lane == 0) part[warp] = acc;
+      __syncthreads();
+      if (sub == 0 && lane == 0 && row < n_bl) {
+        double s = 0.0;
+#pragma unroll
+        for (int u = 0; u < WPR; ++u) s += part[warp + u];   // fixed order
+        w[row] = (float)s;
+      }
+    }
   }
 }
 
 cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out, const int32_t *skip) {
   if (c->n_bl > 0 && c->nnz / c->n_bl < kTChunk && !(c->opt.reserved & 4)) {
     const int wpb = kTThreads / 32;
-    int grid = std::min((c->n_bl + wpb - 1) / wpb, c->n_sm * kTCtasPerSm);
-    k_spmvt_rows<<<std::max(grid, 1), kTThreads, 0, c->stream>>>(c->n_bl, c->d.t_ptr, c->d.t_row, c->d.t_val, g, w_out, skip);
+    const int target = c->n_sm * 32;                  // warps that fill the GPU
+    int wpr = 1;
+    while (wpr < wpb && c->n_bl * wpr < target) wpr *= 2;
+    const int rows_per_cta = wpb / wpr;
+    const int grid = std::max(1, std::min((c->n_bl + rows_per_cta - 1) / rows_per_cta, c->n_sm * kTCtasPerSm));
+    switch (wpr) {
+      case 1: k_spmvt_rows<1><<<grid, kTThreads, 0, c->stream>>>(c->n_bl, c->d.t_ptr, c->d.t_row, c->d.t_val, g, w_out, skip); break;
+      case 2: k_spmvt_rows<2><<<grid, kTThreads, 0, c->stream>>>(c->n_bl, c->d.t_ptr, c->d.t_row, c->d.t_val, g, w_out, skip); break;
+      case 4: k_spmvt_rows<4><<<grid, kTThreads, 0, c->stream>>>(c->n_bl, c->d.t_ptr, c->d.t_row, c->d.t_val, g, w_out, skip); break;
+      default: k_spmvt_rows<8><<<grid, kTThreads, 0, c->stream>>>(c->n_bl, c->d.t_ptr, c->d.t_row, c->d.t_val, g, w_out, skip); break;
+    }
     return cudaGetLastError();
   }
   if (c->n_tchunks > 0) {
