@@ -79,7 +79,7 @@ static dao_status enqueue_dose(Ctx *c) {
 static dao_status enqueue_pricing(Ctx *c) {
   API_CUDA(launch_spmv_t(c, c->d.g, c->d.w));
   API_CUDA(launch_pricing(c, c->d.w, c->d.row_bl_ptr, c->d.beam_row_ptr, c->n_rows, c->n_beams, c->d.left, c->d.right,
-                          c->d.vstar, c->d.row_absmax, c->d.beam_price, c->d.beam_absmax, nullptr, true));
+                          c->d.vstar, c->d.row_absmax, c->d.beam_price, c->d.beam_absmax, nullptr, true, c->max_row_len));
   return DAO_OK;
 }
 // step 7 (append + column) and step 8
@@ -268,7 +268,8 @@ dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out) {
     API_CUDA(launch_spmv_t(c, c->d.g, c->d.w));
     if (timers) API_CUDA(cudaEventRecord(c->ev[3], c->stream));
     API_CUDA(launch_pricing(c, c->d.w, c->d.row_bl_ptr, c->d.beam_row_ptr, c->n_rows, c->n_beams, c->d.left,
-                            c->d.right, c->d.vstar, c->d.row_absmax, c->d.beam_price, c->d.beam_absmax, nullptr, true));
+                            c->d.right, c->d.vstar, c->d.row_absmax, c->d.beam_price, c->d.beam_absmax, nullptr, true,
+                            c->max_row_len));
     if (timers) API_CUDA(cudaEventRecord(c->ev[4], c->stream));
     st = enqueue_column(c);
     if (st != DAO_OK) return st;
@@ -430,7 +431,7 @@ dao_status dao_price_from_w(dao_ctx *ctx, const float *w_dev, const int32_t *row
     beam_abs = row_abs + n_rows;
   }
   API_CUDA(launch_pricing(c, w_dev, row_bl_ptr_dev, beam_row_ptr_dev, n_rows, n_beams, left_dev, right_dev, vstar_dev,
-                          row_abs, beam_price_dev, beam_abs, best_dev, false));
+                          row_abs, beam_price_dev, beam_abs, best_dev, false, own ? c->max_row_len : -1));
   return DAO_OK;
 }
 

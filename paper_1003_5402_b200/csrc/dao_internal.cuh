@@ -82,7 +82,7 @@ struct DevState {
   uint32_t bar_gen;
   int64_t pg_iter_total;
   int32_t n_duplicates;
-  int32_t pad_;
+  int32_t price_maxlen;    // longest leaf row of caller-provided MLC tables (dao_price_from_w), decided on the device
 };
 
 // Device state of the FMO solve (dao_fmo.cu); the host reads it every few iterations.
@@ -189,6 +189,7 @@ struct Ctx {
   int64_t nnz = 0;
   int32_t n_vox_pad = 0;        // n_vox rounded up to a multiple of 128
   int32_t max_rows_per_beam = 0;
+  int32_t max_row_len = 0;      // longest leaf row of the context's own MLC tables
   int32_t max_beam_width = 0;   // widest beam in lateral positions (max over rows of row_col0 + row length)
   int32_t n_slices = 0;
   int64_t sell_elems = 0;
@@ -250,7 +251,7 @@ void spmv_configure(Ctx *c);
 cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, const int32_t *beam_row_ptr,
                            int32_t n_rows, int32_t n_beams, int32_t *left, int32_t *right, double *vstar,
                            double *row_absmax, double *beam_price, double *beam_absmax, int32_t *best_out,
-                           bool update_state);
+                           bool update_state, int32_t max_row_len = 0 /* 0 = unknown: warp-per-row kernel */);
 cudaError_t launch_append_candidate(Ctx *c);
 size_t chain_pricing_smem(int32_t max_rows, int32_t width);   // shared memory of k_price_chain
 

@@ -6,7 +6,12 @@
 
 #include <math_constants.h>
 
+#include <algorithm>
+
 namespace dao {
+
+constexpr int kPriceSeqMaxLen = 88;    // longest leaf row the thread-per-row kernel stages
+constexpr int kPriceSeqMinRows = 32768; // below this the warp-per-row kernel has the lower latency
 
 // ------------------------------------------------------------------------------------------
 // step 5.  One warp per leaf row.  With S_0 = 0 and S_r = w_1 + .. + w_r (fp64 sums of the fp32
@@ -22,9 +27,11 @@ __global__ void __launch_bounds__(256) k_price_rows(const float *__restrict__ w,
                                                     const int32_t *__restrict__ row_bl_ptr, int32_t n_rows,
                                                     double *__restrict__ vstar, int32_t *__restrict__ left,
                                                     int32_t *__restrict__ right,
-                                                    double *__restrict__ row_absmax) {
+                                                    double *__restrict__ row_absmax,
+                                                    const int32_t *__restrict__ maxlen_flag) {
   const int lane = threadIdx.x & 31;
   const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (maxlen_flag && *maxlen_flag <= kPriceSeqMaxLen) return;     // the thread-per-row kernel takes this launch
   if (row >= n_rows) return;
   const int32_t b0 = row_bl_ptr[row];
   const int32_t n = row_bl_ptr[row + 1] - b0;
@@ -88,6 +95,58 @@ __global__ void __launch_bounds__(256) k_price_rows(const float *__restrict__ w,
     right[row] = best_r;
     row_absmax[row] = amax;
   }
+}
+
+// ------------------------------------------------------------------------------------------
+// step 5 for MANY leaf rows (the 10^4-10^5-row end of BASELINE.json configs[3]): thread per row, which is the
+// paper's own launch shape, but fed through shared memory: a warp copies the beamlets of its 32
+// consecutive rows (one contiguous slice of w) with coalesced loads, then every lane runs the printed scan
+// over its own row sequentially in fp64 -- literally the oracle's loop, strict comparisons
+// included, so ties and sums agree bit for bit.  The warp-per-row kernel above stays in use for few rows
+// (lower latency) and for rows too long for the staging buffer.
+// ------------------------------------------------------------------------------------------
+constexpr int kPriceStageFloats = 33 * kPriceSeqMaxLen;    // per warp: 32 rows of up to 88 beamlets + 1 word of skew per 32 (46.5 KB static per CTA) (+ skew against bank conflicts)
+__global__ void __launch_bounds__(128) k_price_rows_seq(const float *__restrict__ w,
+                                                        const int32_t *__restrict__ row_bl_ptr, int32_t n_rows,
+                                                        double *__restrict__ vstar, int32_t *__restrict__ left,
+                                                        int32_t *__restrict__ right, double *__restrict__ row_absmax,
+                                                        const int32_t *__restrict__ maxlen_flag) {
+  __shared__ float stage[4][kPriceStageFloats];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (maxlen_flag && *maxlen_flag > kPriceSeqMaxLen) return;      // rows too long: the warp-per-row kernel runs
+  const int row0 = (blockIdx.x * 4 + warp) * 32;
+  if (row0 >= n_rows) return;
+  const int rows = min(32, n_rows - row0);
+  const int32_t b0 = row_bl_ptr[row0], b1 = row_bl_ptr[row0 + rows];
+  float *buf = stage[warp];
+  // element e of the slice goes to buf[e + e / 32]: consecutive rows start 1 word further apart than their
+  // length, which spreads the lanes' sequential reads over the banks for the usual equal-length rows
+  for (int32_t e = lane; e < b1 - b0; e += 32) buf[e + (e >> 5)] = w[b0 + e];
+  __syncwarp();
+  if (lane >= rows) return;
+  const int row = row0 + lane;
+  const int32_t s0 = row_bl_ptr[row] - b0, n = row_bl_ptr[row + 1] - row_bl_ptr[row];
+  double v = 0.0, vbar = 0.0, best = 0.0, amax = 0.0;
+  int32_t l = 0, bl = 0, br = 0;
+  for (int32_t i = 0; i < n; ++i) {
+    const int32_t e = s0 + i;
+    const double wv = (double)buf[e + (e >> 5)];
+    amax = fmax(amax, fabs(wv));
+    v += wv;
+    if (v > vbar) { vbar = v; l = i + 1; }            // :163
+    if (v - vbar < best) { best = v - vbar; bl = l; br = i + 1; }   // :165
+  }
+  vstar[row] = best; left[row] = bl; right[row] = br; row_absmax[row] = amax;
+}
+
+// longest leaf row of device-resident MLC tables (the caller's, in dao_price_from_w)
+__global__ void k_price_maxlen(const int32_t *__restrict__ row_bl_ptr, int32_t n_rows, int32_t *__restrict__ out) {
+  int m = 0;
+  for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < n_rows; r += gridDim.x * blockDim.x)
+    m = max(m, row_bl_ptr[r + 1] - row_bl_ptr[r]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
 }
 
 // step 6a: price_b = sum over the rows of beam b of v* (PAPER.md:169).  One warp per beam,
@@ -412,7 +471,7 @@ size_t chain_pricing_smem(int32_t max_rows, int32_t width) {
 cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, const int32_t *beam_row_ptr,
                            int32_t n_rows, int32_t n_beams, int32_t *left, int32_t *right, double *vstar,
                            double *row_absmax, double *beam_price, double *beam_absmax, int32_t *best_out,
-                           bool update_state) {
+                           bool update_state, int32_t max_row_len) {
   const int wpb = 8;
   if (c->opt.mlc_mode == DAO_MLC_JAWS_ONLY) {
     // the context's own MLC tables only (dao_price_from_w refuses caller tables in this mode)
@@ -433,9 +492,26 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   } else {
-    if (n_rows > 0) {
+    // max_row_len > 0: known on the host (the context's own tables); < 0: caller tables, decided on the device
+    const bool seq_possible = n_rows >= kPriceSeqMinRows && max_row_len != 0;
+    const int32_t *flag = nullptr;
+    if (seq_possible && max_row_len < 0) {
+      int32_t *f = &c->d.state->price_maxlen;
+      cudaError_t e = cudaMemsetAsync(f, 0, sizeof(int32_t), c->stream);
+      if (e != cudaSuccess) return e;
+      k_price_maxlen<<<std::min((n_rows + 255) / 256, c->n_sm * 4), 256, 0, c->stream>>>(row_bl_ptr, n_rows, f);
+      e = cudaGetLastError();
+      if (e != cudaSuccess) return e;
+      flag = f;
+    }
+    if (seq_possible && (flag || max_row_len <= kPriceSeqMaxLen)) {
+      k_price_rows_seq<<<(n_rows + 127) / 128, 128, 0, c->stream>>>(w, row_bl_ptr, n_rows, vstar, left, right, row_absmax, flag);
+      cudaError_t e = cudaGetLastError();
+      if (e != cudaSuccess) return e;
+    }
+    if (n_rows > 0 && (!seq_possible || flag || max_row_len > kPriceSeqMaxLen)) {
       k_price_rows<<<(n_rows + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(w, row_bl_ptr, n_rows, vstar, left,
-                                                                        right, row_absmax);
+                                                                        right, row_absmax, flag);
       cudaError_t e = cudaGetLastError();
       if (e != cudaSuccess) return e;
     }

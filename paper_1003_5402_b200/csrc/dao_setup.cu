@@ -567,6 +567,8 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   c->row_col0.assign((size_t)dm.n_rows, 0);
   if (mlc->row_col0) c->row_col0.assign(mlc->row_col0, mlc->row_col0 + dm.n_rows);
   c->max_beam_width = 0;
+  c->max_row_len = 0;
+  for (int r = 0; r < dm.n_rows; ++r) c->max_row_len = std::max(c->max_row_len, c->row_bl_ptr[r + 1] - c->row_bl_ptr[r]);
   for (int r = 0; r < dm.n_rows; ++r)
     c->max_beam_width = std::max(c->max_beam_width, c->row_col0[r] + (c->row_bl_ptr[r + 1] - c->row_bl_ptr[r]));
   if (c->opt.mlc_mode == DAO_MLC_JAWS_ONLY &&

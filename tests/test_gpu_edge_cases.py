@@ -120,3 +120,32 @@ def test_pricing_row_lengths_around_the_warp_tiles(D, mini, row_len):
     pr = orc.price(wi.astype(np.float64), brp, rbp)
     assert np.array_equal(le, pr.left) and np.array_equal(ri, pr.right) and np.array_equal(vs, pr.vstar)
     assert best[0] == pr.best_beam
+
+
+@pytest.mark.parametrize("n_rows,row_len", [(32768, 20), (40000, 80), (33001, 88), (33000, 89), (20000, 33)])
+def test_pricing_many_rows_thread_per_row_kernel(D, n_rows, row_len):
+    """>= 32768 rows of <= 88 beamlets take the thread-per-row kernel (the paper's launch shape, PAPER.md:169);
+    longer rows fall back to warp-per-row, decided on the device for caller-provided tables.  Bit-exact on
+    integer-valued w (ties), band rule on random w."""
+    w, brp, rbp = phantom.pricing_rows(n_rows, row_len, rows_per_beam=40, seed=n_rows % 7)
+    wi = np.round(w * 2).astype(np.float32)
+
+    class Host:            # any context whose scratch (>= n_vox entries) holds the caller's tables
+        n_vox, n_bl, n_beams, n_rows = 50000, 4, 1, 1
+        row_ptr = np.arange(50001, dtype=np.int32); col_idx = (np.arange(50000) % 4).astype(np.int32)
+        val = np.ones(50000, np.float32); nnz = 50000
+        beam_row_ptr = np.array([0, 1], np.int32); row_bl_ptr = np.array([0, 4], np.int32)
+        vox_struct = np.zeros(50000, np.int32)
+        t_under = np.array([1.0], np.float32); w_under = np.array([10.0], np.float32)
+        t_over = np.array([1.05], np.float32); w_over = np.array([5.0], np.float32)
+        prescription = 1.0
+    with D.Dao(Host()) as d:
+        le, ri, vs, bp, best = (t.cpu().numpy() for t in d.price_from_w(_dev(w), _dev(rbp), _dev(brp)))
+        li, rii, vi, bpi, besti = (t.cpu().numpy() for t in d.price_from_w(_dev(wi), _dev(rbp), _dev(brp)))
+    pr = orc.price(w.astype(np.float64), brp, rbp)
+    assert np.abs(vs - pr.vstar).max() <= 1e-6 * max(1.0, np.abs(pr.vstar).max())
+    assert (le == pr.left).mean() >= 0.999 and (ri == pr.right).mean() >= 0.999
+    pu.check_beam(bp, best[0], pr.beam_price)
+    pi = orc.price(wi.astype(np.float64), brp, rbp)
+    assert np.array_equal(li, pi.left) and np.array_equal(rii, pi.right) and np.array_equal(vi, pi.vstar)
+    assert besti[0] == pi.best_beam
