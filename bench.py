@@ -251,6 +251,44 @@ def run_sweep(args):
                       f"{1e6 * tw:.1f} | {same}/{n_rows} | {'same' if int(best[0]) == pr.best_beam else 'differs'} |", flush=True)
 
 
+def run_widened(args):
+    """Measurements of the SURVEY 8(f) rows built beyond the paper's experiments, on the bench workload: the FMO
+    workload (8f-2), the re-optimisation mode (8f-1) and the alternative MLC rules (8f-4).  Markdown table."""
+    import torch
+    from paper_1003_5402_b200 import build, dao
+    from paper_1003_5402_b200.inputs import phantom
+    build.build()
+    peak, peak_src = load_peaks()
+    ph = phantom.make(args.config, 0)
+    print(f"workload {args.config}: {ph.name}, V={ph.n_vox}, N={ph.n_bl}, nnz={ph.nnz}; HBM peak {peak:.0f} GB/s ({peak_src})\n")
+    print("| row | what | result |")
+    print("|---|---|---|")
+    with dao.Dao(ph, k_max=N_APERTURES) as d:
+        d.fmo_solve(max_iter=50)
+        f = d.fmo_solve(max_iter=1000, tol=1e-9)
+        per_it = f.seconds / max(1, f.n_iter)
+        moved = 3 * 8 * ph.nnz                      # dose SpMV + SpMV^T + dz SpMV per iteration
+        print(f"| 8f-2 FMO | {f.n_iter} projected-gradient iterations from x = 0 | {f.seconds:.3f} s, {1e6 * per_it:.0f} us per iteration "
+              f"(3 SpMV-class passes = {moved / per_it * 1e-9:.0f} GB/s, {moved / per_it * 1e-9 / peak:.2f} of peak), F = {f.objective:.6g}, "
+              f"{f.n_ls_evals} line-search evaluations |")
+    modes = [("consecutive (the paper's experiments)", dao.MLC_CONSECUTIVE), ("8f-4 jaws-only", dao.MLC_JAWS_ONLY),
+             ("8f-4 interdigitation", dao.MLC_INTERDIGITATION), ("8f-4 connectedness", dao.MLC_CONNECTED)]
+    for name, code in modes:
+        with dao.Dao(ph, k_max=N_APERTURES, mlc_mode=code) as d:
+            d.run(N_APERTURES); d.reset()
+            i = d.run(N_APERTURES)
+        n = max(1, i.n_iterations)
+        print(f"| {name} | {i.n_apertures}-aperture plan | {i.seconds_total:.4f} s, pricing {1e6 * i.seconds_price / n:.1f} us per iteration, "
+              f"master {1e6 * i.seconds_master / n:.0f} us, F = {i.objective:.6g}, {i.n_pg_iter_total} projected-gradient iterations |")
+    pr = phantom.make(args.config + "_reopt", 0)
+    with dao.Dao(pr, k_max=N_APERTURES) as d:
+        d.run(N_APERTURES); d.reset()
+        i = d.run(N_APERTURES)
+    n = max(1, i.n_iterations)
+    print(f"| 8f-1 re-optimisation (per-voxel T_j) | {i.n_apertures}-aperture plan | {i.seconds_total:.4f} s, dose SpMV {1e6 * i.seconds_spmv / n:.1f} us, "
+          f"master {1e6 * i.seconds_master / n:.0f} us per iteration, F = {i.objective:.6g}, {i.n_pg_iter_total} projected-gradient iterations |")
+
+
 def main():
     global N_APERTURES, METRIC
     ap = argparse.ArgumentParser()
@@ -264,6 +302,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[3] kernel sweep (markdown table)")
+    ap.add_argument("--widened", action="store_true", help="measure the SURVEY 8(f) rows (FMO, re-optimisation, MLC modes)")
     ap.add_argument("--sweep-reps", type=int, default=15)
     ap.add_argument("--sweep-only", default="", help="comma-separated subset of the sweep matrices")
     args = ap.parse_args()
@@ -278,6 +317,10 @@ def main():
     if args.sweep:
         if rank == 0:
             run_sweep(args)
+        return
+    if args.widened:
+        if rank == 0:
+            run_widened(args)
         return
     args.warmup = max(args.warmup, 3)
 

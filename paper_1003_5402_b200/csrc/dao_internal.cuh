@@ -145,6 +145,7 @@ struct DevPtrs {
   int32_t *bl_row;         // [n_bl]
   int32_t *row_beam;       // [n_rows]
   int32_t *row_col0;       // [n_rows] lateral position of the first beamlet of every row
+  int32_t *chain_from;     // [n_rows][(W+1)^2] back-pointers of the chain pricing modes (W = widest beam)
   // vectors
   float *x;                // [n_bl]
   float *xmask;            // [n_bl]

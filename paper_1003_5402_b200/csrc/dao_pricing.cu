@@ -260,9 +260,11 @@ __global__ void __launch_bounds__(256) k_price_jaws(const float *__restrict__ w,
 // the feasible apertures of a beam are chains over its leaf rows, so the best one is a shortest path through
 // the layered graph rows x leaf states (a, b) (lateral tip positions, 0 <= a <= b <= W; closed when a == b):
 //   f_m(s) = val_m(s) + min { f_{m-1}(s') : s' compatible with s }.
-// One CTA per beam; the row prefix sums, two layers of f and the back-pointers live in shared memory; a thread
-// owns states s = t, t + 256, ... of the current row and scans the previous layer in state order with strict
-// comparisons, which reproduces the oracle's choice among equal minima.  Thread 0 walks the back-pointers.
+// One CTA per beam; the row prefix sums and two layers of f live in shared memory, the back-pointers in the
+// workspace.  Both compatibility rules are dominance conditions (a' <= x, b' >= y), so the inner minimum is a
+// 2-D prefix minimum of the previous layer: two sweeps of O(W^2) per row instead of O(W^4) comparisons, with the
+// key (value, state index), which reproduces the oracle's choice (first minimiser in state order) among equal
+// minima.  Thread 0 walks the back-pointers.
 //   J2: a_m <= b_{m+1} and a_{m+1} <= b_m for adjacent rows (a closed pair may park anywhere in [0, W]);
 //   J3: the open rows are consecutive and adjacent open intervals share a lateral position.
 // An open row stays inside its own beamlets.
@@ -271,18 +273,17 @@ __global__ void __launch_bounds__(256) k_price_chain(int32_t mode, const float *
                                                      const int32_t *__restrict__ beam_row_ptr,
                                                      const int32_t *__restrict__ row_bl_ptr,
                                                      const int32_t *__restrict__ row_col0, int32_t width, int32_t max_rows,
+                                                     int32_t *__restrict__ from_g /* [n_rows][(width+1)^2] */,
                                                      double *__restrict__ vstar, int32_t *__restrict__ left,
                                                      int32_t *__restrict__ right, double *__restrict__ beam_price,
                                                      double *__restrict__ beam_absmax) {
   extern __shared__ double sm_d[];
-  const int ld = width + 1;
-  const int S = (width + 1) * (width + 2) / 2;
-  double *P = sm_d;                                         // [max_rows][ld]
-  double *f0 = P + (size_t)max_rows * ld;                   // [S]
-  double *f1 = f0 + S;                                      // [S]
-  int16_t *sa = reinterpret_cast<int16_t *>(f1 + S);        // [S]
-  int16_t *sb = sa + S;                                     // [S]
-  int16_t *from = sb + S;                                   // [max_rows][S]
+  const int ld = width + 1, S = ld * ld;                    // state (a, b) has index a * ld + b (valid when a <= b)
+  double *P = sm_d;                                         // [max_rows][ld] row prefix sums over lateral positions
+  double *fp = P + (size_t)max_rows * ld;                   // [S] previous layer (inf = infeasible)
+  double *fc = fp + S;                                      // [S] current layer
+  double *G = fc + S;                                       // [S] G[x][y] = min { f_prev(a', b') : a' <= x, b' >= y }
+  int32_t *Garg = reinterpret_cast<int32_t *>(G + S);       // [S] its first minimiser in state order
   __shared__ double s_val[256];
   __shared__ int32_t s_m[256], s_s[256];
   __shared__ double s_abs[256];
@@ -302,43 +303,66 @@ __global__ void __launch_bounds__(256) k_price_chain(int32_t mode, const float *
       P[m * ld + c + 1] = s;
     }
   }
-  for (int a = t; a <= width; a += 256) {                   // states in the order a, then b
-    int k = a * (width + 1) - a * (a - 1) / 2;
-    for (int bb = a; bb <= width; ++bb, ++k) { sa[k] = (int16_t)a; sb[k] = (int16_t)bb; }
-  }
   __syncthreads();
-  double best = CUDART_INF;                                 // J3: best end of an open run seen by this thread
+  double best = (mode == 3) ? 0.0 : CUDART_INF;            // J3: best end of an open run seen by this thread
   int32_t best_m = -1, best_s = -1;
-  if (mode == 3) best = 0.0;
-  double *fp = f0, *fc = f1;
   for (int m = 0; m < R; ++m) {
     const int32_t r = r0 + m, c0 = row_col0 ? row_col0[r] : 0, n = row_bl_ptr[r + 1] - row_bl_ptr[r];
+    if (m > 0) {
+      // 2-D prefix minimum of the previous layer with the key (value, state index): first along a' ...
+      for (int y = t; y < ld; y += 256) {
+        double v = CUDART_INF;
+        int32_t arg = -1;
+        for (int x = 0; x < ld; ++x) {
+          const double f = fp[x * ld + y];
+          if (f < v) { v = f; arg = x * ld + y; }           // ascending a': ties keep the smaller index
+          G[x * ld + y] = v;
+          Garg[x * ld + y] = arg;
+        }
+      }
+      __syncthreads();
+      // ... then along b' (descending), comparing indices on ties
+      for (int x = t; x < ld; x += 256) {
+        double v = CUDART_INF;
+        int32_t arg = -1;
+        for (int y = ld - 1; y >= 0; --y) {
+          const double f = G[x * ld + y];
+          const int32_t fa = Garg[x * ld + y];
+          if (fa >= 0 && (f < v || (f == v && fa < arg))) { v = f; arg = fa; }
+          G[x * ld + y] = v;
+          Garg[x * ld + y] = arg;
+        }
+      }
+      __syncthreads();
+    }
+    int32_t *from = from_g + (size_t)(r0 + m) * S;
     for (int s = t; s < S; s += 256) {
-      const int a = sa[s], bb = sb[s];
+      const int a = s / ld, bb = s - a * ld;
       double out = CUDART_INF;
-      int arg = -1;
+      int32_t arg = -1;
       const bool open = a < bb;
-      const bool valid = open ? (a >= c0 && bb <= c0 + n) : (mode != 3);
+      const bool valid = a <= bb && (open ? (a >= c0 && bb <= c0 + n) : (mode != 3));
       if (valid) {
         const double val = open ? P[m * ld + bb] - P[m * ld + a] : 0.0;
         double prev = 0.0;
+        bool ok = true;
         if (m > 0) {
-          prev = (mode == 3) ? 0.0 : CUDART_INF;            // J3: the run may start at this row
-          for (int q = 0; q < S; ++q) {
-            const double fq = fp[q];
-            if (fq == CUDART_INF) continue;
-            const int a0 = sa[q], b0 = sb[q];
-            const bool ok = (mode == 2) ? (a0 <= bb && a <= b0) : (max(a0, a) < min(b0, bb));
-            if (ok && fq < prev) { prev = fq; arg = q; }
+          if (mode == 2) {                                  // a' <= b and b' >= a
+            prev = G[bb * ld + a];
+            arg = Garg[bb * ld + a];
+            ok = arg >= 0;
+          } else {                                          // overlap: a' <= b - 1 and b' >= a + 1; or start the run here
+            const double gv = G[(bb - 1) * ld + (a + 1)];
+            if (gv < 0.0) { prev = gv; arg = Garg[(bb - 1) * ld + (a + 1)]; }
           }
         }
-        if (prev != CUDART_INF) {
+        if (ok) {
           out = val + prev;
           if (mode == 3 && out < best) { best = out; best_m = m; best_s = s; }
         }
       }
       fc[s] = out;
-      from[(size_t)m * S + s] = (int16_t)arg;
+      from[s] = arg;
     }
     __syncthreads();
     double *tmp = fp; fp = fc; fc = tmp;
@@ -363,18 +387,20 @@ __global__ void __launch_bounds__(256) k_price_chain(int32_t mode, const float *
     __syncthreads();
   }
   for (int m = t; m < R; m += 256) { left[r0 + m] = 0; right[r0 + m] = 0; vstar[r0 + m] = 0.0; }
+  __threadfence_block();
   __syncthreads();
   if (t == 0) {
     double price = s_val[0];
     int m = s_m[0], s = s_s[0];
     if (s < 0) { price = 0.0; m = -1; }                     // nothing improves: closed aperture
-    for (; m >= 0 && s >= 0; s = from[(size_t)m * S + s], --m) {
-      const int a = sa[s], bb = sb[s];
+    for (; m >= 0 && s >= 0; --m) {
+      const int a = s / ld, bb = s - a * ld;
       if (a < bb) {
         const int32_t r = r0 + m, c0 = row_col0 ? row_col0[r] : 0;
         left[r] = a - c0; right[r] = bb - c0;
         vstar[r] = P[m * ld + bb] - P[m * ld + a];
       }
+      s = from_g[(size_t)(r0 + m) * S + s];
     }
     beam_price[b] = price;
     beam_absmax[b] = s_abs[0];
@@ -464,8 +490,8 @@ __global__ void __launch_bounds__(256) k_price_select(const double *__restrict__
 }
 
 size_t chain_pricing_smem(int32_t max_rows, int32_t width) {
-  const size_t S = (size_t)(width + 1) * (size_t)(width + 2) / 2;
-  return align_up((size_t)max_rows * (size_t)(width + 1) * 8 + 2 * S * 8 + 2 * S * 2 + (size_t)max_rows * S * 2, 16);
+  const size_t S = (size_t)(width + 1) * (size_t)(width + 1);
+  return align_up((size_t)max_rows * (size_t)(width + 1) * 8 + 3 * S * 8 + S * 4, 16);
 }
 
 cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, const int32_t *beam_row_ptr,
@@ -487,7 +513,7 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
     cudaError_t e = cudaFuncSetAttribute(k_price_chain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k_price_chain<<<n_beams, 256, smem, c->stream>>>(c->opt.mlc_mode, w, beam_row_ptr, row_bl_ptr, c->d.row_col0,
-                                                     c->max_beam_width, c->max_rows_per_beam, vstar, left, right,
+                                                     c->max_beam_width, c->max_rows_per_beam, c->d.chain_from, vstar, left, right,
                                                      beam_price, beam_absmax);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;

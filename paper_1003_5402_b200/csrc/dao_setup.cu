@@ -92,6 +92,7 @@ struct Carver {
 
 struct Dims {
   int32_t n_vox, n_bl, n_beams, n_rows, k_max, max_rows;
+  int32_t chain_states;        // (W+1)^2 leaf states per row of the chain pricing modes, 0 otherwise
   int64_t nnz;
 };
 
@@ -119,6 +120,7 @@ static void carve_workspace(Carver &cv, const Dims &dm, const HostLayout &L, Dev
   d->bl_row = cv.take<int32_t>((size_t)dm.n_bl);
   d->row_beam = cv.take<int32_t>((size_t)dm.n_rows);
   d->row_col0 = cv.take<int32_t>((size_t)dm.n_rows);
+  d->chain_from = cv.take<int32_t>((size_t)dm.n_rows * (size_t)dm.chain_states + 4);
   d->x = cv.take<float>((size_t)dm.n_bl);
   d->xmask = cv.take<float>((size_t)dm.n_bl);
   d->z = cv.take<float>(vp);
@@ -242,6 +244,14 @@ static dao_status check_args(const dao_csr *D, const dao_mlc *mlc, const dao_str
   dm->n_vox = D->n_vox; dm->n_bl = D->n_bl; dm->nnz = D->nnz;
   dm->n_beams = mlc->n_beams; dm->n_rows = mlc->n_rows; dm->k_max = opt->k_max;
   dm->max_rows = std::max(max_rows, 1);
+  dm->chain_states = 0;
+  if (opt->mlc_mode == DAO_MLC_INTERDIGITATION || opt->mlc_mode == DAO_MLC_CONNECTED) {
+    int32_t width = 0;
+    for (int r = 0; r < mlc->n_rows; ++r)
+      width = std::max(width, (mlc->row_col0 ? mlc->row_col0[r] : 0) + (mlc->row_bl_ptr[r + 1] - mlc->row_bl_ptr[r]));
+    if (width > 1000) { *err = "interdigitation / connectedness pricing: beam wider than 1000 beamlets"; return DAO_E_UNSUPPORTED; }
+    dm->chain_states = (width + 1) * (width + 1);
+  }
   return DAO_OK;
 }
 
