@@ -149,10 +149,11 @@ def test_cfg1_plan_50_apertures(D, cfg1):
           f"pg iterations {info.n_pg_iter_total} kkt gap {gap:.2e}")
 
 
-@pytest.mark.parametrize("config,n_ap", [("cfg2", 50), ("cfg4", 100)])
+@pytest.mark.parametrize("config,n_ap", [("cfg2", 50), ("cfg4", 100), ("cfg1_reopt", 50)])
 def test_other_full_size_configs(D, config, n_ap):
-    """BASELINE.json configs[2] (5-field head-and-neck shape, 50 apertures) and configs[4] (7-field stress
-    case at 2 mm voxels, 100 apertures) at full size: kernels element by element, then the free-running
+    """BASELINE.json configs[2] (5-field head-and-neck shape, 50 apertures), configs[4] (7-field stress
+    case at 2 mm voxels, 100 apertures) and configs[1] posed as the re-optimisation problem (PAPER.md:254:
+    per-voxel reference dose T_j, alpha_j = beta_j = 1) at full size: kernels element by element, then the free-running
     plan checked by the oracle at the GPU's plan (dose, objective, master optimality).  Prints the
     per-kernel-class time split configs[4] asks for."""
     ph = phantom.make(config, seed=0)
