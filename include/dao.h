@@ -121,7 +121,7 @@ typedef struct {
 /* Options.  Zero-initialise, then dao_default_options, then override. */
 typedef struct {
   int32_t k_max;             /* capacity of the aperture pool, 1..DAO_MAX_APERTURES (default 50) */
-  int32_t master_max_iter;   /* cap on projected-gradient iterations per master solve (default 2000) */
+  int32_t master_max_iter;   /* cap on projected-gradient / Newton iterations per master solve (default 2000) */
   double master_tol;         /* stop when max_k |p_k| * max(1, max_k y_k) <= master_tol * F, p = projected
                                 steepest-descent direction (default 1e-7); reading S2 */
   double price_tol;          /* optimal iff price_b* >= -price_tol * max_i |w_i| * (rows in b*) (default 1e-6, the
@@ -131,7 +131,10 @@ typedef struct {
                                 |phi'(0)| (phi(t) = F(z + t dz)) or when it ends on a bound still descending;
                                 otherwise t is refined by a safeguarded Newton search (default 0.01); S2 */
   int32_t master_method;     /* 0 = plain gradient projection, 1 = gradient projection with conjugate
-                                (Polak-Ribiere+) directions on the free face (default 1) */
+                                (Polak-Ribiere+) directions on the free face, 2 = projected Newton on the free
+                                variables (exact Hessian A^T diag(2c) A of the piecewise-quadratic F on the fp64
+                                tensor cores, one pass over A per iteration; default 2).  Same stopping test
+                                and the same (unique) optimal value for all three; reading S2 */
   int32_t sell_sigma;        /* sorting window (rows) of the internal sliced-ELL layout of D; 1 = keep the
                                 caller's voxel order; 0 = library default */
   int32_t timers;            /* non-zero: CUDA-event timers per kernel class in dao_run (default 1) */
@@ -159,12 +162,14 @@ typedef struct {
 
 typedef struct {
   int32_t n_apertures;       /* pool size after the call */
-  int32_t n_pg_iter;         /* projected-gradient iterations taken */
+  int32_t n_pg_iter;         /* projected-gradient (methods 0, 1) or Newton (method 2) iterations taken */
   int32_t hit_max_iter;      /* 1: stopped by master_max_iter */
   int32_t n_restarts;        /* conjugate-direction restarts (method 1) */
   double objective;          /* F(A y) at return */
   double kkt_residual;       /* max_k of |grad_k| where y_k > 0 and max(0, -grad_k) where y_k = 0 */
   double pg_norm;            /* max_k |p_k| at return */
+  int32_t n_passes;          /* passes over the aperture-dose block A (4 V K bytes each) */
+  int32_t reserved;
 } dao_master_info;
 
 typedef struct {
@@ -177,6 +182,9 @@ typedef struct {
   double seconds_total;      /* device time of the call (CUDA events) */
   /* per kernel class, summed over iterations; zero when options.timers == 0 */
   double seconds_intensity, seconds_spmv, seconds_spmv_t, seconds_price, seconds_column, seconds_master;
+  int64_t n_passes_total;    /* passes over the aperture-dose block A made by the master solves of this call */
+  int32_t n_hit_max_iter;    /* master solves of this call that stopped on master_max_iter */
+  int32_t reserved;
 } dao_run_info;
 
 /* One record per column-generation iteration, retrievable after dao_run / dao_solve_master. */
@@ -189,6 +197,8 @@ typedef struct {
   double objective_before;   /* F before the aperture was added (at pricing time) */
   double objective;          /* F(A y) after the master solve */
   double kkt_residual;
+  int32_t n_passes;          /* passes over the aperture-dose block A made by the master solve (4 V K bytes each) */
+  int32_t hit_max_iter;      /* 1: that master solve stopped on master_max_iter (or could not make progress) */
 } dao_iter_record;
 
 typedef struct {

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libdao.so")
-SOURCES = ["dao_api.cu", "dao_setup.cu", "dao_spmv.cu", "dao_spmvt.cu", "dao_pricing.cu", "dao_master.cu", "dao_fmo.cu"]
+SOURCES = ["dao_api.cu", "dao_setup.cu", "dao_spmv.cu", "dao_spmvt.cu", "dao_pricing.cu", "dao_master.cu", "dao_newton.cu", "dao_fmo.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC]

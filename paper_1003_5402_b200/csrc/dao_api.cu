@@ -101,7 +101,7 @@ void dao_default_options(dao_options *opt) {
   opt->master_max_iter = 2000;
   opt->master_tol = 1e-7;
   opt->price_tol = 1e-6;
-  opt->master_method = 1;
+  opt->master_method = 2;
   opt->master_ls_tol = 0.01;
   opt->sell_sigma = 0;
   opt->timers = 1;
@@ -215,6 +215,8 @@ static void fill_master_info(const Ctx *c, dao_master_info *out) {
   out->objective = h.m_F;
   out->kkt_residual = h.m_kkt;
   out->pg_norm = h.m_pg;
+  out->n_passes = h.m_passes;
+  out->reserved = 0;
 }
 
 dao_status dao_solve_master(dao_ctx *ctx, dao_master_info *out) {
@@ -258,6 +260,8 @@ dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out) {
   if (st != DAO_OK) return st;
   const int64_t pg0 = c->h_state->pg_iter_total;
   const int32_t dup0 = c->h_state->n_duplicates;
+  const int64_t pass0 = c->h_state->pass_total;
+  const int32_t hit0 = c->h_state->n_hit_max;
   double acc[6] = {0, 0, 0, 0, 0, 0};
   while (c->K < max_apertures) {
     if (timers) API_CUDA(cudaEventRecord(c->ev[0], c->stream));
@@ -303,6 +307,8 @@ dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out) {
   info.n_apertures = c->K;
   info.n_duplicates = c->h_state->n_duplicates - dup0;
   info.n_pg_iter_total = c->h_state->pg_iter_total - pg0;
+  info.n_passes_total = c->h_state->pass_total - pass0;
+  info.n_hit_max_iter = c->h_state->n_hit_max - hit0;
   info.objective = c->h_state->F;
   info.seconds_total = ms * 1e-3;
   info.seconds_intensity = acc[0]; info.seconds_spmv = acc[1]; info.seconds_spmv_t = acc[2];
@@ -473,7 +479,7 @@ dao_status dao_set_pool(dao_ctx *ctx, int32_t n_apertures, const int32_t *beam, 
                                                             c->d.row_bl_ptr, c->d.ap_beam, c->d.ap_left, c->d.ap_right,
                                                             c->d.xmask);
     API_CUDA(cudaGetLastError());
-    API_CUDA(launch_spmv(c, kSpmvPlain, c->d.xmask, c->d.A + (size_t)k * c->n_vox_pad));
+    API_CUDA(launch_spmv(c, kSpmvColumn, c->d.xmask, c->d.A, nullptr, k));
   }
   API_CUDA(cudaStreamSynchronize(c->stream));   // le/ri/yy are stack-owned
   c->K = K;

@@ -47,7 +47,23 @@ constexpr int kMasterProfSlots = 16;   // phase timers of the master (ns): 0 ini
 constexpr int kFmoLsGridMax = 1024;   // CTAs of the FMO line-search kernels
 constexpr int kMaxStruct = 255;
 constexpr int kNoStruct = 255;         // sid value of a voxel without penalty
-constexpr int kMaxRedux = DAO_MAX_APERTURES + 8;   // doubles per grid reduction in the master
+constexpr int kMaxRedux = DAO_MAX_APERTURES + 8;   // doubles per grid reduction in the master (methods 0, 1)
+
+// ---- master_method = 2 (projected Newton, dao_newton.cu) ----
+// The aperture-dose block is stored TILED: tile t (T internal voxels) holds its k_max columns back to
+// back, each padded to TP = T + 4 floats (TP = 4 mod 32: conflict-free tensor-core fragment loads), so
+// the K live columns of a tile are ONE contiguous range = one bulk copy.
+struct NewtonLayout {
+  int32_t T = 0;            // voxels per tile (0: plain aperture-major layout, methods 0 and 1)
+  int32_t TP = 0;           // floats per column inside a tile
+  int32_t n_tiles = 0;      // ceil(n_vox_pad / T)
+  int64_t tile_stride = 0;  // floats between consecutive tiles = k_max * TP
+  int32_t n_stages = 0;     // ring stages of stage_bytes
+  int32_t stage_bytes = 0;  // k_max * TP * 4 rounded to 128
+  int32_t nb_max = 0;       // 8x8 block rows of the augmented Hessian at K = k_max: ceil((k_max + 1) / 8)
+  int32_t n_red = 0;        // doubles per grid reduction: nb_max (nb_max + 1) / 2 * 64 + 8
+  size_t smem = 0;          // dynamic shared memory of k_master_newton
+};
 
 // ------------------------------------------------------------------------------------------
 // Device-resident state shared by the kernels of one context (one instance in global memory).
@@ -81,6 +97,9 @@ struct DevState {
   uint32_t bar_count;
   uint32_t bar_gen;
   int64_t pg_iter_total;
+  int64_t pass_total;      // passes over the aperture-dose block A (each reads 4 V K bytes) since dao_create / dao_reset
+  int32_t m_passes;        // passes over A of the last master solve
+  int32_t n_hit_max;       // master solves that stopped on the iteration cap since dao_create / dao_reset
   int32_t n_duplicates;
   int32_t price_maxlen;    // longest leaf row of caller-provided MLC tables (dao_price_from_w), decided on the device
 };
@@ -203,6 +222,8 @@ struct Ctx {
   cudaStream_t stream = nullptr;
   int device = 0, n_sm = 0;
   int spmv_grid = 0, master_grid = 0;
+  int red_stride = kMaxRedux;   // slots per CTA of the grid reductions (ll_part)
+  NewtonLayout nwt{};           // master_method = 2
   size_t master_smem = 0;
   int master_slab = 0, master_stages = 0, master_z_in_smem = 0;
   bool x_in_smem = true;
@@ -242,8 +263,11 @@ dao_status setup_sizes(const dao_csr *D, const dao_mlc *mlc, const dao_structs *
 
 // dao_spmv.cu
 enum SpmvMode { kSpmvObjective = 0, kSpmvPlain = 1, kSpmvColumn = 2, kSpmvPlainUserOrder = 3 };
-// `skip` (device, may be null): when *skip != 0 the kernels return at once (device-side loop control)
-cudaError_t launch_spmv(Ctx *c, SpmvMode mode, const float *x, float *out, const int32_t *skip = nullptr);
+// `skip` (device, may be null): when *skip != 0 the kernels return at once (device-side loop control).
+// kSpmvColumn writes column `a_col` of the dose block A (a_col < 0: column K of the device state, only
+// when a candidate is pending), whatever its layout (a_index); `out` is ignored in that mode.
+cudaError_t launch_spmv(Ctx *c, SpmvMode mode, const float *x, float *out, const int32_t *skip = nullptr,
+                        int32_t a_col = -1);
 cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out, const int32_t *skip = nullptr);
 cudaError_t launch_intensity(Ctx *c);
 void spmv_configure(Ctx *c);
@@ -259,8 +283,21 @@ size_t chain_pricing_smem(int32_t max_rows, int32_t width);   // shared memory o
 // dao_fmo.cu
 dao_status fmo_solve(Ctx *c, int32_t max_iter, double tol, bool warm_start, dao_fmo_info *out);
 
-// dao_master.cu
+// dao_master.cu (methods 0, 1) -- both dispatch to dao_newton.cu when master_method = 2
 cudaError_t master_configure(Ctx *c);
 cudaError_t launch_master(Ctx *c, bool add_candidate);
+
+// dao_newton.cu (method 2)
+NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct);   // host only, no device query
+cudaError_t newton_configure(Ctx *c);
+cudaError_t launch_newton(Ctx *c, bool add_candidate);
+
+// Position of (internal voxel i, aperture column k) in the dose block A (floats)
+__host__ __device__ __forceinline__ size_t a_index(int32_t tile_T, int32_t tile_TP, int64_t tile_stride,
+                                                   int32_t n_vox_pad, int32_t i, int32_t k) {
+  if (tile_T == 0) return (size_t)k * (size_t)n_vox_pad + (size_t)i;
+  const int32_t t = i / tile_T;
+  return (size_t)t * (size_t)tile_stride + (size_t)k * (size_t)tile_TP + (size_t)(i - t * tile_T);
+}
 
 }  // namespace dao

@@ -22,6 +22,7 @@
 // here is DESIGN.md reading S2.
 #include "dao_internal.cuh"
 #include "dao_ptx.cuh"
+#include "dao_grid_reduce.cuh"
 
 #include <math_constants.h>
 
@@ -46,6 +47,7 @@ struct MasterParams {
   uint4 *ll_part;          // [2][grid][kMaxRedux] flagged slots
   uint4 *ll_result;        // [2][kMaxRedux]
   uint32_t *epoch;         // reduction counter, survives dao_reset
+  int32_t red_stride;      // slots per CTA in ll_part
   unsigned long long *prof;  // optional [kMasterProfSlots] phase timers (ns), CTA 0 only
   DevState *st;
   dao_iter_record *history;
@@ -56,110 +58,6 @@ struct MasterParams {
   int32_t k_max;
   double tol;
   double ls_tol;           // |phi'(t)| <= ls_tol * |phi'(0)| accepts a step
-};
-
-constexpr int kNW = kMasterWorkers / 32;  // worker warps
-
-// ---- small helpers ---------------------------------------------------------------------------
-__device__ __forceinline__ void wsync() { asm volatile("bar.sync 1, %0;" ::"n"(kMasterWorkers) : "memory"); }
-
-__device__ __forceinline__ double warp_max_d(double v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-  return v;
-}
-__device__ __forceinline__ double warp_min_d(double v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
-  return v;
-}
-__device__ __forceinline__ unsigned long long gtimer() {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-  return t;
-}
-
-// ---- flagged slots ---------------------------------------------------------------------------
-__device__ __forceinline__ void ll_store(uint4 *slot, double v, uint32_t ep) {
-  const unsigned long long u = (unsigned long long)__double_as_longlong(v);
-  asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(slot), "r"((uint32_t)u), "r"(ep),
-               "r"((uint32_t)(u >> 32)), "r"(ep)
-               : "memory");
-}
-__device__ __forceinline__ uint4 ll_load(const uint4 *slot) {
-  uint4 w;
-  asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4];"
-               : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w)
-               : "l"(slot)
-               : "memory");
-  return w;
-}
-__device__ __forceinline__ double ll_value(const uint4 &w) {
-  return __longlong_as_double((long long)(((unsigned long long)w.z << 32) | (unsigned long long)w.x));
-}
-
-// One warp sums value `i` of every CTA's slot of this epoch: lane l takes the CTAs l, l+32, ...
-// in that order, then a shuffle tree (fixed order).  Every lane returns the total.
-// (A push variant -- every CTA stores into a private inbox of every reader -- was measured slower:
-// 3.8 us against 2.6 us for the small reduction on B200.)
-constexpr int kMaxGridOver32 = (kMasterMaxGrid + 31) / 32;
-__device__ __forceinline__ double ll_warp_gather(const uint4 *part /*[grid][kMaxRedux]*/, int i, uint32_t ep,
-                                                 int lane) {
-  const int grid = (int)gridDim.x;
-  uint4 w[kMaxGridOver32];
-#pragma unroll
-  for (int j = 0; j < kMaxGridOver32; ++j) {
-    const int b = lane + 32 * j;
-    if (b < grid) w[j] = ll_load(part + (size_t)b * kMaxRedux + i);
-  }
-  double s = 0.0;
-#pragma unroll
-  for (int j = 0; j < kMaxGridOver32; ++j) {
-    const int b = lane + 32 * j;
-    if (b < grid) {
-      while (w[j].y != ep || w[j].w != ep) w[j] = ll_load(part + (size_t)b * kMaxRedux + i);
-      s += ll_value(w[j]);
-    }
-  }
-  return warp_sum_f64(s);
-}
-
-struct Reducer {
-  uint4 *part;      // [2][grid][kMaxRedux]
-  uint4 *result;    // [2][kMaxRedux]
-  uint32_t ep;      // epoch of the last reduction
-
-  // n <= kNW values: every CTA reads every CTA's slot (one hop).  vals/out in shared memory.
-  __device__ __noinline__ void small(int n, const double *vals, double *out) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    ++ep;
-    uint4 *buf = part + (size_t)(ep & 1u) * gridDim.x * kMaxRedux;
-    if (tid < n) ll_store(buf + (size_t)blockIdx.x * kMaxRedux + tid, vals[tid], ep);
-    if (warp < n) {
-      const double s = ll_warp_gather(buf, warp, ep, lane);
-      if (lane == 0) out[warp] = s;
-    }
-    wsync();
-  }
-  // n <= kMaxRedux values: CTA i sums value i and publishes the total (two hops).
-  __device__ __noinline__ void large(int n, const double *vals, double *out) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    ++ep;
-    uint4 *buf = part + (size_t)(ep & 1u) * gridDim.x * kMaxRedux;
-    uint4 *res = result + (size_t)(ep & 1u) * kMaxRedux;
-    if (tid < n) ll_store(buf + (size_t)blockIdx.x * kMaxRedux + tid, vals[tid], ep);
-    // values this CTA owns: i = blockIdx.x + j * gridDim.x, one warp each
-    for (int i = (int)blockIdx.x + warp * (int)gridDim.x; i < n; i += kNW * (int)gridDim.x) {
-      const double s = ll_warp_gather(buf, i, ep, lane);
-      if (lane == 0) ll_store(res + i, s, ep);
-    }
-    if (tid < n) {
-      uint4 w = ll_load(res + tid);
-      while (w.y != ep || w.w != ep) w = ll_load(res + tid);
-      out[tid] = ll_value(w);
-    }
-    wsync();
-  }
 };
 
 // Block-wide sums of NV per-thread doubles -> vals[0..NV) (fixed order: shuffle tree, then warps in order)
@@ -313,29 +211,6 @@ __device__ __noinline__ void master_direction(int K, int iters, bool force_resta
 // ---- the A stream ----------------------------------------------------------------------------
 // Stage sequence of ONE pass: for tile (kMasterTileVox voxels of the slab) { for k < K { A[k][tile] } }.
 // The producer repeats that sequence for ever; consumers walk it with the same counters.
-struct RingPos {
-  int stage;
-  uint32_t phase;
-  __device__ __forceinline__ void advance(int n_stages) {
-    if (++stage == n_stages) { stage = 0; phase ^= 1u; }
-  }
-};
-
-__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
-  uint32_t ok;
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-      "selp.u32 %0, 1, 0, p;\n\t}"
-      : "=r"(ok)
-      : "r"(smem_addr(bar)), "r"(parity)
-      : "memory");
-  return ok != 0;
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
-}
-
 struct MasterSmem {          // carved from dynamic shared memory by every thread identically
   unsigned char *ring;       // [n_stages][kMasterStageBytes]
   uint64_t *full, *empty;    // [n_stages]
@@ -369,7 +244,7 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
   const int added = (p.add_candidate && cand) ? 1 : 0;
   const int K = K0 + added;
   if ((p.add_candidate && !added) || K == 0) {     // converged, pool full or empty pool: nothing to do
-    if (blockIdx.x == 0 && tid == 0) { p.st->m_added = 0; p.st->m_iters = 0; }
+    if (blockIdx.x == 0 && tid == 0) { p.st->m_added = 0; p.st->m_iters = 0; p.st->m_passes = 0; }
     return;
   }
 
@@ -476,7 +351,7 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
       if (vts) vts[j] = p.vt[i];
     }
   }
-  Reducer red{p.ll_part, p.ll_result, 0u};
+  Reducer red{p.ll_part, p.ll_result, 0u, p.red_stride};
   if (tid == 0) si[7] = (int)*p.epoch;
   wsync();
   red.ep = (uint32_t)si[7];
@@ -597,11 +472,13 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
   int iters = 0, restarts = 0, since_restart = 0;
   bool force_restart = true;
   int hit_max = 0;
+  int passes = (int)pass_no;    // passes over A so far (the initial z = A y, if any)
   double F = CUDART_INF, kkt = 0.0, pgmax = 0.0;
 
   for (;;) {
     // ============ phase G: g(z + t dz), grad = A^T g, F, phi'(t), phi''(t) ================
     double f_acc = 0.0, s1_acc = 0.0, s2_acc = 0.0;
+    ++passes;
     const bool rev = (pass_no++ & 1u) != 0u;
     for (int ti = 0; ti < n_tiles; ++ti) {
       const int tile = rev ? n_tiles - 1 - ti : ti;
@@ -792,6 +669,7 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
     force_restart = false;
 
     // ================= phase D: commit z, dz = A p, curvature =============================
+    ++passes;
     const double h_acc = pass_d(p_s, sm.dzs, t_trial, true);
     {
       double hv[1] = {h_acc};
@@ -837,7 +715,10 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
       DevState *st = p.st;
       st->K = K;
       st->m_iters = iters;
+      st->m_passes = passes;             // gradient passes (incl. repeated ones after a refined step) + dz passes
+      st->pass_total += passes;
       st->m_hit_max = hit_max;
+      st->n_hit_max += hit_max ? 1 : 0;
       st->m_restarts = restarts;
       st->m_added = added;
       st->m_F = F;
@@ -855,6 +736,8 @@ __global__ void __launch_bounds__(kMasterThreads, kMasterCtasPerSm) k_master(Mas
         rec.objective_before = st->F;
         rec.objective = F;
         rec.kkt_residual = kkt;
+        rec.n_passes = passes;
+        rec.hit_max_iter = hit_max;
         p.history[K - 1] = rec;
       }
     }
@@ -870,6 +753,7 @@ static size_t master_fixed_smem(const Ctx *c, int n_stages) {
 }
 
 cudaError_t master_configure(Ctx *c) {
+  if (c->opt.master_method == 2) return newton_configure(c);
   c->master_grid = std::min(c->n_sm * kMasterCtasPerSm, kMasterMaxGrid);
   int slab = (c->n_vox_pad + c->master_grid - 1) / c->master_grid;
   slab = (slab + 127) / 128 * 128;
@@ -909,6 +793,7 @@ cudaError_t master_configure(Ctx *c) {
 }
 
 cudaError_t launch_master(Ctx *c, bool add_candidate) {
+  if (c->opt.master_method == 2) return launch_newton(c, add_candidate);
   MasterParams p{};
   p.A = c->d.A;
   p.n_vox_pad = c->n_vox_pad;
@@ -925,6 +810,7 @@ cudaError_t launch_master(Ctx *c, bool add_candidate) {
   p.ll_part = c->d.ll_part;
   p.ll_result = c->d.ll_result;
   p.epoch = c->d.m_epoch;
+  p.red_stride = c->red_stride;
   p.prof = (c->opt.reserved & 2) ? c->d.m_prof : nullptr;
   p.st = c->d.state;
   p.history = c->d.history;

@@ -94,7 +94,15 @@ struct Dims {
   int32_t n_vox, n_bl, n_beams, n_rows, k_max, max_rows;
   int32_t chain_states;        // (W+1)^2 leaf states per row of the chain pricing modes, 0 otherwise
   int64_t nnz;
+  int32_t master_method;
+  int32_t n_struct;
 };
+
+// layout of the dose block and of the grid-reduction slots, decided by the master method alone
+static NewtonLayout layout_of_master(const Dims &dm, int32_t n_vox_pad) {
+  if (dm.master_method == 2) return newton_layout(dm.k_max, n_vox_pad, dm.n_struct);
+  return NewtonLayout{};
+}
 
 static int64_t tchunks_of(int64_t nnz) { return (nnz + kTChunk - 1) / kTChunk; }
 
@@ -136,14 +144,16 @@ static void carve_workspace(Carver &cv, const Dims &dm, const HostLayout &L, Dev
   d->ap_beam = cv.take<int32_t>((size_t)dm.k_max);
   d->ap_left = cv.take<int32_t>((size_t)dm.k_max * dm.max_rows);
   d->ap_right = cv.take<int32_t>((size_t)dm.k_max * dm.max_rows);
-  d->A = cv.take<float>((size_t)dm.k_max * vp);
+  const NewtonLayout nl = layout_of_master(dm, L.n_vox_pad);
+  d->A = cv.take<float>(nl.T ? (size_t)nl.n_tiles * (size_t)nl.tile_stride : (size_t)dm.k_max * vp);
   d->y = cv.take<double>((size_t)DAO_MAX_APERTURES);
   d->mz = cv.take<double>(vp);
   d->mdz = cv.take<double>(vp);
   {
     const size_t g = (size_t)std::min(n_sm * kMasterCtasPerSm, kMasterMaxGrid);
-    d->ll_part = cv.take<uint4>(2 * g * kMaxRedux);
-    d->ll_result = cv.take<uint4>(2 * kMaxRedux);
+    const size_t stride = nl.T ? (size_t)nl.n_red : (size_t)kMaxRedux;
+    d->ll_part = cv.take<uint4>(2 * g * stride);
+    d->ll_result = cv.take<uint4>(2 * stride);
   }
   d->m_epoch = cv.take<uint32_t>(64);
   d->m_prof = cv.take<unsigned long long>(kMasterProfSlots);
@@ -218,7 +228,7 @@ static dao_status check_args(const dao_csr *D, const dao_mlc *mlc, const dao_str
   if (opt->k_max < 1) { *err = "k_max must be >= 1"; return DAO_E_ARG; }
   if (opt->k_max > DAO_MAX_APERTURES) { *err = "k_max > DAO_MAX_APERTURES"; return DAO_E_UNSUPPORTED; }
   if (opt->master_max_iter < 0 || !(opt->master_tol >= 0.0) || !(opt->price_tol >= 0.0) ||
-      (opt->master_method != 0 && opt->master_method != 1) || opt->sell_sigma < 0 ||
+      (opt->master_method < 0 || opt->master_method > 2) || opt->sell_sigma < 0 ||
       !(opt->master_ls_tol > 0.0) || !(opt->master_ls_tol < 1.0) ||
       (opt->mlc_mode < DAO_MLC_CONSECUTIVE || opt->mlc_mode > DAO_MLC_CONNECTED)) {
     *err = "bad option value"; return DAO_E_ARG;
@@ -244,6 +254,8 @@ static dao_status check_args(const dao_csr *D, const dao_mlc *mlc, const dao_str
   dm->n_vox = D->n_vox; dm->n_bl = D->n_bl; dm->nnz = D->nnz;
   dm->n_beams = mlc->n_beams; dm->n_rows = mlc->n_rows; dm->k_max = opt->k_max;
   dm->max_rows = std::max(max_rows, 1);
+  dm->master_method = opt->master_method;
+  dm->n_struct = s->n_struct;
   dm->chain_states = 0;
   if (opt->mlc_mode == DAO_MLC_INTERDIGITATION || opt->mlc_mode == DAO_MLC_CONNECTED) {
     int32_t width = 0;
@@ -749,11 +761,15 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   SETUP_CUDA(cudaMemsetAsync(d.y, 0, DAO_MAX_APERTURES * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.mz, 0, vp * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.mdz, 0, vp * 8, q));
+  c->nwt = layout_of_master(dm, L.n_vox_pad);
+  c->red_stride = c->nwt.T ? c->nwt.n_red : kMaxRedux;
   {
     const size_t g = (size_t)std::min(c->n_sm * kMasterCtasPerSm, kMasterMaxGrid);
-    SETUP_CUDA(cudaMemsetAsync(d.ll_part, 0, 2 * g * kMaxRedux * sizeof(uint4), q));
-    SETUP_CUDA(cudaMemsetAsync(d.ll_result, 0, 2 * kMaxRedux * sizeof(uint4), q));
+    SETUP_CUDA(cudaMemsetAsync(d.ll_part, 0, 2 * g * (size_t)c->red_stride * sizeof(uint4), q));
+    SETUP_CUDA(cudaMemsetAsync(d.ll_result, 0, 2 * (size_t)c->red_stride * sizeof(uint4), q));
   }
+  // the tiled dose block is read with its padding (tile tails, the 4 pad floats of every column): finite zeros
+  if (c->nwt.T) SETUP_CUDA(cudaMemsetAsync(d.A, 0, (size_t)c->nwt.n_tiles * (size_t)c->nwt.tile_stride * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.m_epoch, 0, 64 * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.m_prof, 0, kMasterProfSlots * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.ap_beam, 0, (size_t)dm.k_max * 4, q));

@@ -68,12 +68,15 @@ struct SpmvParams {
   double *f_part;
   DevState *st;
   const int32_t *skip;       // device flag (may be null): non-zero -> the launch does nothing
+  // column mode: layout of the dose block A (a_index) and the column to write (< 0: the pool size K)
+  int32_t a_T, a_TP, a_col;
+  int64_t a_stride;
 };
 
 // per-row epilogue: objective / gradient (step 3) or plain store
 template <int MODE>
 __device__ __forceinline__ void spmv_store(const SpmvParams &p, float *out, const StructEntry *stab_s, int i,
-                                           double acc, double &f_acc) {
+                                           double acc, double &f_acc, int kcol) {
   if (MODE == kSpmvObjective) {
     const int s = p.sid[i];
     double gv = 0.0;
@@ -93,6 +96,8 @@ __device__ __forceinline__ void spmv_store(const SpmvParams &p, float *out, cons
   } else if (MODE == kSpmvPlainUserOrder) {
     const int32_t j = p.perm[i];
     if (j >= 0) out[j] = (float)acc;
+  } else if (MODE == kSpmvColumn) {
+    out[a_index(p.a_T, p.a_TP, p.a_stride, p.n_vox_pad, i, kcol)] = (float)acc;
   } else {
     out[i] = (float)acc;
   }
@@ -155,9 +160,13 @@ __global__ void __launch_bounds__(kSpmvRingThreads, 1) k_spmv_ring(SpmvParams p)
 
   float *out = p.out;
   if (p.skip && *p.skip) return;
+  int kcol = 0;
   if (MODE == kSpmvColumn) {
-    if (!p.st->cand_valid) return;                       // nothing to add (converged or pool full)
-    out += (size_t)p.st->K * (size_t)p.n_vox_pad;
+    kcol = p.a_col;
+    if (kcol < 0) {
+      if (!p.st->cand_valid) return;                     // nothing to add (converged or pool full)
+      kcol = p.st->K;
+    }
   }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (lane == 0) {
@@ -232,7 +241,7 @@ __global__ void __launch_bounds__(kSpmvRingThreads, 1) k_spmv_ring(SpmvParams p)
       __syncwarp();                          // every lane is done with the stage before it is refilled
       issue();
     }
-    spmv_store<MODE>(p, out, stab_s, slice * 32 + lane, acc, f_acc);
+    spmv_store<MODE>(p, out, stab_s, slice * 32 + lane, acc, f_acc, kcol);
   }
   if (MODE == kSpmvObjective) spmv_finish_objective(p, f_acc, red);
 }
@@ -247,9 +256,13 @@ __global__ void __launch_bounds__(kSpmvThreads, 2) k_spmv_sell(SpmvParams p) {
 
   float *out = p.out;
   if (p.skip && *p.skip) return;
+  int kcol = 0;
   if (MODE == kSpmvColumn) {
-    if (!p.st->cand_valid) return;
-    out += (size_t)p.st->K * (size_t)p.n_vox_pad;
+    kcol = p.a_col;
+    if (kcol < 0) {
+      if (!p.st->cand_valid) return;                     // nothing to add (converged or pool full)
+      kcol = p.st->K;
+    }
   }
   if (XS) {
     for (int i = threadIdx.x; i < p.n_bl; i += blockDim.x) xs[i] = p.x[i];
@@ -289,13 +302,13 @@ __global__ void __launch_bounds__(kSpmvThreads, 2) k_spmv_sell(SpmvParams p) {
       const float xv = XS ? xs[cc] : __ldg(p.x + cc);
       acc = fma((double)vv, (double)xv, acc);
     }
-    spmv_store<MODE>(p, out, stab_s, slice * 32 + lane, acc, f_acc);
+    spmv_store<MODE>(p, out, stab_s, slice * 32 + lane, acc, f_acc, kcol);
   }
   if (MODE == kSpmvObjective) spmv_finish_objective(p, f_acc, red);
 }
 
 template <int MODE>
-static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out, const int32_t *skip) {
+static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out, const int32_t *skip, int32_t a_col) {
   SpmvParams p{};
   p.col = c->d.sell_col;
   p.val = c->d.sell_val;
@@ -313,6 +326,8 @@ static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out, const in
   p.f_part = c->d.f_part;
   p.st = c->d.state;
   p.skip = skip;
+  p.a_T = c->nwt.T; p.a_TP = c->nwt.TP; p.a_stride = c->nwt.tile_stride; p.a_col = a_col;
+  if (MODE == kSpmvColumn) p.out = c->d.A;
   if (c->spmv_ring_warps > 0) {
     const int nw = c->spmv_ring_warps;
     const size_t smem = (size_t)nw * kRingStages * kRingStageBytes + align_up((size_t)nw * kRingStages * 8, 128) +
@@ -341,12 +356,12 @@ static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out, const in
   return cudaGetLastError();
 }
 
-cudaError_t launch_spmv(Ctx *c, SpmvMode mode, const float *x, float *out, const int32_t *skip) {
+cudaError_t launch_spmv(Ctx *c, SpmvMode mode, const float *x, float *out, const int32_t *skip, int32_t a_col) {
   switch (mode) {
-    case kSpmvObjective: return launch_spmv_mode<kSpmvObjective>(c, x, out, skip);
-    case kSpmvPlain: return launch_spmv_mode<kSpmvPlain>(c, x, out, skip);
-    case kSpmvColumn: return launch_spmv_mode<kSpmvColumn>(c, x, out, skip);
-    default: return launch_spmv_mode<kSpmvPlainUserOrder>(c, x, out, skip);
+    case kSpmvObjective: return launch_spmv_mode<kSpmvObjective>(c, x, out, skip, a_col);
+    case kSpmvPlain: return launch_spmv_mode<kSpmvPlain>(c, x, out, skip, a_col);
+    case kSpmvColumn: return launch_spmv_mode<kSpmvColumn>(c, x, out, skip, a_col);
+    default: return launch_spmv_mode<kSpmvPlainUserOrder>(c, x, out, skip, a_col);
   }
 }
 

@@ -73,7 +73,7 @@ class CPriceInfo(C.Structure):
 class CMasterInfo(C.Structure):
     _fields_ = [("n_apertures", C.c_int32), ("n_pg_iter", C.c_int32), ("hit_max_iter", C.c_int32),
                 ("n_restarts", C.c_int32), ("objective", C.c_double), ("kkt_residual", C.c_double),
-                ("pg_norm", C.c_double)]
+                ("pg_norm", C.c_double), ("n_passes", C.c_int32), ("reserved", C.c_int32)]
 
 
 class CRunInfo(C.Structure):
@@ -81,13 +81,14 @@ class CRunInfo(C.Structure):
                 ("n_duplicates", C.c_int32), ("n_pg_iter_total", C.c_int64), ("objective", C.c_double),
                 ("seconds_total", C.c_double), ("seconds_intensity", C.c_double), ("seconds_spmv", C.c_double),
                 ("seconds_spmv_t", C.c_double), ("seconds_price", C.c_double), ("seconds_column", C.c_double),
-                ("seconds_master", C.c_double)]
+                ("seconds_master", C.c_double), ("n_passes_total", C.c_int64), ("n_hit_max_iter", C.c_int32),
+                ("reserved", C.c_int32)]
 
 
 class CIterRecord(C.Structure):
     _fields_ = [("k", C.c_int32), ("beam", C.c_int32), ("n_pg_iter", C.c_int32), ("duplicate", C.c_int32),
                 ("price", C.c_double), ("objective_before", C.c_double), ("objective", C.c_double),
-                ("kkt_residual", C.c_double)]
+                ("kkt_residual", C.c_double), ("n_passes", C.c_int32), ("hit_max_iter", C.c_int32)]
 
 
 class CFmoInfo(C.Structure):
@@ -110,7 +111,7 @@ class CDims(C.Structure):
 
 ITER_RECORD_DTYPE = np.dtype([("k", "<i4"), ("beam", "<i4"), ("n_pg_iter", "<i4"), ("duplicate", "<i4"),
                               ("price", "<f8"), ("objective_before", "<f8"), ("objective", "<f8"),
-                              ("kkt_residual", "<f8")])
+                              ("kkt_residual", "<f8"), ("n_passes", "<i4"), ("hit_max_iter", "<i4")])
 
 _lib = None
 
