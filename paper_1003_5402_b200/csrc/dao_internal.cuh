@@ -50,6 +50,7 @@ constexpr int kNoStruct = 255;         // sid value of a voxel without penalty
 constexpr int kMaxRedux = DAO_MAX_APERTURES + 8;   // doubles per grid reduction in the master (methods 0, 1)
 
 // ---- master_method = 2 (projected Newton, dao_newton.cu) ----
+constexpr int kNewtonMaxK = 103;   // largest pool method 2 handles (13 block rows of the Hessian); larger k_max: method 1
 // The aperture-dose block is stored TILED: tile t (T internal voxels) holds its k_max columns back to
 // back, each padded to TP = T + 4 floats (TP = 4 mod 32: conflict-free tensor-core fragment loads), so
 // the K live columns of a tile are ONE contiguous range = one bulk copy.
@@ -62,6 +63,8 @@ struct NewtonLayout {
   int32_t stage_bytes = 0;  // k_max * TP * 4 rounded to 128
   int32_t nb_max = 0;       // 8x8 block rows of the augmented Hessian at K = k_max: ceil((k_max + 1) / 8)
   int32_t n_red = 0;        // doubles per grid reduction: nb_max (nb_max + 1) / 2 * 64 + 8
+  int32_t AC = 0;           // active voxels per chunk of the Hessian phase
+  int32_t lbuf_doubles = 0; // shared buffer of the LDL^T factorisation and of the fp64 tile W of the Hessian phase
   size_t smem = 0;          // dynamic shared memory of k_master_newton
 };
 

@@ -32,9 +32,16 @@
 
 namespace dao {
 
-constexpr int kNwtMaxB = 10;            // 8x8 blocks of H a warp may own (153 blocks at K = 128 over 16 warps)
-constexpr int kNwtMaxBlocks = 160;      // >= nb (nb + 1) / 2 for nb = 17
-constexpr int kNwtZThreads = kMasterWorkers;
+constexpr int kNwtStrips = 3;           // strips of H blocks a warp may own: 8 back warps x 3 = the 24 strips of K <= kNewtonMaxK
+constexpr int kNwtStripLen = 5;         // 8x8 blocks per strip (one block row, consecutive block columns)
+constexpr int kNwtMaxStrips = 48;       // >= sum_I ceil((nb - I) / 4) for nb = 17 (45)
+#ifndef DAO_NWT_MIN_STAGES
+#define DAO_NWT_MIN_STAGES 2
+#endif
+constexpr int kNwtMinStages = DAO_NWT_MIN_STAGES;   // ring stages a layout must have (2: bigger W chunks win, measured)
+constexpr int kNwtFront = 8;             // front warps: dose, penalty, active list, fp64 tile W
+constexpr int kNwtBack = kNW - kNwtFront;   // back warps: H += W W^T on the fp64 tensor cores
+constexpr int kNwtFrontThreads = kNwtFront * 32;
 
 struct NewtonParams {
   const float *A;            // tiled dose block
@@ -45,7 +52,12 @@ struct NewtonParams {
   int32_t n_stages;
   int32_t stage_bytes;
   int32_t n_red_cap;         // capacity (doubles) of the reduction staging array = slots per CTA
-  int32_t lbuf_doubles;      // capacity of the factorisation buffer
+  int32_t lbuf_doubles;      // capacity of the factorisation buffer (also holds the W tile)
+  int32_t AC;                // active voxels per chunk of the H phase (power of two)
+  int32_t w_doubles;         // doubles per W tile: (8 nb_max + 1) (AC + 4)
+  int32_t srow;              // 8 nb_max
+  int32_t ks_shift;          // log2 of the k-slices per voxel of the dose loop: T << ks_shift = 256 front threads
+  int32_t debug;             // timing experiments only (dao_options.reserved >> 3): 1 no DMMA, 2 no W conversion, 4 no Z loop
   int32_t n_struct;
   const uint8_t *sid;
   const float *vt;           // per-voxel thresholds T_j (re-optimisation mode) or null
@@ -64,6 +76,24 @@ struct NewtonParams {
   int32_t k_max;
   double tol;
 };
+
+// barrier over the front warps
+__device__ __forceinline__ void fsync() { asm volatile("bar.sync 2, %0;" ::"n"(kNwtFrontThreads) : "memory"); }
+
+// fp32 -> fp64 of a finite value >= 0 on the integer pipe (F2F.F64.F32 runs at 16 per clock and SM with ~90
+// cycles of latency, measured): exact for normal numbers; +0 maps to 2^-127 -- the dose loop subtracts exactly
+// what that adds, the Hessian tile does not care (products with 1e-38 vanish).
+__device__ __forceinline__ double cvt_pos(float x) {
+  // (b << 29) as a 64-bit product puts b >> 3 into the high word; one IMAD.WIDE with the exponent re-bias added
+  const unsigned long long r = (unsigned long long)__float_as_uint(x) * 0x20000000ull + 0x3800000000000000ull;
+  return __longlong_as_double((long long)r);
+}
+
+__device__ __forceinline__ double lds_f64(uint32_t addr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+  return v;
+}
 
 __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -84,7 +114,9 @@ __device__ __forceinline__ double h_sym(const double *hred, int nb, int a, int b
 // packed lower triangle
 __device__ __forceinline__ int lidx(int i, int j) { return (i * (i + 1)) / 2 + j; }
 
-__global__ void __launch_bounds__(kMasterThreads, 1) k_master_newton(NewtonParams p) {
+// 16 warps exactly: a 17th (a dedicated producer warp, as in k_master) would be allocated as 20 warps and cap the
+// kernel at 96 registers, which made the compiler serialise the tensor-core loop through one temporary register.
+__global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParams p) {
   extern __shared__ __align__(128) unsigned char dyn_smem[];
   __shared__ double y_s[DAO_MAX_APERTURES];        // accepted point
   __shared__ double ytr_s[DAO_MAX_APERTURES];      // trial point of the current pass
@@ -93,13 +125,12 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master_newton(NewtonParam
   __shared__ double dpiv_s[DAO_MAX_APERTURES + 1]; // pivots of the LDL^T factorisation
   __shared__ double xs_s[DAO_MAX_APERTURES + 1];   // solution on the free set
   __shared__ int fr_s[DAO_MAX_APERTURES];          // free variables
-  __shared__ unsigned short blk_s[kNwtMaxBlocks];  // block -> (I << 8) | J
+  __shared__ unsigned short strip_s[kNwtMaxStrips];  // strip -> (I << 8) | J0, longest strips first
   __shared__ double sc[16];
   __shared__ int si[16];
   __shared__ int wcnt_s[kNW];
+  __shared__ volatile int wmeta_s[2];              // per W buffer: columns (multiple of 4) | last chunk of its tile << 16
   __shared__ double fred_s[kNW];
-  __shared__ volatile int s_stop;
-  __shared__ volatile unsigned s_consumed_stage, s_consumed_phase;
   __shared__ unsigned long long prof_s[kMasterProfSlots];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -125,61 +156,26 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master_newton(NewtonParam
   unsigned char *ring = q; q += (size_t)NS * p.stage_bytes;
   uint64_t *full = reinterpret_cast<uint64_t *>(q); q += 128;
   uint64_t *empty = reinterpret_cast<uint64_t *>(q); q += 128;
+  uint64_t *wfull = empty + 8, *wempty = empty + 10;   // the two W buffers (n_stages <= 6)
   StructEntry *stab = reinterpret_cast<StructEntry *>(q); q += align_up_c((size_t)p.n_struct * sizeof(StructEntry), 128);
   double *hred = reinterpret_cast<double *>(q); q += align_up_c((size_t)p.n_red_cap * 8, 128);
   double *lbuf = reinterpret_cast<double *>(q); q += align_up_c((size_t)p.lbuf_doubles * 8, 128);
-  double *zpart = reinterpret_cast<double *>(q); q += (size_t)kNwtZThreads * 8;
+  double *wbuf = lbuf;                             // the two W tiles of the H phase share the factorisation buffer
+  const int AC = p.AC, WP = p.AC + 4;              // active voxels per chunk, row pitch of W (4 mod 16: conflict-free)
+  const int ac_shift = 31 - __clz(AC);
+  const int w_doubles = p.w_doubles;               // doubles per W tile
+  const int srow = p.srow;                         // row of W that holds the curvature weights s_a
   double *gs = reinterpret_cast<double *>(q); q += align_up_c((size_t)(T + 4) * 8, 128);
   double *ss = reinterpret_cast<double *>(q); q += align_up_c((size_t)(T + 4) * 8, 128);
   unsigned short *list = reinterpret_cast<unsigned short *>(q);
 
   if (tid == 0) {
-    for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], kNW); }
-    s_stop = 0;
+    for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], kNwtFront); }
+    for (int s = 0; s < 2; ++s) { mbar_init(&wfull[s], kNwtFront); mbar_init(&wempty[s], kNwtBack); }
     for (int i = 0; i < kMasterProfSlots; ++i) prof_s[i] = 0ull;
   }
   fence_mbar_init();
   __syncthreads();
-
-  // =============================== producer warp ================================================
-  if (warp == kNW) {
-    if (lane == 0) {
-      RingPos pp{0, 0u};
-      bool first_round = true;
-      bool stop = ntl == 0;
-      const uint32_t bytes = (uint32_t)K * (uint32_t)TP * 4u;
-      // every pass reads the same tiles; odd passes walk them backwards (what was read last is read
-      // first: an LRU-like L2 keeps serving the most recent part of A once 4 V K bytes exceed it)
-      for (unsigned pass = 0; !stop; ++pass) {
-        const bool rev = (pass & 1u) != 0u;
-        for (int ti = 0; ti < ntl && !stop; ++ti) {
-          const int tile = tb0 + (rev ? ntl - 1 - ti : ti) * tstep;
-          if (!first_round) {
-            while (!mbar_try_wait(&empty[pp.stage], pp.phase ^ 1u)) {
-              if (s_stop) { stop = true; break; }
-            }
-            if (stop) break;
-          }
-          mbar_arrive_expect_tx(&full[pp.stage], bytes);
-          bulk_g2s(ring + (size_t)pp.stage * p.stage_bytes, p.A + (size_t)tile * (size_t)p.tile_stride, bytes,
-                   &full[pp.stage]);
-          pp.advance(NS);
-          if (pp.stage == 0) first_round = false;
-        }
-      }
-      while (!s_stop) { __nanosleep(100); }
-      if (ntl > 0) {
-        // drain: every issued stage must have landed before the CTA may exit
-        RingPos cp{(int)s_consumed_stage, s_consumed_phase};
-        while (cp.stage != pp.stage || cp.phase != pp.phase) {
-          mbar_wait(&full[cp.stage], cp.phase);
-          cp.advance(NS);
-        }
-      }
-    }
-    __syncthreads();     // matches the final barrier of the workers
-    return;
-  }
 
   // =============================== worker warps =================================================
   const int nb = (K + 1 + 7) >> 3;                 // 8x8 block rows of the augmented matrix (K columns + gradient)
@@ -192,32 +188,46 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master_newton(NewtonParam
     d_s[tid] = 0.0;
     grad_s[tid] = 0.0;
   }
-  for (int bi = tid; bi < nblocks; bi += kMasterWorkers) {   // block table (row-major upper triangle)
-    int I = 0, rem = bi;
-    while (rem >= nb - I) { rem -= nb - I; ++I; }
-    blk_s[bi] = (unsigned short)((I << 8) | (I + rem));
-  }
-  if (tid < 4) { gs[T + tid] = 0.0; ss[T + tid] = 0.0; }      // the dummy voxel that pads a quad
   Reducer red{p.ll_part, p.ll_result, 0u, p.n_red_cap};
   if (tid == 0) si[7] = (int)*p.epoch;
   wsync();
   red.ep = (uint32_t)si[7];
 
-  // distribution of the H blocks: NC classes of warps x NG groups; class c owns the blocks c, c + NC, ...;
-  // group g takes the quads g, g + NG, ... of the active voxels of a tile
+  // Distribution of the H blocks over the BACK warps.  The upper block triangle is cut into STRIPS of <= 4
+  // consecutive blocks of one block row (one A fragment serves the whole strip); the strips, longest first, are
+  // dealt to NC classes of back warps in snake order; the NG = 12 / NC warps of a class (groups) share the quads
+  // of active voxels.
+  if (tid == 0) {
+    int n = 0;
+    for (int len = kNwtStripLen; len >= 1; --len)
+      for (int I = 0; I < nb; ++I)
+        for (int J0 = I; J0 < nb; J0 += kNwtStripLen)
+          if (min(kNwtStripLen, nb - J0) == len) strip_s[n++] = (unsigned short)((I << 8) | J0);
+    si[8] = n;
+  }
+  wsync();
+  const int nstrips = si[8];
   int NC = 1;
-  while ((nblocks + NC - 1) / NC > kNwtMaxB || (NC < kNW && (nblocks + NC - 1) / NC > 7 && nblocks >= 2 * NC)) NC <<= 1;
-  if (NC > kNW) NC = kNW;
-  const int NG = kNW / NC;
-  const int cls = warp % NC, grp = warp / NC;
-  const int nmine = (nblocks - cls + NC - 1) / NC;     // blocks of this warp
-  // Z phase: thread = (k-slice, voxel)
-  const int KS = kNwtZThreads / T;                     // k-slices
-  const int zs = tid / T, zv = tid - zs * T;
-  const int kchunk = (K + KS - 1) / KS;
-  const int zk0 = min(K, zs * kchunk), zk1 = min(K, zk0 + kchunk);
-  const bool z_on = zs < KS;
-  const int fin_warps = T >> 5;                        // warps that finalise voxels (T <= 256)
+  while (NC < kNwtBack && ((nstrips + NC - 1) / NC > kNwtStrips || kNwtBack % NC != 0)) ++NC;
+  const int NG = kNwtBack / NC;
+  const bool is_front = warp < kNwtFront;
+  const int bw = is_front ? 0 : warp - kNwtFront;
+  const int cls = bw % NC, grp = bw / NC;
+  int nstr = 0;
+  int st_offa[kNwtStrips], st_offb[kNwtStrips], st_len[kNwtStrips], st_blk[kNwtStrips];
+#pragma unroll
+  for (int s = 0; s < kNwtStrips; ++s) {
+    const int i = s * NC + ((s & 1) ? NC - 1 - cls : cls);
+    st_offa[s] = st_offb[s] = st_len[s] = st_blk[s] = 0;
+    if (!is_front && i < nstrips) {
+      const int I = strip_s[i] >> 8, J0 = strip_s[i] & 255;
+      st_offa[s] = (I * 8 + (lane >> 2)) * WP;
+      st_offb[s] = (J0 * 8 + (lane >> 2)) * WP;
+      st_len[s] = min(kNwtStripLen, nb - J0);
+      st_blk[s] = blk_index(nb, I, J0);
+      nstr = s + 1;
+    }
+  }
 
   const bool prof = (p.prof != nullptr) && blockIdx.x == 0 && tid == 0;
   unsigned long long tprof = prof ? gtimer() : 0ull;
@@ -230,114 +240,313 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master_newton(NewtonParam
     }                                                     \
   } while (0)
 
-  RingPos cp{0, 0u};
+  RingPos cp{0, 0u};                       // front warps: position in the A stream
+  // The A stream is fed by lane 0 of the LAST back warp while it waits for W tiles (issuing a bulk copy costs the
+  // issuing thread ~500 cycles: on a front warp that is the critical path of every tile).  Every pass reads the
+  // same tiles, odd passes backwards (what was read last is read first: an LRU-like L2 keeps serving the most
+  // recent part of A once 4 V K bytes exceed it); the sequence simply continues into the next pass, so the first
+  // stages of a pass are in flight while the grid reduces (a pass that never happens is drained before the exit).
+  RingPos ip{0, 0u};                       // issue position
+  int issued_total = 0, consumed_total = 0, issue_ti = 0;
+  bool issue_rev = false;
+  const bool is_issuer = tid == kMasterWorkers - 32;
+  const uint32_t tile_bytes = (uint32_t)K * (uint32_t)TP * 4u;
+  auto feed = [&]() {                      // issue copies while stages are free; never blocks
+    while (ntl > 0) {
+      // the stage was used before: all front warps must have released it (try_wait would block for ~0.5 us)
+      if (issued_total >= NS && !mbar_test_wait(&empty[ip.stage], ip.phase ^ 1u)) break;
+      const int tile = tb0 + (issue_rev ? ntl - 1 - issue_ti : issue_ti) * tstep;
+      mbar_arrive_expect_tx(&full[ip.stage], tile_bytes);
+      bulk_g2s(ring + (size_t)ip.stage * p.stage_bytes, p.A + (size_t)tile * (size_t)p.tile_stride, tile_bytes,
+               &full[ip.stage]);
+      ip.advance(NS);
+      ++issued_total;
+      if (++issue_ti == ntl) { issue_ti = 0; issue_rev = !issue_rev; }
+    }
+  };
+  RingPos wp{0, 0u};                       // position in the two W buffers (front: producing, back: consuming)
+  bool w_first_round = true;
   unsigned pass_no = 0;
-  const int rowoff = (lane >> 2) * TP;
   const int r8 = lane >> 2, c2 = (lane & 3) * 2;
+  const double kTiny = 5.877471754111438e-39;      // 2^-127 = cvt_pos(+0)
 
   // ---- one pass over A at the point yv: z, F, pi, grad, H -> hred (reduced over the grid) ----
+  // Front warps (4): per tile  Z (dose of every voxel, thread = voxel), P (penalty, gradient, curvature weight,
+  // list of the active voxels), W (fp64 tile of the active voxels, chunk by chunk into one of two buffers).
+  // Back warps (12): per chunk  H += W W^T on the fp64 tensor cores.  The two sides meet only on the mbarriers of
+  // the W buffers; the A stage is released by the front warps as soon as the tile's last chunk is converted.
   auto pass = [&](const double *yv) {
-    double acc[kNwtMaxB][2];
-#pragma unroll
-    for (int j = 0; j < kNwtMaxB; ++j) { acc[j][0] = 0.0; acc[j][1] = 0.0; }
-    unsigned blk[kNwtMaxB];
-#pragma unroll
-    for (int j = 0; j < kNwtMaxB; ++j) blk[j] = (j < nmine) ? (unsigned)blk_s[cls + j * NC] : 0u;
     double f_acc = 0.0;
     const bool rev = (pass_no++ & 1u) != 0u;
-    for (int ti = 0; ti < ntl; ++ti) {
-      const int tile = tb0 + (rev ? ntl - 1 - ti : ti) * tstep;
-      mbar_wait(&full[cp.stage], cp.phase);
-      const float *M = reinterpret_cast<const float *>(ring + (size_t)cp.stage * p.stage_bytes);
-      // ---- Z: partial doses ----
-      if (z_on) {
-        double a0 = 0.0, a1 = 0.0;
-        const float *col = M + zv;
-        int k = zk0;
-        for (; k + 1 < zk1; k += 2) {
-          a0 = fma(yv[k], (double)col[(size_t)k * TP], a0);
-          a1 = fma(yv[k + 1], (double)col[(size_t)(k + 1) * TP], a1);
+    if (is_front) {
+      // thread = (voxel, k-slice): T * KS = 256 front threads, the KS slices of a voxel in adjacent lanes
+      const int ks_shift = p.ks_shift, KS = 1 << ks_shift;
+      const int v0 = tid >> ks_shift, zsl = tid & (KS - 1);
+      const int nI = (K > zsl) ? (K - zsl + KS - 1) >> ks_shift : 0;      // columns zsl, zsl + KS, ... of this thread
+      const int rstep = TP << ks_shift;
+      // what the +0 -> 2^-127 of cvt_pos adds to a dose, accumulated exactly like the dose itself
+      double zc;
+      {
+        double c[4] = {0.0, 0.0, 0.0, 0.0};
+        int i = 0;
+        for (; i + 3 < nI; i += 4) {
+#pragma unroll
+          for (int u = 0; u < 4; ++u) c[u] = fma(yv[zsl + ((i + u) << ks_shift)], kTiny, c[u]);
         }
-        if (k < zk1) a0 = fma(yv[k], (double)col[(size_t)k * TP], a0);
-        zpart[tid] = a0 + a1;
+#pragma unroll
+        for (int u = 0; u < 3; ++u)
+          if (i + u < nI) c[u] = fma(yv[zsl + ((i + u) << ks_shift)], kTiny, c[u]);
+        zc = (c[0] + c[1]) + (c[2] + c[3]);
       }
-      wsync();
-      // ---- P: dose, penalty, gradient, curvature weight, active flag ----
-      bool active = false;
-      if (tid < T) {
-        double z = 0.0;
-        for (int s = 0; s < KS; ++s) z += zpart[s * T + tid];
-        const int vg = tile * T + tid;
-        double gv = 0.0, sv = 0.0;
-        if (vg < p.n_vox_pad) {
-          const int s = p.sid[vg];
-          if (s != kNoStruct) {
-            StructEntry e = stab[s];
-            if (p.vt) e.tm = e.tp = (double)p.vt[vg];
-            const double un = fmax(e.tm - z, 0.0), ov = fmax(z - e.tp, 0.0);
+      // structure id / threshold of this thread's voxel, fetched one tile ahead (an L2 round trip is longer than Z)
+      int sid_n = kNoStruct;
+      float vt_n = 0.f;
+      auto fetch_sid = [&](int ti_) {
+        sid_n = kNoStruct;
+        vt_n = 0.f;
+        if (ti_ < ntl) {
+          const int vg = (tb0 + (rev ? ntl - 1 - ti_ : ti_) * tstep) * T + v0;
+          if (zsl == 0 && vg < p.n_vox_pad) {
+            if (p.debug & 16) sid_n = (vg & 7) == 0 ? 0 : kNoStruct;      // timing experiment: no global load
+            else { sid_n = p.sid[vg]; if (p.vt) vt_n = p.vt[vg]; }
+          }
+        }
+      };
+      fetch_sid(0);
+      for (int ti = 0; ti < ntl; ++ti) {
+        const int tile = tb0 + (rev ? ntl - 1 - ti : ti) * tstep;
+        long long tc = prof ? clock64() : 0ll;
+#define CYC_MARK(slot)                                    \
+  do {                                                    \
+    if (prof) {                                           \
+      const long long now_ = clock64();                   \
+      prof_s[slot] += (unsigned long long)(now_ - tc);    \
+      tc = now_;                                          \
+    }                                                     \
+  } while (0)
+        // structure id / threshold of this thread's voxel: issued before the wait, used after the Z loop
+        const int vg0 = tile * T + v0;
+        const bool in0 = zsl == 0 && vg0 < p.n_vox_pad;
+        const int sid0 = sid_n;
+        const float vt0 = vt_n;
+        fetch_sid(ti + 1);
+        mbar_wait(&full[cp.stage], cp.phase);
+        CYC_MARK(12);
+        const float *M = reinterpret_cast<const float *>(ring + (size_t)cp.stage * p.stage_bytes);
+        // ---- Z ----
+        double z0;
+        {
+          // four independent chains; the loads of a group of 4 columns are issued together, one group ahead of
+          // their use (one or two warps per scheduler cannot hide the shared-memory latency any other way)
+          double a[4] = {0.0, 0.0, 0.0, 0.0};
+          const float *pa = M + v0 + zsl * TP;
+          const double *py = yv + zsl;
+          float f[4];
+          double yk[4];
+          if (!(p.debug & 4)) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+              const int ii = max(min(u, nI - 1), 0);
+              f[u] = pa[(size_t)ii * rstep];
+              yk[u] = py[ii << ks_shift];
+            }
+            int i = 0;
+            for (; i + 7 < nI; i += 4) {                 // the next group exists in full: no clamps
+              float n[4];
+              double yn[4];
+              pa += 4 * rstep;
+              py += 4 << ks_shift;
+#pragma unroll
+              for (int u = 0; u < 4; ++u) { n[u] = pa[(size_t)u * rstep]; yn[u] = py[u << ks_shift]; }
+#pragma unroll
+              for (int u = 0; u < 4; ++u) a[u] = fma(yk[u], cvt_pos(f[u]), a[u]);
+#pragma unroll
+              for (int u = 0; u < 4; ++u) { f[u] = n[u]; yk[u] = yn[u]; }
+            }
+            if (i + 3 < nI) {                            // one more full group; its successor is partial
+              float n[4];
+              double yn[4];
+              pa += 4 * rstep;
+              py += 4 << ks_shift;
+#pragma unroll
+              for (int u = 0; u < 4; ++u) {
+                const int uu = min(u, nI - 1 - (i + 4));     // >= 0 when the partial group is not empty
+                n[u] = pa[(size_t)max(uu, 0) * rstep];
+                yn[u] = py[max(uu, 0) << ks_shift];
+              }
+#pragma unroll
+              for (int u = 0; u < 4; ++u) a[u] = fma(yk[u], cvt_pos(f[u]), a[u]);
+#pragma unroll
+              for (int u = 0; u < 4; ++u) { f[u] = n[u]; yk[u] = yn[u]; }
+              i += 4;
+            }
+#pragma unroll
+            for (int u = 0; u < 3; ++u)
+              if (i + u < nI) a[u] = fma(yk[u], cvt_pos(f[u]), a[u]);
+          }
+          z0 = ((a[0] + a[1]) + (a[2] + a[3])) - zc;
+          // the slices of a voxel sit in adjacent lanes: fixed butterfly
+          for (int o = 1; o < KS; o <<= 1) z0 += __shfl_xor_sync(0xffffffffu, z0, o);
+        }
+        CYC_MARK(13);
+        // ---- P ----
+        bool act0 = false;
+        double sq0 = 0.0, gq0 = 0.0;                             // s_j = 2 c_j, pi_j / s_j
+        if (in0) {
+          if (sid0 != kNoStruct) {
+            StructEntry e = stab[sid0];
+            if (p.vt) e.tm = e.tp = (double)vt0;
+            const double un = fmax(e.tm - z0, 0.0), ov = fmax(z0 - e.tp, 0.0);
             f_acc += e.a * un * un + e.b * ov * ov;
-            gv = -2.0 * e.a * un + 2.0 * e.b * ov;
-            sv = 2.0 * ((un > 0.0 ? e.a : 0.0) + (ov > 0.0 ? e.b : 0.0));
+            const double gv = -2.0 * e.a * un + 2.0 * e.b * ov;
+            const double sv = 2.0 * ((un > 0.0 ? e.a : 0.0) + (ov > 0.0 ? e.b : 0.0));
+            if (sv != 0.0) {
+              act0 = true;
+              sq0 = sv;
+              // pi / s = -(T^- - z) below the band, z - T^+ above it; both sides at once only if T^- > T^+
+              gq0 = (un > 0.0 && ov > 0.0) ? gv / sv : (un > 0.0 ? -un : ov);
+            }
           }
-          p.mz[vg] = z;
+          if (!(p.debug & 8)) p.mz[vg0] = z0;
         }
-        gs[tid] = gv;
-        ss[tid] = sv;
-        active = sv != 0.0;
-      }
-      int rank = 0;
-      if (warp < fin_warps) {
-        const unsigned m = __ballot_sync(0xffffffffu, active);
-        rank = __popc(m & ((1u << lane) - 1u));
-        if (lane == 0) wcnt_s[warp] = __popc(m);
-      }
-      wsync();
-      int n_act = 0, my_off = 0;
-      for (int w = 0; w < fin_warps; ++w) {
-        const int cnt = wcnt_s[w];
-        if (w < warp) my_off += cnt;
-        n_act += cnt;
-      }
-      if (active) list[my_off + rank] = (unsigned short)tid;
-      if (tid < 4 && n_act + tid < ((n_act + 3) & ~3)) list[n_act + tid] = (unsigned short)T;
-      wsync();
-      // ---- H: augmented Gram matrix over the active voxels, fp64 tensor cores ----
-      const int nq = (n_act + 3) >> 2;
-      for (int qd = grp; qd < nq; qd += NG) {
-        const int vox = (int)list[qd * 4 + (lane & 3)];
-        const double sv = ss[vox], gv = gs[vox];
-        const float *Mv = M + rowoff + vox;
+        const unsigned m0 = __ballot_sync(0xffffffffu, act0);
+        if (lane == 0) wcnt_s[warp] = __popc(m0);
+        fsync();
+        int n_act = 0, off0 = 0;
 #pragma unroll
-        for (int j = 0; j < kNwtMaxB; ++j) {
-          if (j < nmine) {
-            const int I = (int)(blk[j] >> 8), J = (int)(blk[j] & 255u);
-            const int ka = I * 8 + r8, kb = J * 8 + r8;
-            double a = 0.0, b = 0.0;
-            if (ka < K) a = (double)Mv[(size_t)I * 8 * TP];
-            if (kb < K) b = sv * (double)Mv[(size_t)J * 8 * TP];
-            else if (kb == K) b = gv;
-            dmma884(acc[j][0], acc[j][1], a, b);
-          }
+        for (int w = 0; w < kNwtFront; ++w) {
+          const int cnt = wcnt_s[w];
+          if (w < warp) off0 += cnt;
+          n_act += cnt;
         }
-      }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[cp.stage]);
-      cp.advance(NS);
-    }
-    PROF_MARK(1);
-    // ---- CTA partial: the groups add their blocks in group order ----
-    for (int gg = 0; gg < NG; ++gg) {
-      if (grp == gg) {
+        if (act0) {
+          const int i = off0 + __popc(m0 & ((1u << lane) - 1u));
+          list[i] = (unsigned short)v0; gs[i] = gq0; ss[i] = sq0;
+        }
+        if (prof) prof_s[11] += (unsigned long long)n_act;
+        fsync();
+        CYC_MARK(14);
+        // ---- W: chunks of AC active voxels.  W[k][a] = A[k][v_a] in fp64 (integer pipe only), row K: pi_a / s_a,
+        //      row 8 nb_max: s_a.  The back warps scale the B fragment by s_a. ----
+        int c0 = 0;
+        do {
+          const int nca = min(AC, n_act - c0), nca4 = (nca + 3) & ~3;
+          if (!w_first_round) mbar_spin_wait(&wempty[wp.stage], wp.phase ^ 1u);
+          CYC_MARK(5);
+          double *wt = wbuf + (size_t)wp.stage * w_doubles;
+          if (tid < nca4) wt[(size_t)srow * WP + tid] = (tid < nca) ? ss[c0 + tid] : 0.0;
+          if (tid < nca4) wt[(size_t)K * WP + tid] = (tid < nca) ? gs[c0 + tid] : 0.0;
+          {
+            // thread = (column a, row parity); the voxel of the column is looked up once
+            const int a = tid & (AC - 1), kpar = tid >> ac_shift, kstep = kNwtFrontThreads >> ac_shift;
+            if (a < nca4 && !(p.debug & 2)) {
+              const bool live = a < nca;
+              const float *src = M + (live ? (int)list[c0 + a] : 0);
+              double *dst = wt + a;
+              for (int k = kpar; k < K; k += 4 * kstep) {
+                float f[4];
 #pragma unroll
-        for (int j = 0; j < kNwtMaxB; ++j) {
-          if (j < nmine) {
-            double *h = hred + (size_t)(cls + j * NC) * 64 + r8 * 8 + c2;
-            if (gg == 0) { h[0] = acc[j][0]; h[1] = acc[j][1]; }
-            else { h[0] += acc[j][0]; h[1] += acc[j][1]; }
+                for (int u = 0; u < 4; ++u) f[u] = src[(size_t)min(k + u * kstep, K - 1) * TP];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                  if (k + u * kstep < K) dst[(size_t)(k + u * kstep) * WP] = live ? cvt_pos(f[u]) : 0.0;
+              }
+            }
           }
-        }
+          c0 += AC;
+          if (tid == 0) wmeta_s[wp.stage] = nca4 | (c0 >= n_act ? 0x10000 : 0);
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&wfull[wp.stage]);
+          wp.advance(2);
+          if (wp.stage == 0) w_first_round = false;
+          CYC_MARK(6);
+        } while (c0 < n_act);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[cp.stage]);
+        cp.advance(NS);
+        ++consumed_total;
+      }
+#undef CYC_MARK
+      wsync();
+      PROF_MARK(1);
+      for (int gg = 0; gg < NG; ++gg) wsync();         // the back warps add up their blocks
+    } else {
+      double acc[kNwtStrips][kNwtStripLen][2];
+#pragma unroll
+      for (int s = 0; s < kNwtStrips; ++s)
+#pragma unroll
+        for (int m = 0; m < kNwtStripLen; ++m) { acc[s][m][0] = 0.0; acc[s][m][1] = 0.0; }
+      for (int ti = 0; ti < ntl; ++ti) {
+        bool last;
+        do {
+          const bool bprof = (p.prof != nullptr) && blockIdx.x == 0 && tid == kNwtFrontThreads;
+          long long tb = bprof ? clock64() : 0ll;
+          while (!mbar_test_wait(&wfull[wp.stage], wp.phase)) {
+            if (is_issuer) feed();
+          }
+          if (is_issuer) feed();
+          if (bprof) { const long long n_ = clock64(); prof_s[0] += (unsigned long long)(n_ - tb); tb = n_; }
+          const int meta = wmeta_s[wp.stage];
+          last = (meta & 0x10000) != 0;
+          const int nq = (meta & 0xffff) >> 2;
+          const double *wt = wbuf + (size_t)wp.stage * w_doubles;
+          const uint32_t wt_s = smem_addr(wt);
+          for (int qd = grp; qd < ((p.debug & 1) ? 0 : nq); qd += NG) {
+            const uint32_t wq = wt_s + (uint32_t)(qd * 4 + (lane & 3)) * 8u;
+            const double sv = lds_f64(wq + (uint32_t)(srow * WP) * 8u);
+#pragma unroll
+            for (int s = 0; s < kNwtStrips; ++s) {
+              if (s < nstr) {
+                // all fragments of the strip are requested before the first tensor-core instruction (volatile loads:
+                // left alone, the compiler sinks every load next to its predicated mma and the chain
+                // load -> scale -> mma runs once per block, 75 cycles instead of 16); a short strip re-reads
+                // its last block
+                const double fa = lds_f64(wq + (uint32_t)st_offa[s] * 8u);
+                double fb[kNwtStripLen];
+#pragma unroll
+                for (int m = 0; m < kNwtStripLen; ++m)
+                  fb[m] = lds_f64(wq + (uint32_t)(st_offb[s] + min(m, st_len[s] - 1) * 8 * WP) * 8u);
+#pragma unroll
+                for (int m = 0; m < kNwtStripLen; ++m) fb[m] *= sv;
+                if (st_len[s] == kNwtStripLen) {           // full strip: straight-line tensor-core code
+#pragma unroll
+                  for (int m = 0; m < kNwtStripLen; ++m) dmma884(acc[s][m][0], acc[s][m][1], fa, fb[m]);
+                } else {
+#pragma unroll
+                  for (int m = 0; m < kNwtStripLen; ++m) {
+                    if (m < st_len[s]) dmma884(acc[s][m][0], acc[s][m][1], fa, fb[m]);
+                  }
+                }
+              }
+            }
+          }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&wempty[wp.stage]);
+          wp.advance(2);
+          if (bprof) { prof_s[15] += (unsigned long long)(clock64() - tb); prof_s[7] += 1ull; }
+        } while (!last);
       }
       wsync();
+      if (is_issuer) feed();                           // every stage is free now: the first tiles of the next pass
+      // ---- CTA partial: the groups add their blocks in group order ----
+      for (int gg = 0; gg < NG; ++gg) {
+        if (grp == gg) {
+#pragma unroll
+          for (int s = 0; s < kNwtStrips; ++s) {
+            if (s < nstr) {
+#pragma unroll
+              for (int m = 0; m < kNwtStripLen; ++m) {
+                if (m < st_len[s]) {
+                  double *h = hred + (size_t)(st_blk[s] + m) * 64 + r8 * 8 + c2;
+                  if (gg == 0) { h[0] = acc[s][m][0]; h[1] = acc[s][m][1]; }
+                  else { h[0] += acc[s][m][0]; h[1] += acc[s][m][1]; }
+                }
+              }
+            }
+          }
+        }
+        wsync();
+      }
     }
     {
       const double fs = warp_sum_f64(f_acc);
@@ -346,7 +555,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master_newton(NewtonParam
     wsync();
     if (tid == 0) {
       double s = 0.0;
-      for (int w = 0; w < kNW; ++w) s += fred_s[w];
+      for (int w = 0; w < kNwtFront; ++w) s += fred_s[w];
       hred[nblocks * 64] = s;
     }
     wsync();
@@ -474,11 +683,11 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master_newton(NewtonParam
         if (!(dj > ridge)) dj = ridge;
         if (tid == 0) dpiv_s[j] = dj;
         const double inv = 1.0 / dj;
-        // trailing update: rows i in (j, nf], columns k in (j, min(i, nf - 1)]
-        const int nrow = nf - j;                           // rows j+1 .. nf
-        for (int e = tid; e < nrow * nrow; e += kMasterWorkers) {
-          const int i = j + 1 + e / nrow, k = j + 1 + e % nrow;
-          if (k <= i && k < nf) lbuf[lidx(i, k)] = fma(-lbuf[lidx(i, j)] * inv, lbuf[lidx(k, j)], lbuf[lidx(i, k)]);
+        // trailing update: rows i in (j, nf], columns k in (j, min(i, nf - 1)]; warp = rows, lane = columns
+        for (int i = j + 1 + warp; i <= nf; i += kNW) {
+          const double cij = -lbuf[lidx(i, j)] * inv;
+          for (int k = j + 1 + lane; k <= i && k < nf; k += 32)
+            lbuf[lidx(i, k)] = fma(cij, lbuf[lidx(k, j)], lbuf[lidx(i, k)]);
         }
         wsync();
       }
@@ -603,20 +812,20 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master_newton(NewtonParam
   wsync();
 
   // ---- publish ----
+  // drain: every issued stage must have landed before the CTA may exit
+  if (is_issuer) si[9] = issued_total;
+  wsync();
   if (tid == 0) {
-    s_consumed_stage = (unsigned)cp.stage;
-    s_consumed_phase = cp.phase;
-    __threadfence_block();
-    s_stop = 1;
+    for (const int n_issued = si[9]; consumed_total < n_issued; ++consumed_total) {
+      mbar_wait(&full[cp.stage], cp.phase);
+      cp.advance(NS);
+    }
   }
   if (blockIdx.x == 0) {
     if (tid < K) p.y[tid] = y_s[tid];
     if (tid == 0) {
       *p.epoch = red.ep;
       if (p.prof) {
-        prof_s[8] += (unsigned long long)iters;
-        prof_s[9] += 1ull;
-        prof_s[7] += (unsigned long long)passes;
         PROF_MARK(10);
         for (int i = 0; i < kMasterProfSlots; ++i) p.prof[i] += prof_s[i];
       }
@@ -651,7 +860,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master_newton(NewtonParam
     }
   }
 #undef PROF_MARK
-  __syncthreads();       // the producer warp joins after draining the ring
+  __syncthreads();       // nobody leaves before the ring is drained
 }
 
 // ------------------------------------------------------------------------------------------
@@ -659,7 +868,7 @@ __global__ void __launch_bounds__(kMasterThreads, 1) k_master_newton(NewtonParam
 // ------------------------------------------------------------------------------------------
 static size_t newton_fixed_smem(int32_t k_max, int32_t T, int32_t n_struct, int32_t n_red, int32_t lbuf_doubles) {
   return 128 + 128 + align_up((size_t)std::max(n_struct, 1) * sizeof(StructEntry), 128) + align_up((size_t)n_red * 8, 128) +
-         align_up((size_t)lbuf_doubles * 8, 128) + (size_t)kNwtZThreads * 8 + 2 * align_up((size_t)(T + 4) * 8, 128) +
+         align_up((size_t)lbuf_doubles * 8, 128) + 2 * align_up((size_t)(T + 4) * 8, 128) +
          align_up((size_t)(T + 8) * 2, 128);
 }
 
@@ -667,20 +876,26 @@ NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct) {
   NewtonLayout L;
   L.nb_max = (k_max + 1 + 7) / 8;
   L.n_red = L.nb_max * (L.nb_max + 1) / 2 * 64 + 8;
-  const int32_t lbuf = (k_max + 1) * (k_max + 2) / 2 + 8;
   // 227 KB opt-in maximum per CTA on sm_100; ~9 KB of static tables, 1 KB reserved by the system
   const size_t budget = (size_t)227 * 1024 - (size_t)10 * 1024;
-  static const int32_t cand[] = {256, 192, 128, 96, 64, 32};
-  for (int32_t T : cand) {
-    const int32_t TP = T + 4;
-    const int32_t stage = (int32_t)align_up((size_t)k_max * TP * 4, 128);
-    const size_t fixed = newton_fixed_smem(k_max, T, n_struct, L.n_red, lbuf);
-    if (fixed + (size_t)3 * stage > budget && T != 32) continue;
-    int32_t stages = 2;
-    while (stages < 6 && fixed + (size_t)(stages + 1) * stage <= budget) ++stages;
-    L.T = T; L.TP = TP; L.stage_bytes = stage; L.n_stages = stages;
-    L.smem = fixed + (size_t)stages * stage;
-    break;
+  static const int32_t cand_t[] = {256, 128, 64, 32};        // T x k-slices = 256 front threads
+  static const int32_t cand_ac[] = {64, 32, 16};
+  for (int32_t T : cand_t) {
+    for (int32_t AC : cand_ac) {
+      const int32_t lbuf = std::max((k_max + 1) * (k_max + 2) / 2 + 8, 2 * (8 * L.nb_max + 1) * (AC + 4));
+      const int32_t TP = T + 4;
+      const int32_t stage = (int32_t)align_up((size_t)k_max * TP * 4, 128);
+      const size_t fixed = newton_fixed_smem(k_max, T, n_struct, L.n_red, lbuf);
+      if (fixed + (size_t)kNwtMinStages * stage > budget && !(AC == 16 && T == 32)) continue;
+      if (AC == 16 && T > 32) continue;                      // rather a smaller tile than 4-quad chunks
+      int32_t stages = 2;
+      while (stages < 6 && fixed + (size_t)(stages + 1) * stage <= budget) ++stages;
+      L.T = T; L.TP = TP; L.stage_bytes = stage; L.n_stages = stages;
+      L.AC = AC; L.lbuf_doubles = lbuf;
+      L.smem = fixed + (size_t)stages * stage;
+      break;
+    }
+    if (L.T) break;
   }
   L.n_tiles = (n_vox_pad + L.T - 1) / L.T;
   L.tile_stride = (int64_t)k_max * L.TP;
@@ -693,7 +908,7 @@ cudaError_t newton_configure(Ctx *c) {
   cudaError_t e = cudaFuncSetAttribute(k_master_newton, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem);
   if (e != cudaSuccess) return e;
   int nbk = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nbk, k_master_newton, kMasterThreads, L.smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nbk, k_master_newton, kMasterWorkers, L.smem);
   if (e != cudaSuccess) return e;
   if (nbk < 1) return cudaErrorLaunchOutOfResources;
   return cudaSuccess;
@@ -707,7 +922,13 @@ cudaError_t launch_newton(Ctx *c, bool add_candidate) {
   p.T = L.T; p.TP = L.TP; p.tile_stride = L.tile_stride; p.n_tiles = L.n_tiles;
   p.n_stages = L.n_stages; p.stage_bytes = L.stage_bytes;
   p.n_red_cap = L.n_red;
-  p.lbuf_doubles = (c->opt.k_max + 1) * (c->opt.k_max + 2) / 2 + 8;
+  p.lbuf_doubles = L.lbuf_doubles;
+  p.AC = L.AC;
+  p.w_doubles = (8 * L.nb_max + 1) * (L.AC + 4);
+  p.srow = 8 * L.nb_max;
+  p.debug = c->opt.reserved >> 3;
+  p.ks_shift = 0;
+  while ((L.T << p.ks_shift) < kNwtFrontThreads) ++p.ks_shift;
   p.n_struct = std::max(c->n_struct, 1);
   p.sid = c->d.sid;
   p.vt = c->has_vt ? c->d.vt : nullptr;
@@ -726,7 +947,7 @@ cudaError_t launch_newton(Ctx *c, bool add_candidate) {
   p.k_max = c->opt.k_max;
   p.tol = c->opt.master_tol;
   void *args[] = {&p};
-  return cudaLaunchCooperativeKernel((void *)k_master_newton, dim3(c->master_grid), dim3(kMasterThreads), args, L.smem,
+  return cudaLaunchCooperativeKernel((void *)k_master_newton, dim3(c->master_grid), dim3(kMasterWorkers), args, L.smem,
                                      c->stream);
 }
 

@@ -254,7 +254,8 @@ static dao_status check_args(const dao_csr *D, const dao_mlc *mlc, const dao_str
   dm->n_vox = D->n_vox; dm->n_bl = D->n_bl; dm->nnz = D->nnz;
   dm->n_beams = mlc->n_beams; dm->n_rows = mlc->n_rows; dm->k_max = opt->k_max;
   dm->max_rows = std::max(max_rows, 1);
-  dm->master_method = opt->master_method;
+  // the projected-Newton master handles pools up to kNewtonMaxK apertures; larger pools use method 1
+  dm->master_method = (opt->master_method == 2 && opt->k_max > kNewtonMaxK) ? 1 : opt->master_method;
   dm->n_struct = s->n_struct;
   dm->chain_states = 0;
   if (opt->mlc_mode == DAO_MLC_INTERDIGITATION || opt->mlc_mode == DAO_MLC_CONNECTED) {
@@ -556,6 +557,7 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   Dims dm{};
   dao_status st = check_args(D, mlc, s, &c->opt, &dm, &c->err);
   if (st != DAO_OK) return st;
+  c->opt.master_method = dm.master_method;
   c->n_sm = query_sm_count(&c->device, &c->err);
   if (c->n_sm < 0) return DAO_E_CUDA;
   if (!workspace || !scratch || ((uintptr_t)workspace & 255) || ((uintptr_t)scratch & 255)) {
