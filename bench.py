@@ -92,22 +92,35 @@ def algorithmic_bytes(ph, sell_elems=None):
     }
 
 
+TRAFFIC_CSV = os.path.join("profiles", "r02_traffic.csv")   # one `ncu --set full` capture per kernel; see profiles/r02_traffic.md
+
+
 def ncu_traffic(kernel: str):
-    """DRAM bytes per launch of `kernel` from the newest profiles/*_traffic.csv (one `ncu --set full`
-    capture, see the .md beside it); None when no capture is committed."""
+    """DRAM bytes (read + write) of ONE captured launch of `kernel`, with what identifies that launch (pool size K,
+    passes over A), from TRAFFIC_CSV; None when the capture is not committed."""
     import csv
-    import glob
-    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv")))
-    if not files:
+    path = os.path.join(ROOT, TRAFFIC_CSV)
+    if not os.path.exists(path):
         return None
     try:
-        with open(files[-1]) as f:
+        with open(path) as f:
             for row in csv.DictReader(f):
                 if row["kernel"] == kernel:
-                    return int(row["dram_bytes_per_launch"])
+                    return {"dram_bytes": int(row["dram_bytes_per_launch"]), "K": int(row.get("K") or 0),
+                            "passes": int(row.get("passes") or 0), "pg_iterations": int(row.get("pg_iterations") or 0)}
     except Exception:
         pass
     return None
+
+
+def master_alg_bytes(method: int, V: int, K: int, n_iter: int, n_passes: int) -> float:
+    """Algorithmic bytes of one master solve.  Methods 0/1: per projected-gradient
+    iteration 2*4*V*K (two passes over A) + (n_ls + 3)*8*V with n_ls = the repeated gradient passes per iteration.
+    Method 2: every pass reads A once (4*V*K), reads sid (V) and writes the fp64 dose (8*V)."""
+    if method == 2:
+        return float(n_passes) * (4.0 * V * K + 9.0 * V)
+    n_ls = max(0, n_passes - (2 * n_iter + 1))
+    return n_iter * (2.0 * 4.0 * V * K + 3.0 * 8.0 * V) + n_ls * (4.0 * V * K + 8.0 * V)
 
 
 def reduce_max(x: float, world: int, device: str = "cuda") -> float:
@@ -127,32 +140,43 @@ def job_seconds_per_plan(elapsed_max: float, steps: int, world: int) -> float:
     return elapsed_max / (steps * world)
 
 
+def time_oracle(ph, n_ap):
+    """Seconds the oracle, as it stands (one host core), takes for the first n_ap column-generation iterations."""
+    from oracle import dao_oracle as orc
+    orc.build()
+    t0 = time.perf_counter()
+    plan = orc.run(ph, n_ap)
+    return time.perf_counter() - t0, plan
+
+
+def cpu_baseline_of(ph, args):
+    """The reported CPU baseline: ONE full plan of the oracle (about 140 s for cfg1 on one core), not an extrapolation;
+    --ref-apertures < apertures times a prefix instead and says so."""
+    n_ap = min(args.ref_apertures or N_APERTURES, N_APERTURES)
+    dt, plan = time_oracle(ph, n_ap)
+    full = n_ap == N_APERTURES
+    return {"value": dt if full else dt * N_APERTURES / n_ap, "unit": "s", "cores": 1, "kind": "oracle",
+            "objective": plan.objective,
+            "sample": (f"one full {N_APERTURES}-aperture plan of {ph.name} (measured, {dt:.1f} s, not extrapolated)" if full else
+                       f"first {n_ap} of {N_APERTURES} column-generation iterations ({dt:.1f} s) scaled by {N_APERTURES}/{n_ap}: "
+                       "an UNDER-estimate, later iterations carry larger master problems")}
+
+
 def run_reference(args, rank, world):
-    """The reference arm: the oracle, as it stands, on the host cores; bounded sample."""
+    """The reference arm: the oracle, as it stands, on the host cores.  One full plan per step; because a plan
+    takes minutes, --steps / --warmup above 1 / 0 are ignored (said in `sample`)."""
     if rank != 0:
         return
-    from oracle import dao_oracle as orc
     from paper_1003_5402_b200.inputs import phantom
-    orc.build()
     ph = phantom.make(args.config, 0)
-    n_ap = args.ref_apertures
-    times = []
-    for i in range(args.warmup + args.steps):
-        t0 = time.perf_counter()
-        orc.run(ph, n_ap)
-        dt = time.perf_counter() - t0
-        if i >= args.warmup:
-            times.append(dt)
-    per_plan = float(np.mean(times)) * N_APERTURES / n_ap
-    cpu = {"value": per_plan, "unit": "s", "cores": 1, "kind": "oracle",
-           "sample": f"first {n_ap} of {N_APERTURES} column-generation iterations of {ph.name}, time scaled by {N_APERTURES}/{n_ap} "
-                     "(later iterations carry larger master problems, so this under-states the full plan)"}
+    cpu = cpu_baseline_of(ph, args)
+    cpu["sample"] += "; --steps/--warmup ignored: 1 timed plan, no warm-up"
     print(json.dumps({
-        "impl": "reference", "metric": METRIC, "value": per_plan, "unit": "s", "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(times)),
+        "impl": "reference", "metric": METRIC, "value": cpu["value"], "unit": "s", "n_gpus": args.gpus,
+        "steps": 1, "warmup": 0, "ms_per_step": 1e3 * cpu["value"],
         "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_config(ph, args), "cpu_baseline": cpu,
-        "e2e": {"value": per_plan, "unit": "s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+        "e2e": {"value": cpu["value"], "unit": "s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
 def workload_config(ph, args):
@@ -298,7 +322,10 @@ def main():
     ap.add_argument("--config", default="cfg1")
     ap.add_argument("--impl", default="dao", choices=["dao", "reference"])
     ap.add_argument("--apertures", type=int, default=N_APERTURES, help="apertures per plan (50; configs[4] asks for 100)")
-    ap.add_argument("--ref-apertures", type=int, default=12, help="apertures per step of the reference arm / cpu_baseline")
+    ap.add_argument("--ref-apertures", type=int, default=0,
+                    help="apertures of the oracle run behind cpu_baseline / --impl reference (0 = the full plan; fewer = a scaled prefix)")
+    ap.add_argument("--master-method", type=int, default=2, help="dao_options.master_method (2 = projected Newton, 1 = conjugated gradient projection)")
+    ap.add_argument("--split-steps", type=int, default=2, help="plans of the separate per-kernel-class timing pass")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[3] kernel sweep (markdown table)")
@@ -343,8 +370,11 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    d = dao.Dao(ph, k_max=N_APERTURES)
+    # ---- timed region: K plans through dao_run, NO event timers inside the library ----
+    opts = dict(k_max=N_APERTURES, master_method=args.master_method)
+    d = dao.Dao(ph, timers=0, **opts)
     dims = d.dims()
+    method = int(d.opt.master_method)
     infos = []
     for _ in range(args.warmup):
         d.reset()
@@ -365,58 +395,110 @@ def main():
     sec_per_plan = job_seconds_per_plan(elapsed, args.steps, world)   # N replicas produce N plans per step
     last = infos[-1]
     n_it = sum(i.n_iterations for i in infos)
+    launches = sum(i.n_kernel_launches for i in infos)
+    d.close()
 
-    # ---- per-kernel-class device time (CUDA events on the launching stream, inside dao_run) ----
+    # ---- per-kernel-class split: a separate pass with the library's CUDA-event timers on (same kernels, same plan;
+    #      the events cost a few us per iteration, which is why they are not in the timed region) ----
+    dt_ = dao.Dao(ph, timers=1, **opts)
+    dt_.run(N_APERTURES)
+    tinfos = []
+    for _ in range(max(1, args.split_steps)):
+        dt_.reset()
+        tinfos.append(dt_.run(N_APERTURES))
+    hist = dt_.get_vector(dao.VEC_HISTORY)[:tinfos[-1].n_apertures]
+    it_sec = dt_.get_vector(dao.VEC_ITER_SECONDS).reshape(-1, 6)[:tinfos[-1].n_iterations]
+    dt_.close()
+    n_it_t = sum(i.n_iterations for i in tinfos)
     ab = algorithmic_bytes(ph)
     classes = {"intensity": "seconds_intensity", "spmv": "seconds_spmv", "spmv_t": "seconds_spmv_t",
                "price": "seconds_price", "column": "seconds_column", "master": "seconds_master"}
-    tot = {k: sum(getattr(i, f) for i in infos) for k, f in classes.items()}
+    tot = {k: sum(getattr(i, f) for i in tinfos) for k, f in classes.items()}
     tsum = sum(tot.values())
     kernels = {}
     for k in classes:
-        avg = tot[k] / max(1, n_it)
+        avg = tot[k] / max(1, n_it_t)
         kernels[k] = {"avg_us": 1e6 * avg, "share": tot[k] / tsum if tsum > 0 else None}
         if k in ab and avg > 0:
             gbs = ab[k] / avg * 1e-9
             kernels[k].update({"alg_bytes": ab[k], "GBps": gbs, "frac_of_hbm_peak": gbs / peak})
-    # master: bytes the projected-gradient loop must move: 2 passes over the dense block per iteration
-    pg_total = sum(i.n_pg_iter_total for i in infos)
-    hist = d.get_vector(dao.VEC_HISTORY)[:last.n_apertures]
-    master_bytes_plan = float(sum(int(h["n_pg_iter"]) * (2 * 4 * ph.n_vox * int(h["k"]) + 3 * 17 * ph.n_vox) for h in hist))
-    kernels["master"].update({"pg_iterations_per_plan": pg_total / args.steps, "alg_bytes_per_plan": master_bytes_plan,
-                              "GBps": master_bytes_plan * args.steps / tot["master"] * 1e-9 if tot["master"] > 0 else None,
-                              "note": "dense block A (4*V*K bytes <= L2) is L2-resident: GB/s is not an HBM figure"})
+
+    # ---- the master: algorithmic bytes per solve from the per-iteration history, split by where A lives ----
+    V = ph.n_vox
+    l2_bytes = int(torch.cuda.get_device_properties(local_rank).L2_cache_size)
+    vpad = (V + 127) // 128 * 128
+    solves = []
+    for h, sec in zip(hist, it_sec):
+        K = int(h["k"])
+        solves.append({"K": K, "bytes": master_alg_bytes(method, V, K, int(h["n_pg_iter"]), int(h["n_passes"])),
+                       "s": float(sec[5]), "passes": int(h["n_passes"]), "iters": int(h["n_pg_iter"]),
+                       "regime": "hbm" if 4.0 * vpad * K >= 0.8 * l2_bytes else "l2"})
+    master_bytes_plan = sum(x["bytes"] for x in solves)
+    master_s_plan = sum(x["s"] for x in solves)
+    regimes = {}
+    for r in ("l2", "hbm"):
+        sel = [x for x in solves if x["regime"] == r]
+        if sel:
+            bsum, ssum = sum(x["bytes"] for x in sel), sum(x["s"] for x in sel)
+            regimes[r] = {"solves": len(sel), "K_range": [min(x["K"] for x in sel), max(x["K"] for x in sel)],
+                          "alg_bytes": bsum, "seconds": ssum, "achieved_GBps": bsum / ssum * 1e-9 if ssum > 0 else None,
+                          "share_of_master_time": ssum / master_s_plan if master_s_plan > 0 else None}
+    if "l2" in regimes:
+        regimes["l2"].update({"peak": None, "note": "4*V*K fits the L2: L2-bandwidth regime, no measured L2 peak on this pool"})
+    if "hbm" in regimes:
+        regimes["hbm"].update({"peak": peak, "frac": regimes["hbm"]["achieved_GBps"] / peak})
+    kernels["master"].update({
+        "method": method, "iterations_per_plan": sum(x["iters"] for x in solves), "passes_over_A_per_plan": sum(x["passes"] for x in solves),
+        "alg_bytes_per_plan": master_bytes_plan, "GBps": master_bytes_plan / master_s_plan * 1e-9 if master_s_plan > 0 else None,
+        "regimes": regimes})
     plan_bytes = N_APERTURES * (ab["spmv"] + ab["spmv_t"] + ab["price"] + ab["column"]) + master_bytes_plan
-    # `roofline` describes the kernel that dominates the step (k_master, ~90 % of a plan); the SpMV-class kernels the
-    # metric names are in `roofline_kernels`.  achieved = algorithmic bytes per launch / average launch duration
-    # (CUDA events on the launching stream inside dao_run); peak = measured HBM copy bandwidth.
-    n_master = max(1, n_it)
-    master_alg_per_launch = master_bytes_plan * args.steps / n_master
-    master_avg = tot["master"] / n_master
-    master_gbs = master_alg_per_launch / master_avg * 1e-9 if master_avg > 0 else None
-    roofline = {"kernel": "k_master (restricted master problem: projected gradient over the dense block A)",
-                "bound": "hbm", "achieved": master_gbs, "peak": peak, "unit": "GB/s",
-                "frac": master_gbs / peak if master_gbs else None, "traffic": ncu_traffic("k_master"),
-                "peak_source": peak_src, "alg_bytes_per_launch": master_alg_per_launch,
-                "alg_bytes_model": "per projected-gradient iteration 2 passes over A (2*4*V*K) + 3 passes over z, dz, sid (3*17*V)",
-                "avg_launch_us": 1e6 * master_avg, "share_of_step": kernels["master"]["share"],
-                "note": "alg_bytes_per_launch is the average over the solves of a plan (K = 1..50); traffic is the ncu DRAM "
-                        "figure of ONE late solve (K = 47, profiles/r01d_ncu_full.md).  While 4*V*K is well below the 126 MB L2 "
-                        "(K <~ 40 here) the block is L2-resident and a solve reads ~70 MB from DRAM; late in the plan it "
-                        "streams from HBM and DRAM traffic equals the algorithmic bytes"}
+
+    master_kernel = "k_master_newton" if method == 2 else "k_master"
+    master_model = ("per pass over A: 4*V*K (A read once) + V (sid) + 8*V (fp64 dose written); a solve makes `passes` passes"
+                    if method == 2 else
+                    "SURVEY 8(d): per projected-gradient iteration 2*4*V*K + (n_ls+3)*8*V, n_ls = repeated gradient passes")
+
+    def traffic_of(kernel, alg_of_launch):
+        """ncu DRAM bytes of ONE captured launch next to the algorithmic bytes of that same launch."""
+        t = ncu_traffic(kernel)
+        if t is None:
+            return None, None
+        return t["dram_bytes"], {"source": TRAFFIC_CSV, "launch": {k: v for k, v in t.items() if k != "dram_bytes" and v},
+                                 "alg_bytes_of_that_launch": alg_of_launch(t),
+                                 "dram_over_alg": t["dram_bytes"] / alg_of_launch(t) if alg_of_launch(t) else None}
 
     def class_roofline(key, kernel_name, label):
         k = kernels[key]
+        tr, trd = traffic_of(kernel_name, lambda t: ab[key])
         return {"kernel": label, "bound": "hbm", "achieved": k.get("GBps"), "peak": peak, "unit": "GB/s",
                 "frac": k.get("frac_of_hbm_peak"), "frac_of_nominal_8000": (k.get("GBps") or 0.0) / 8000.0,
-                "traffic": ncu_traffic(kernel_name), "alg_bytes_per_launch": ab[key],
-                "avg_launch_us": k["avg_us"], "share_of_step": k["share"]}
+                "traffic": tr, "traffic_detail": trd, "alg_bytes_per_launch": ab[key],
+                "avg_launch_us": k["avg_us"], "share_of_step": k["share"], "peak_source": peak_src}
 
     roofline_kernels = {
         "spmv": class_roofline("spmv", "k_spmv_ring<0>", "k_spmv_ring<0> (dose SpMV + fused objective/gradient)"),
         "spmv_t": class_roofline("spmv_t", "k_spmvt", "k_spmvt + k_spmvt_finish (w = D^T pi)"),
         "column": class_roofline("column", "k_spmv_ring<2>", "k_spmv_ring<2> (aperture column a_K = D 1_A)"),
         "sell_padding": dims.sell_elems / max(1, ph.nnz)}
+    # the master's roofline object: the HBM regime when the plan has one (A streams from DRAM), else the L2 regime
+    hb = regimes.get("hbm")
+    head = hb or regimes.get("l2") or {}
+    mtr, mtrd = traffic_of(master_kernel, lambda t: master_alg_bytes(method, V, t["K"], t["pg_iterations"], t["passes"]))
+    n_head = max(1, head.get("solves", 1))
+    master_roofline = {
+        "kernel": f"{master_kernel} (restricted master problem over the dense block A, method {method})",
+        "bound": "hbm" if hb else "l2", "achieved": head.get("achieved_GBps"), "peak": peak if hb else None, "unit": "GB/s",
+        "frac": hb["frac"] if hb else None, "traffic": mtr, "traffic_detail": mtrd, "peak_source": peak_src,
+        "alg_bytes_per_launch": head.get("alg_bytes", 0.0) / n_head, "avg_launch_us": 1e6 * head.get("seconds", 0.0) / n_head,
+        "alg_bytes_model": master_model, "share_of_step": kernels["master"]["share"],
+        "regime": (f"solves with 4*V_pad*K >= 0.8 x L2 ({l2_bytes >> 20} MB): K = {hb['K_range'][0]}..{hb['K_range'][1]}, "
+                   f"{100 * hb['share_of_master_time']:.0f} % of the master's time; the other solves are L2-resident (see regimes)"
+                   if hb else "every solve is L2-resident: no HBM figure, no measured L2 peak"),
+        "regimes": regimes}
+    shares = {k: (kernels[k]["share"] or 0.0) for k in kernels}
+    dominant = max(shares, key=shares.get)
+    roofline = master_roofline if dominant == "master" else roofline_kernels[dominant]
+    roofline["dominant_class"] = dominant
 
     # ---- e2e: host (pinned) buffers -> dao_create -> dao_run -> dao_get_plan, wall clock ----
     e2e = None
@@ -428,7 +510,7 @@ def main():
         for i in range(args.e2e_steps + 1):
             barrier()
             t0 = time.perf_counter()
-            with dao.Dao(php, k_max=N_APERTURES) as d2:
+            with dao.Dao(php, timers=0, **opts) as d2:
                 inf = d2.run(N_APERTURES)
                 plan = d2.get_plan()
                 d2h = int(plan.beams.nbytes + plan.intensity.nbytes + plan.ap_row_ptr.nbytes + plan.left.nbytes +
@@ -439,38 +521,34 @@ def main():
         e = float(np.mean(ts))
         e = reduce_max(e, world)
         e2e = {"value": e / world, "unit": "s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-               "includes": "dao_create from pinned host CSR (H2D + sliced-ELL + transpose build), dao_run(50), dao_get_plan"}
+               "includes": f"dao_create from pinned host CSR (H2D + sliced-ELL + transpose build), dao_run({N_APERTURES}), dao_get_plan"}
 
-    # ---- CPU baseline: the oracle as it stands, bounded sample, rank 0, N = 1 only ----
+    # ---- CPU baseline: the oracle as it stands, one full plan, rank 0, N = 1 only ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        from oracle import dao_oracle as orc
-        orc.build()
-        n_ap = args.ref_apertures
-        t0 = time.perf_counter()
-        orc.run(ph, n_ap)
-        dt = time.perf_counter() - t0
-        cpu = {"value": dt * N_APERTURES / n_ap, "unit": "s", "cores": 1, "kind": "oracle",
-               "sample": f"first {n_ap} of {N_APERTURES} column-generation iterations ({dt:.1f} s), scaled by {N_APERTURES}/{n_ap}; "
-                         "later iterations carry larger master problems, so the full plan takes longer"}
+        cpu = cpu_baseline_of(ph, args)
 
     if rank == 0:
-        launches_per_plan = sum(i.n_iterations for i in infos) / args.steps * 10 + 2
         out = {"metric": METRIC, "value": sec_per_plan, "unit": "s", "n_gpus": world, "steps": args.steps,
                "warmup": args.warmup, "ms_per_step": 1e3 * elapsed / args.steps, "higher_is_better": False,
-               "scaling": "weak", "vs_baseline": None, "dtype": "f64", "storage_dtype": "f32/int32", "data": "synthetic",
+               "scaling": "weak", "vs_baseline": None, "dtype": "f32 storage, f64 accumulate", "data": "synthetic",
                "config": workload_config(ph, args), "clocks": clocks, "e2e": e2e,
-               "gpu_launches": int(launches_per_plan * args.steps), "roofline": roofline, "roofline_kernels": roofline_kernels, "cpu_baseline": cpu,
-               "kernels": kernels,
+               "gpu_launches": int(launches), "roofline": roofline, "roofline_kernels": roofline_kernels,
+               "roofline_master": master_roofline, "cpu_baseline": cpu, "kernels": kernels,
                "plan": {"objective": last.objective, "apertures": last.n_apertures, "cg_iterations_per_s": n_it / elapsed,
-                        "pg_iterations": int(last.n_pg_iter_total), "converged": int(last.converged),
+                        "master_iterations": int(last.n_pg_iter_total), "master_passes_over_A": int(last.n_passes_total),
+                        "master_hit_max_iter": int(last.n_hit_max_iter), "converged": int(last.converged),
+                        "duplicates": int(last.n_duplicates), "kernel_launches_per_plan": int(last.n_kernel_launches),
                         "bytes_moved_roofline_s": plan_bytes / (peak * 1e9),
                         "frac_of_bytes_moved_roofline": plan_bytes / (peak * 1e9) / (elapsed / args.steps),
+                        "bytes_model": "sum over iterations of the SURVEY 8(d) bytes of the three SpMV-class kernels and pricing + the "
+                                       "master's algorithmic bytes (roofline_master.alg_bytes_model), all over the measured HBM peak",
                         "master_tol": d.opt.master_tol, "master_max_iter": d.opt.master_max_iter,
-                        "master_method": d.opt.master_method},
+                        "master_method": method},
+               "timers": "value / ms_per_step: dao_run with timers = 0; kernels / roofline*: a separate pass with the library's "
+                         "CUDA-event timers on",
                "paper_context": "0.7-2.5 s per 50-aperture plan on a Tesla C1060 for ~20x smaller clinical cases (PAPER.md:202)"}
         print(json.dumps(out))
-    d.close()
     if world > 1:
         dist.destroy_process_group()
 

@@ -126,7 +126,8 @@ typedef struct {
                                 steepest-descent direction (default 1e-7); reading S2 */
   double price_tol;          /* optimal iff price_b* >= -price_tol * max_i |w_i| * (rows in b*) (default 1e-6, the
                                 fp32 noise floor of w), or iff the best candidate duplicates an aperture of the
-                                pool (its negative price is then residue of the master solve); S3, S6 */
+                                pool after a CONVERGED master solve whose KKT residual explains the price (the
+                                negative price is then residue of that solve); S3, S6 */
   double master_ls_tol;      /* a step t along the search direction is accepted when |phi'(t)| <= master_ls_tol *
                                 |phi'(0)| (phi(t) = F(z + t dz)) or when it ends on a bound still descending;
                                 otherwise t is refined by a safeguarded Newton search (default 0.01); S2 */
@@ -159,6 +160,10 @@ typedef struct {
   double w_abs_max;          /* max_i |w_i| (used by the optimality test) */
   int32_t n_open_beamlets;   /* beamlets opened by the candidate */
   int32_t duplicate;         /* 1: the candidate equals an aperture already in the pool (reading S6) */
+  int32_t stalled;           /* 1: the candidate is a duplicate with an improving price after a master solve that did
+                                not converge (or whose residue does not explain the price): no candidate is stored and
+                                optimality is NOT claimed (converged = 0); solve the master further and price again */
+  int32_t reserved;
 } dao_price_info;
 
 typedef struct {
@@ -185,6 +190,8 @@ typedef struct {
   double seconds_intensity, seconds_spmv, seconds_spmv_t, seconds_price, seconds_column, seconds_master;
   int64_t n_passes_total;    /* passes over the aperture-dose block A made by the master solves of this call */
   int32_t n_hit_max_iter;    /* master solves of this call that stopped on master_max_iter */
+  int32_t n_kernel_launches; /* kernels this call launched (counted at the launch sites of the library) */
+  int32_t stalled;           /* 1: stopped on a duplicate candidate after an unconverged master solve (S6): converged = 0 */
   int32_t reserved;
 } dao_run_info;
 
@@ -224,6 +231,9 @@ typedef enum {               /* dao_get_vector selectors; lengths in elements */
   DAO_VEC_BEAM_PRICE = 8,    /* double [n_beams] */
   DAO_VEC_HISTORY = 9,       /* dao_iter_record [k_max] (first n_apertures valid) */
   DAO_VEC_MASTER_Z = 10,     /* double [n_vox]  z = A y as the master holds it, caller's voxel order */
+  DAO_VEC_ITER_SECONDS = 12, /* double [k_max][6]  HOST only: device seconds of every column-generation iteration of the last
+                                dao_run per kernel class {intensity, dose SpMV, SpMV^T, pricing, column, master}
+                                (CUDA events; zeros when options.timers == 0 and beyond the iterations run) */
   DAO_VEC_MASTER_PHASES = 11 /* uint64 [16]     phase timers of the master kernel, accumulated since dao_create when
                                 dao_options.reserved has bit 1 (value 2) set, else zeros.  Nanoseconds of CTA 0 in:
                                 0 set-up and z = A y, 1 gradient pass over A, 2 gradient reduction, 3 direction,

@@ -310,6 +310,8 @@ class Plan:
     y: np.ndarray = field(default_factory=lambda: np.zeros(0))
     objective: float = float("nan")
     converged: bool = False
+    stalled: bool = False          # stopped on a duplicate candidate after an unconverged master (reading S6)
+    n_duplicates: int = 0
     history: List[Iteration] = field(default_factory=list)
     A: Optional[np.ndarray] = None
 
@@ -321,9 +323,17 @@ def price_converged(pr: Pricing, w, beam_row_ptr, price_tol: float) -> bool:
 
 
 def run(ph, max_apertures: int, master_tol: float = 1e-10, master_max_iter: int = 20000,
-        price_tol: float = 1e-9, method: str = "newton", keep_A: bool = False, mlc: str = "consecutive") -> Plan:
+        price_tol: float = 1e-9, method: str = "newton", keep_A: bool = False, mlc: str = "consecutive",
+        stop_on_duplicate: bool = True) -> Plan:
     """O9: the column-generation loop.  `ph` is any object with the Phantom fields.  mlc = "consecutive"
-    (the paper's experiments) or "jaws" (jaws-only delivery, reading J1)."""
+    (the paper's experiments) or "jaws" (jaws-only delivery, reading J1).
+
+    stop_on_duplicate (reading S6; the paper is silent): a candidate that equals an aperture k of the
+    pool has the reduced cost dF/dy_k of the master, >= 0 at the master's optimum, so its negative price is residue
+    of the master solve and, being the minimum over all apertures, bounds every other reduced cost.  The loop then
+    stops: `converged` if that master solve met its stopping test and the residue is of the size the solve reports
+    (-price <= 10 max(kkt, price tolerance)), `stalled` otherwise (appending the same column again cannot help).
+    With the default tolerances (1e-10) the rule never fires; False appends the duplicate (SURVEY's first reading)."""
     vp = voxel_params_of(ph)
     n_vox, n_bl = ph.n_vox, ph.n_bl
     A = np.zeros((max_apertures, n_vox), dtype=np.float64)
@@ -346,6 +356,16 @@ def run(ph, max_apertures: int, master_tol: float = 1e-10, master_max_iter: int 
         b = pr.best_beam
         r0, r1 = int(ph.beam_row_ptr[b]), int(ph.beam_row_ptr[b + 1])
         le, ri = pr.left[r0:r1].copy(), pr.right[r0:r1].copy()
+        if stop_on_duplicate and any(pb == b and np.array_equal(pl, le) and np.array_equal(prr, ri)
+                                     for pb, pl, prr in zip(plan.beams, plan.lefts, plan.rights)):
+            plan.n_duplicates += 1
+            last = plan.history[-1]
+            tol_abs = price_tol * float(np.max(np.abs(w))) * (r1 - r0)
+            if last.n_master_iter < master_max_iter and -pr.price <= 10.0 * max(last.kkt, tol_abs):
+                plan.converged = True
+            else:
+                plan.stalled = True
+            break
         A[it] = aperture_column(ph.row_ptr, ph.col_idx, ph.val,
                                 aperture_open_mask(n_bl, b, le, ri, ph.beam_row_ptr, ph.row_bl_ptr))
         y = np.r_[y, 0.0]

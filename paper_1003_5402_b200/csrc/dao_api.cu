@@ -195,7 +195,8 @@ dao_status dao_price(dao_ctx *ctx, dao_price_info *out) {
   c->objective = h.F;
   if (out) {
     out->beam = h.cand_beam;
-    out->converged = h.done;
+    out->converged = h.done == 1 ? 1 : 0;
+    out->stalled = h.done == 2 ? 1 : 0;
     out->price = h.cand_price;
     out->objective = h.F;
     out->w_abs_max = h.w_abs_max;
@@ -262,7 +263,10 @@ dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out) {
   const int32_t dup0 = c->h_state->n_duplicates;
   const int64_t pass0 = c->h_state->pass_total;
   const int32_t hit0 = c->h_state->n_hit_max;
+  const int64_t launches0 = c->n_launches;
   double acc[6] = {0, 0, 0, 0, 0, 0};
+  int n_resolve = 0;
+  c->iter_seconds.clear();
   while (c->K < max_apertures) {
     if (timers) API_CUDA(cudaEventRecord(c->ev[0], c->stream));
     API_CUDA(launch_intensity(c));
@@ -289,9 +293,18 @@ dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out) {
         float ms = 0.f;
         API_CUDA(cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]));
         acc[i] += ms * 1e-3;
+        c->iter_seconds.push_back(ms * 1e-3);
       }
     }
-    if (c->h_state->done) { info.converged = 1; break; }
+    if (c->h_state->done == 2 && n_resolve < 2 && c->K > 0) {
+      // stalled on a duplicate after an unconverged master (S6): solve the master further, then price again
+      ++n_resolve;
+      API_CUDA(launch_master(c, false));
+      st = read_state(c);
+      if (st != DAO_OK) return st;
+      continue;
+    }
+    if (c->h_state->done) { info.converged = c->h_state->done == 1 ? 1 : 0; info.stalled = c->h_state->done == 2 ? 1 : 0; break; }
     if (c->K == k_before) break;        // nothing was added (pool full)
   }
   // final dose evaluation of the returned plan (steps 1-3)
@@ -309,6 +322,7 @@ dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out) {
   info.n_pg_iter_total = c->h_state->pg_iter_total - pg0;
   info.n_passes_total = c->h_state->pass_total - pass0;
   info.n_hit_max_iter = c->h_state->n_hit_max - hit0;
+  info.n_kernel_launches = (int32_t)(c->n_launches - launches0);
   info.objective = c->h_state->F;
   info.seconds_total = ms * 1e-3;
   info.seconds_intensity = acc[0]; info.seconds_spmv = acc[1]; info.seconds_spmv_t = acc[2];
@@ -381,6 +395,13 @@ dao_status dao_get_vector(dao_ctx *ctx, int32_t which, void *dst, dao_memspace m
     case DAO_VEC_BEAM_PRICE: src = c->d.beam_price; bytes = (size_t)c->n_beams * 8; break;
     case DAO_VEC_MASTER_PHASES: src = c->d.m_prof; bytes = (size_t)kMasterProfSlots * 8; break;
     case DAO_VEC_HISTORY: src = c->d.history; bytes = (size_t)c->opt.k_max * sizeof(dao_iter_record); break;
+    case DAO_VEC_ITER_SECONDS: {                          // host-resident: filled by dao_run from its CUDA events
+      if (mem != DAO_MEM_HOST) return fail(c, DAO_E_ARG, "DAO_VEC_ITER_SECONDS is host data");
+      double *out = reinterpret_cast<double *>(dst);
+      const size_t n = (size_t)c->opt.k_max * 6;
+      for (size_t i = 0; i < n; ++i) out[i] = i < c->iter_seconds.size() ? c->iter_seconds[i] : 0.0;
+      return DAO_OK;
+    }
     default: return fail(c, DAO_E_ARG, "unknown vector selector");
   }
   API_CUDA(cudaMemcpyAsync(dst, src, bytes, mem == DAO_MEM_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, c->stream));

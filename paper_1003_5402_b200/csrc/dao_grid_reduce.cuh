@@ -115,6 +115,57 @@ struct Reducer {
     }
     wsync();
   }
+  // Same result as large() for many values (the Hessian of the Newton master): CTA c owns the CONTIGUOUS range
+  // [c m, (c + 1) m), m = ceil(n / grid), so that what it gathers from every other CTA is one contiguous run of
+  // slots (coalesced) instead of m scattered ones.  Warp w sums the sources w, w + 16, ... in that order, then
+  // the warps are added in order.  scratch: >= kNW * m doubles of shared memory.  vals and out may alias.
+  __device__ __noinline__ void ranges(int n, const double *vals, double *out, double *scratch) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int grid = (int)gridDim.x;
+    ++ep;
+    uint4 *buf = part + (size_t)(ep & 1u) * grid * stride;
+    uint4 *res = result + (size_t)(ep & 1u) * stride;
+    for (int i = tid; i < n; i += kMasterWorkers) ll_store(buf + (size_t)blockIdx.x * stride + i, vals[i], ep);
+    const int m = (n + grid - 1) / grid;
+    const int lo = (int)blockIdx.x * m;
+    const int cnt = max(0, min(m, n - lo));
+    for (int l0 = 0; l0 < cnt; l0 += 32) {
+      const int l = l0 + lane;
+      if (l < cnt) {
+        double s = 0.0;
+        const uint4 *src = buf + lo + l;
+        for (int b0 = warp; b0 < grid; b0 += kNW * 5) {
+          uint4 w[5];
+#pragma unroll
+          for (int j = 0; j < 5; ++j) {
+            const int b = b0 + j * kNW;
+            if (b < grid) w[j] = ll_load(src + (size_t)b * stride);
+          }
+#pragma unroll
+          for (int j = 0; j < 5; ++j) {
+            const int b = b0 + j * kNW;
+            if (b < grid) {
+              while (w[j].y != ep || w[j].w != ep) w[j] = ll_load(src + (size_t)b * stride);
+              s += ll_value(w[j]);
+            }
+          }
+        }
+        scratch[warp * m + l] = s;
+      }
+    }
+    wsync();
+    for (int l = tid; l < cnt; l += kMasterWorkers) {
+      double t = 0.0;
+      for (int w = 0; w < kNW; ++w) t += scratch[w * m + l];
+      ll_store(res + lo + l, t, ep);
+    }
+    for (int i = tid; i < n; i += kMasterWorkers) {
+      uint4 w = ll_load(res + i);
+      while (w.y != ep || w.w != ep) w = ll_load(res + i);
+      out[i] = ll_value(w);
+    }
+    wsync();
+  }
 };
 
 // ---- the A stream of the master kernels: ring position, mbarrier helpers --------------------------

@@ -75,7 +75,7 @@ struct NewtonLayout {
 struct DevState {
   // pool
   int32_t K;               // apertures in the pool
-  int32_t done;            // 1: pricing proved optimality
+  int32_t done;            // 1: pricing proved optimality; 2: stalled on a duplicate candidate after an unconverged master
   // pending candidate (result of the last pricing)
   int32_t cand_valid;
   int32_t cand_beam;
@@ -239,6 +239,8 @@ struct Ctx {
   bool have_candidate = false;
   double objective = 0.0;
   cudaEvent_t ev[8] = {};
+  int64_t n_launches = 0;       // kernels launched on the hot path since dao_create (dao_run reports the difference)
+  std::vector<double> iter_seconds;   // [iterations of the last dao_run][6]: per kernel class, when options.timers != 0
   std::string err;
 };
 

@@ -822,6 +822,7 @@ cudaError_t launch_master(Ctx *c, bool add_candidate) {
   p.tol = c->opt.master_tol;
   p.ls_tol = c->opt.master_ls_tol;
   void *args[] = {&p};
+  ++c->n_launches;
   return cudaLaunchCooperativeKernel((void *)k_master, dim3(c->master_grid), dim3(kMasterThreads), args,
                                      c->master_smem, c->stream);
 }

@@ -89,6 +89,16 @@ __device__ __forceinline__ double cvt_pos(float x) {
   return __longlong_as_double((long long)r);
 }
 
+// 1 / d for a normal d > 0: hardware seed + two Newton steps (full fp64 accuracy to ~1 ulp, deterministic); the
+// IEEE division the compiler emits is a ~30-instruction sequence with a slow path, on the critical path of every pivot
+__device__ __forceinline__ double rcp_f64(double d) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+  r = fma(r, fma(-d, r, 1.0), r);
+  r = fma(r, fma(-d, r, 1.0), r);
+  return r;
+}
+
 __device__ __forceinline__ double lds_f64(uint32_t addr) {
   double v;
   asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
@@ -122,7 +132,8 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
   __shared__ double ytr_s[DAO_MAX_APERTURES];      // trial point of the current pass
   __shared__ double d_s[DAO_MAX_APERTURES];        // Newton direction
   __shared__ double grad_s[DAO_MAX_APERTURES];     // gradient at the accepted point
-  __shared__ double dpiv_s[DAO_MAX_APERTURES + 1]; // pivots of the LDL^T factorisation
+  __shared__ double dpiv_s[DAO_MAX_APERTURES + 1]; // reciprocals of the pivots of the LDL^T factorisation (an fp64
+                                                   // division is ~30 instructions: one per pivot, not one per use)
   __shared__ double xs_s[DAO_MAX_APERTURES + 1];   // solution on the free set
   __shared__ int fr_s[DAO_MAX_APERTURES];          // free variables
   __shared__ unsigned short strip_s[kNwtMaxStrips];  // strip -> (I << 8) | J0, longest strips first
@@ -559,17 +570,23 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
       hred[nblocks * 64] = s;
     }
     wsync();
-    red.large(n_red, hred, hred);
+    red.ranges(n_red, hred, hred, lbuf);             // the W tiles (= lbuf) are idle between passes
     PROF_MARK(2);
   };
 
-  // ---- first pass: everything at the warm start (previous optimum, new column at 0) ----
-  pass(y_s);
-  int passes = 1, iters = 0, hit_max = 0, nbt = 0, stall = 0;
-  bool have_dir = false;
-  double F = hred[nblocks * 64], t_step = 0.0, slope0 = 0.0, kkt = 0.0, pgmax = 0.0;
+  // ---- the first pass evaluates everything at the warm start (previous optimum, new column at 0), every later
+  //      one at a trial point.  pass() has ONE call site: inlined several times the kernel outgrew the instruction
+  //      cache and everything that runs once per iteration ran from L2 (5x slower, measured). ----
+  int passes = 0, iters = 0, hit_max = 0, nbt = 0, stall = 0;
+  bool have_dir = false, restoring = false;
+  double F = 0.0, t_step = 0.0, slope0 = 0.0, kkt = 0.0, pgmax = 0.0;
+  const double *cur = y_s;
 
   for (;;) {
+    pass(cur);
+    ++passes;
+    if (passes == 1) F = hred[nblocks * 64];
+    if (restoring) have_dir = false;
     // ================= decision on the pass just made (warp 0; identical in every CTA) =================
     if (warp == 0) {
       const double F_t = hred[nblocks * 64];
@@ -600,15 +617,14 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
     if (verdict == 0) {                                    // same direction, shorter step
       t_step = sc[0];
       ++nbt;
-      pass(ytr_s);
-      ++passes;
+      cur = ytr_s;
       continue;
     }
     if (verdict == 2) {                                    // no acceptable step: restore z = A y and stop
       hit_max = 1;
-      pass(y_s);
-      ++passes;
-      have_dir = false;
+      restoring = true;
+      cur = y_s;
+      continue;
     }
     if (have_dir) {
       const double F_t = hred[nblocks * 64];
@@ -678,19 +694,73 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
         }
       }
       wsync();
-      for (int j = 0; j < nf; ++j) {
-        double dj = lbuf[lidx(j, j)];
-        if (!(dj > ridge)) dj = ridge;
-        if (tid == 0) dpiv_s[j] = dj;
-        const double inv = 1.0 / dj;
-        // trailing update: rows i in (j, nf], columns k in (j, min(i, nf - 1)]; warp = rows, lane = columns
-        for (int i = j + 1 + warp; i <= nf; i += kNW) {
-          const double cij = -lbuf[lidx(i, j)] * inv;
-          for (int k = j + 1 + lane; k <= i && k < nf; k += 32)
-            lbuf[lidx(i, k)] = fma(cij, lbuf[lidx(k, j)], lbuf[lidx(i, k)]);
+      PROF_MARK(8);
+      if (prof) ++prof_s[10];
+      // Blocked right-looking LDL^T, 8 columns per step and 3 barriers per step (a barrier per column was
+      // measured at ~0.4 us each, 20 us for 50 columns).  Column j keeps the unscaled c_ij = l_ij d_j.
+      constexpr int RB = 8;
+      for (int jb = 0; jb < nf; jb += RB) {
+        const int r = min(RB, nf - jb);
+        // (1) the diagonal block, rows jb .. jb + r - 1: warp 0, one lane per (row, column) pair below the pivot
+        if (warp == 0) {
+          int a = 0;
+          while ((a + 1) * (a + 2) / 2 <= lane) ++a;
+          const int b = lane - a * (a + 1) / 2;            // lane -> (a, b), 0 <= b <= a: a pair below the pivot
+          for (int q = 0; q < r; ++q) {
+            const int j = jb + q;
+            double dj = lbuf[lidx(j, j)];
+            if (!(dj > ridge)) dj = ridge;
+            const double inv = rcp_f64(dj);
+            if (lane == 0) dpiv_s[j] = inv;
+            if (a < r - q - 1) {                           // rows of the block below the pivot
+              const int i = j + 1 + a, k = j + 1 + b;
+              lbuf[lidx(i, k)] = fma(-lbuf[lidx(i, j)] * inv, lbuf[lidx(k, j)], lbuf[lidx(i, k)]);
+            }
+            __syncwarp();
+          }
+        }
+        wsync();
+        // (2) the panel below the block (and the right-hand-side row nf): one thread per row
+        {
+          const int i = jb + r + tid;
+          if (i <= nf) {
+            double v[RB];
+            double *row = lbuf + lidx(i, jb);
+#pragma unroll
+            for (int q = 0; q < RB; ++q) v[q] = (q < r) ? row[q] : 0.0;
+#pragma unroll
+            for (int q = 0; q < RB; ++q) {
+              if (q < r) {
+                const double f = -v[q] * dpiv_s[jb + q];
+#pragma unroll
+                for (int q3 = q + 1; q3 < RB; ++q3)
+                  if (q3 < r) v[q3] = fma(f, lbuf[lidx(jb + q3, jb + q)], v[q3]);
+              }
+            }
+#pragma unroll
+            for (int q = 1; q < RB; ++q)
+              if (q < r) row[q] = v[q];
+          }
+        }
+        wsync();
+        // (3) trailing update: rows i >= jb + r, columns k in [jb + r, min(i, nf - 1)]; warp = rows, lane = columns
+        for (int i = jb + r + warp; i <= nf; i += kNW) {
+          double ci[RB];
+          const double *rowi = lbuf + lidx(i, jb);
+#pragma unroll
+          for (int q = 0; q < RB; ++q) ci[q] = (q < r) ? -rowi[q] * dpiv_s[jb + q] : 0.0;
+          for (int k = jb + r + lane; k <= i && k < nf; k += 32) {
+            const double *rowk = lbuf + lidx(k, jb);
+            double acc = lbuf[lidx(i, k)];
+#pragma unroll
+            for (int q = 0; q < RB; ++q)
+              if (q < r) acc = fma(ci[q], rowk[q], acc);
+            lbuf[lidx(i, k)] = acc;
+          }
         }
         wsync();
       }
+      PROF_MARK(9);
       // back substitution (warp 0): x_i = (u_i - sum_{k > i} c_ki x_k) / d_i, column oriented
       if (warp == 0) {
         double u[4];
@@ -701,7 +771,7 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
         }
         for (int k = nf - 1; k >= 0; --k) {
           const double uk = __shfl_sync(0xffffffffu, (k >> 5) == 0 ? u[0] : (k >> 5) == 1 ? u[1] : (k >> 5) == 2 ? u[2] : u[3], k & 31);
-          const double xk = uk / dpiv_s[k];
+          const double xk = uk * dpiv_s[k];
           if (lane == 0) xs_s[k] = xk;
 #pragma unroll
           for (int m = 0; m < 4; ++m) {
@@ -806,8 +876,7 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
     slope0 = sc[1];
     have_dir = true;
     nbt = 0;
-    pass(ytr_s);
-    ++passes;
+    cur = ytr_s;
   }
   wsync();
 
@@ -826,7 +895,6 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
     if (tid == 0) {
       *p.epoch = red.ep;
       if (p.prof) {
-        PROF_MARK(10);
         for (int i = 0; i < kMasterProfSlots; ++i) p.prof[i] += prof_s[i];
       }
       DevState *st = p.st;
@@ -947,6 +1015,7 @@ cudaError_t launch_newton(Ctx *c, bool add_candidate) {
   p.k_max = c->opt.k_max;
   p.tol = c->opt.master_tol;
   void *args[] = {&p};
+  ++c->n_launches;
   return cudaLaunchCooperativeKernel((void *)k_master_newton, dim3(c->master_grid), dim3(kMasterWorkers), args, L.smem,
                                      c->stream);
 }

@@ -289,6 +289,10 @@ __global__ void __launch_bounds__(256) k_price_chain(int32_t mode, const float *
   __shared__ double s_abs[256];
   const int t = threadIdx.x, b = blockIdx.x;
   const int32_t r0 = beam_row_ptr[b], R = beam_row_ptr[b + 1] - r0;
+  if (R == 0) {                                             // a beam without leaf rows: only the closed aperture
+    if (t == 0) { beam_price[b] = 0.0; beam_absmax[b] = 0.0; }
+    return;
+  }
   double amax = 0.0;
   for (int m = t; m < R; m += 256) {
     const int32_t r = r0 + m, c0 = row_col0 ? row_col0[r] : 0, b0 = row_bl_ptr[r], n = row_bl_ptr[r + 1] - b0;
@@ -456,7 +460,7 @@ __global__ void __launch_bounds__(256) k_price_select(const double *__restrict__
     if (t < o) s_cnt[t] += s_cnt[t + o];
     __syncthreads();
   }
-  // duplicate of an aperture already in the pool? (reading S6: counted, still accepted)
+  // duplicate of an aperture already in the pool? (reading S6: counted; it ends the column generation, see below)
   __shared__ int32_t s_dup;
   if (t == 0) s_dup = 0;
   __syncthreads();
@@ -473,19 +477,25 @@ __global__ void __launch_bounds__(256) k_price_select(const double *__restrict__
   }
   __syncthreads();
   if (t == 0) {
-    // Optimal iff no aperture has a negative reduced cost.  Numerically (readings
-    // S3, S6): the price must be below -price_tol * max|w| * rows, and a candidate identical to a
-    // pool aperture is numerical residue of the master solve (its exact reduced cost is >= 0 and
-    // it is the minimiser), so it also ends the column generation.
-    const bool converged = !(price < -price_tol * absmax * (double)(r1 - r0)) || (s_dup != 0);
+    // Optimal iff no aperture has a negative reduced cost.  Numerically (readings S3, S6): the
+    // price must be below -price_tol * max|w| * rows.  A candidate identical to a pool aperture k has the reduced
+    // cost dF/dy_k of the master, which is >= 0 at the master's optimum: its negative price is residue of the
+    // master solve and, being the minimum over all apertures, bounds every other reduced cost.  It proves
+    // optimality only if that solve CONVERGED and the residue is of the size the solve reports (10 x its KKT
+    // residual, or the price tolerance); otherwise the run is STALLED (done = 2): appending the column again
+    // cannot help, and optimality is not claimed.
+    const double tol_abs = price_tol * absmax * (double)(r1 - r0);
+    const bool improving = price < -tol_abs;
+    int done = improving ? 0 : 1;
+    if (improving && s_dup) done = (!st->m_hit_max && -price <= 10.0 * fmax(st->m_kkt, tol_abs)) ? 1 : 2;
     if (s_dup) st->n_duplicates += 1;
     st->cand_beam = best;
     st->cand_price = price;
     st->w_abs_max = absmax;
     st->cand_nopen = s_cnt[0];
     st->cand_dup = s_dup;
-    st->done = converged ? 1 : 0;
-    st->cand_valid = (!converged && K < k_max) ? 1 : 0;
+    st->done = done;
+    st->cand_valid = (done == 0 && K < k_max) ? 1 : 0;
   }
 }
 
@@ -504,6 +514,7 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
     const size_t smem = (size_t)c->max_rows_per_beam * (size_t)(c->max_beam_width + 1) * sizeof(double);
     cudaError_t e = cudaFuncSetAttribute(k_price_jaws, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
+    ++c->n_launches;
     k_price_jaws<<<n_beams, 256, smem, c->stream>>>(w, beam_row_ptr, row_bl_ptr, c->d.row_col0, c->max_beam_width, vstar,
                                                     left, right, beam_price, beam_absmax);
     e = cudaGetLastError();
@@ -512,6 +523,7 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
     const size_t smem = chain_pricing_smem(c->max_rows_per_beam, c->max_beam_width);
     cudaError_t e = cudaFuncSetAttribute(k_price_chain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
+    ++c->n_launches;
     k_price_chain<<<n_beams, 256, smem, c->stream>>>(c->opt.mlc_mode, w, beam_row_ptr, row_bl_ptr, c->d.row_col0,
                                                      c->max_beam_width, c->max_rows_per_beam, c->d.chain_from, vstar, left, right,
                                                      beam_price, beam_absmax);
@@ -525,27 +537,32 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
       int32_t *f = &c->d.state->price_maxlen;
       cudaError_t e = cudaMemsetAsync(f, 0, sizeof(int32_t), c->stream);
       if (e != cudaSuccess) return e;
+      ++c->n_launches;
       k_price_maxlen<<<std::min((n_rows + 255) / 256, c->n_sm * 4), 256, 0, c->stream>>>(row_bl_ptr, n_rows, f);
       e = cudaGetLastError();
       if (e != cudaSuccess) return e;
       flag = f;
     }
     if (seq_possible && (flag || max_row_len <= kPriceSeqMaxLen)) {
+      ++c->n_launches;
       k_price_rows_seq<<<(n_rows + 127) / 128, 128, 0, c->stream>>>(w, row_bl_ptr, n_rows, vstar, left, right, row_absmax, flag);
       cudaError_t e = cudaGetLastError();
       if (e != cudaSuccess) return e;
     }
     if (n_rows > 0 && (!seq_possible || flag || max_row_len > kPriceSeqMaxLen)) {
+      ++c->n_launches;
       k_price_rows<<<(n_rows + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(w, row_bl_ptr, n_rows, vstar, left,
                                                                         right, row_absmax, flag);
       cudaError_t e = cudaGetLastError();
       if (e != cudaSuccess) return e;
     }
+    ++c->n_launches;
     k_price_beams<<<(n_beams + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(vstar, row_absmax, beam_row_ptr, n_beams,
                                                                          beam_price, beam_absmax);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }
+  ++c->n_launches;
   k_price_select<<<1, 256, 0, c->stream>>>(beam_price, beam_absmax, n_beams, beam_row_ptr, left, right, best_out,
                                            update_state ? c->d.state : nullptr, c->opt.price_tol, c->opt.k_max,
                                            c->max_rows_per_beam, c->d.ap_beam, c->d.ap_left, c->d.ap_right);
@@ -586,6 +603,7 @@ __global__ void k_append_candidate(const DevState *__restrict__ st, int32_t n_bl
 cudaError_t launch_append_candidate(Ctx *c) {
   const int t = 128;
   const int n = c->n_bl > c->max_rows_per_beam ? c->n_bl : c->max_rows_per_beam;
+  ++c->n_launches;
   k_append_candidate<<<(n + t - 1) / t, t, 0, c->stream>>>(c->d.state, c->n_bl, c->max_rows_per_beam, c->d.bl_row,
                                                            c->d.row_beam, c->d.beam_row_ptr, c->d.row_bl_ptr,
                                                            c->d.left, c->d.right, c->d.ap_beam, c->d.ap_left,

@@ -36,6 +36,7 @@ __global__ void k_intensity(const DevState *__restrict__ st, int32_t n_bl, int32
 
 cudaError_t launch_intensity(Ctx *c) {
   const int t = 128;
+  ++c->n_launches;
   k_intensity<<<(c->n_bl + t - 1) / t, t, 0, c->stream>>>(c->d.state, c->n_bl, c->max_rows_per_beam,
                                                           c->d.bl_row, c->d.row_beam, c->d.beam_row_ptr,
                                                           c->d.row_bl_ptr, c->d.ap_beam, c->d.ap_left,
@@ -328,6 +329,7 @@ static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out, const in
   p.skip = skip;
   p.a_T = c->nwt.T; p.a_TP = c->nwt.TP; p.a_stride = c->nwt.tile_stride; p.a_col = a_col;
   if (MODE == kSpmvColumn) p.out = c->d.A;
+  ++c->n_launches;
   if (c->spmv_ring_warps > 0) {
     const int nw = c->spmv_ring_warps;
     const size_t smem = (size_t)nw * kRingStages * kRingStageBytes + align_up((size_t)nw * kRingStages * 8, 128) +

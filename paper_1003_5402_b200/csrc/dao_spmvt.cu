@@ -167,6 +167,7 @@ cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out, const int32_t *s
     while (wpr < wpb && c->n_bl * wpr < target) wpr *= 2;
     const int rows_per_cta = wpb / wpr;
     const int grid = std::max(1, std::min((c->n_bl + rows_per_cta - 1) / rows_per_cta, c->n_sm * kTCtasPerSm));
+    ++c->n_launches;
     switch (wpr) {
       case 1: k_spmvt_rows<1><<<grid, kTThreads, 0, c->stream>>>(c->n_bl, c->d.t_ptr, c->d.t_row, c->d.t_val, g, w_out, skip); break;
       case 2: k_spmvt_rows<2><<<grid, kTThreads, 0, c->stream>>>(c->n_bl, c->d.t_ptr, c->d.t_row, c->d.t_val, g, w_out, skip); break;
@@ -179,6 +180,7 @@ cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out, const int32_t *s
     int grid = c->n_sm * kTCtasPerSm;
     const int need = (c->n_tchunks + kTThreads / 32 - 1) / (kTThreads / 32);
     if (grid > need) grid = need;
+    ++c->n_launches;
     k_spmvt<<<grid, kTThreads, 0, c->stream>>>(c->d.t_ptr, c->d.t_row, c->d.t_val, c->nnz, c->n_tchunks,
                                                c->d.t_first_row, c->d.t_seg_base, g, c->d.t_segsum,
                                                &c->d.state->ticket_misc, skip);
@@ -186,6 +188,7 @@ cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out, const int32_t *s
     if (e != cudaSuccess) return e;
   }
   const int t = 128;
+  ++c->n_launches;
   k_spmvt_finish<<<(c->n_bl + t - 1) / t, t, 0, c->stream>>>(c->n_bl, c->d.t_ptr, c->d.t_first_row,
                                                              c->d.t_seg_base, c->d.t_segsum, w_out,
                                                              &c->d.state->ticket_misc, skip);

@@ -24,7 +24,7 @@ MEM_HOST, MEM_DEVICE = 0, 1
 MLC_CONSECUTIVE, MLC_JAWS_ONLY, MLC_INTERDIGITATION, MLC_CONNECTED = 0, 1, 2, 3
 MAX_APERTURES = 128
 (VEC_Z, VEC_G, VEC_W, VEC_X, VEC_Y, VEC_VSTAR, VEC_LEFT, VEC_RIGHT, VEC_BEAM_PRICE, VEC_HISTORY,
- VEC_MASTER_Z, VEC_MASTER_PHASES) = range(12)
+ VEC_MASTER_Z, VEC_MASTER_PHASES, VEC_ITER_SECONDS) = range(13)
 
 EXPORTS = ["dao_default_options", "dao_workspace_bytes", "dao_create", "dao_price", "dao_solve_master",
            "dao_run", "dao_get_plan", "dao_reset", "dao_destroy", "dao_last_error", "dao_get_vector",
@@ -67,7 +67,8 @@ class CSizes(C.Structure):
 
 class CPriceInfo(C.Structure):
     _fields_ = [("beam", C.c_int32), ("converged", C.c_int32), ("price", C.c_double), ("objective", C.c_double),
-                ("w_abs_max", C.c_double), ("n_open_beamlets", C.c_int32), ("duplicate", C.c_int32)]
+                ("w_abs_max", C.c_double), ("n_open_beamlets", C.c_int32), ("duplicate", C.c_int32),
+                ("stalled", C.c_int32), ("reserved", C.c_int32)]
 
 
 class CMasterInfo(C.Structure):
@@ -82,7 +83,7 @@ class CRunInfo(C.Structure):
                 ("seconds_total", C.c_double), ("seconds_intensity", C.c_double), ("seconds_spmv", C.c_double),
                 ("seconds_spmv_t", C.c_double), ("seconds_price", C.c_double), ("seconds_column", C.c_double),
                 ("seconds_master", C.c_double), ("n_passes_total", C.c_int64), ("n_hit_max_iter", C.c_int32),
-                ("reserved", C.c_int32)]
+                ("n_kernel_launches", C.c_int32), ("stalled", C.c_int32), ("reserved", C.c_int32)]
 
 
 class CIterRecord(C.Structure):
@@ -324,7 +325,8 @@ class Dao:
                   VEC_X: (self.n_bl, np.float32), VEC_Y: (k_max, np.float64), VEC_VSTAR: (self.n_rows, np.float64),
                   VEC_LEFT: (self.n_rows, np.int32), VEC_RIGHT: (self.n_rows, np.int32),
                   VEC_BEAM_PRICE: (self.n_beams, np.float64), VEC_HISTORY: (k_max, ITER_RECORD_DTYPE),
-                  VEC_MASTER_Z: (self.n_vox, np.float64), VEC_MASTER_PHASES: (16, np.uint64)}
+                  VEC_MASTER_Z: (self.n_vox, np.float64), VEC_MASTER_PHASES: (16, np.uint64),
+                  VEC_ITER_SECONDS: (k_max * 6, np.float64)}
         n, dt = shapes[which]
         out = np.zeros(n, dtype=dt)
         self._check(self.lib.dao_get_vector(self._ctx, C.c_int32(which), C.c_void_p(_np_ptr(out)), C.c_int(MEM_HOST)))

@@ -35,6 +35,9 @@ def main():
         "beams": [int(b) for b in plan.beams],
         "price": [float(h.price) for h in plan.history],
         "master_objective": [float(h.objective) for h in plan.history],
+        "master_iterations": [int(h.n_master_iter) for h in plan.history],
+        "kkt": [float(h.kkt) for h in plan.history],
+        "n_duplicates": int(plan.n_duplicates), "stalled": bool(plan.stalled),
         "n_open_beamlets": [int(sum(int(r) - int(l) for l, r in zip(h.left, h.right))) for h in plan.history],
     }
     path = os.path.join(HERE, f"oracle_plan_{config}.json")

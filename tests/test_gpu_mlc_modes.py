@@ -184,3 +184,67 @@ def test_chain_plan_matches_oracle(D, mode, mini):
     n_same = sum(1 for k in range(min(len(ref.beams), len(plan.beams))) if plan.beams[k] == ref.beams[k]
                  and np.array_equal(plan.leaves(k)[0], ref.lefts[k]) and np.array_equal(plan.leaves(k)[1], ref.rights[k]))
     print(f"mini {mode}: F_gpu={info.objective:.10g} F_oracle={ref.objective:.10g} same apertures {n_same}/{len(ref.beams)}")
+
+
+# ----------------------------------------------------------------------------- full size (the widths bench.py --widened times)
+@pytest.fixture(scope="module")
+def cfg1():
+    from paper_1003_5402_b200.inputs import phantom
+    return phantom.make("cfg1", seed=0)
+
+
+@pytest.mark.parametrize("mode", ["jaws", "interdigitation", "connected"])
+def test_mlc_modes_at_full_size(D, cfg1, mode):
+    """configs[1] (widest beam 26 lateral positions: the leaf-state tables of the chain modes and the rectangle scan of
+    the jaws mode at their real shape).  Three column-generation iterations in lock-step -- the oracle prices the GPU's
+    own fp32 w: beam prices to 1e-9, the aperture attains its beam's price and is deliverable -- then the plan is
+    completed and every one of its 50 apertures is checked for deliverability."""
+    ph = cfg1
+    code = {"jaws": D.MLC_JAWS_ONLY, "interdigitation": D.MLC_INTERDIGITATION, "connected": D.MLC_CONNECTED}[mode]
+
+    def deliverable(b, le_rows, ri_rows):
+        le = np.zeros(ph.n_rows, np.int32); ri = np.zeros(ph.n_rows, np.int32)
+        r0 = int(ph.beam_row_ptr[b])
+        le[r0:r0 + le_rows.size] = le_rows; ri[r0:r0 + ri_rows.size] = ri_rows
+        if mode != "jaws":
+            return _chain_feasible(mode, ph, int(b), le, ri)
+        rows = [m for m in range(le_rows.size) if ri_rows[m] > le_rows[m]]
+        if not rows or rows != list(range(rows[0], rows[-1] + 1)):
+            return False
+        c1 = min(int(ph.row_col0[r0 + m] + le_rows[m]) for m in rows)
+        c2 = max(int(ph.row_col0[r0 + m] + ri_rows[m]) for m in rows)
+        for m in rows:
+            c0 = int(ph.row_col0[r0 + m]); n = int(ph.row_bl_ptr[r0 + m + 1] - ph.row_bl_ptr[r0 + m])
+            if (c0 + le_rows[m], c0 + ri_rows[m]) != (max(c1, c0), min(c2, c0 + n)):
+                return False
+        return True
+
+    with D.Dao(ph, k_max=50, mlc_mode=code) as d:
+        for it in range(3):
+            info = d.price()
+            w = d.get_vector(D.VEC_W)
+            le, ri, bp = d.get_vector(D.VEC_LEFT), d.get_vector(D.VEC_RIGHT), d.get_vector(D.VEC_BEAM_PRICE)
+            w64 = w.astype(np.float64)
+            pr = (orc.price_jaws(w64, ph.beam_row_ptr, ph.row_bl_ptr, ph.row_col0) if mode == "jaws" else
+                  orc.price_chain(w64, ph.beam_row_ptr, ph.row_bl_ptr, ph.row_col0, mode))
+            scale = max(float(np.abs(pr.beam_price).max()), 1e-300)
+            np.testing.assert_allclose(bp, pr.beam_price, rtol=0, atol=1e-9 * scale)
+            pu.check_beam(bp, info.beam, pr.beam_price)
+            for b in range(ph.n_beams):
+                rows = range(ph.beam_row_ptr[b], ph.beam_row_ptr[b + 1])
+                got = sum(float(w64[ph.row_bl_ptr[r] + le[r]: ph.row_bl_ptr[r] + ri[r]].sum()) for r in rows)
+                assert abs(got - pr.beam_price[b]) <= 1e-9 * scale
+            r0, r1 = int(ph.beam_row_ptr[info.beam]), int(ph.beam_row_ptr[info.beam + 1])
+            assert deliverable(info.beam, le[r0:r1], ri[r0:r1])
+            assert info.price < 0 and not info.converged
+            m = d.solve_master()
+            assert m.n_apertures == it + 1 and not m.hit_max_iter
+        info = d.run(50)
+        plan = d.get_plan()
+    assert info.n_apertures == 50
+    for k, b in enumerate(plan.beams):
+        assert deliverable(int(b), *plan.leaves(k)), (mode, k)
+    cons_gold = 0.008774594169620595        # oracle_plan_cfg1.json: the separable rule's 50-aperture objective
+    assert info.objective >= cons_gold * (1 - 1e-3)          # every alternative rule restricts the consecutive one
+    print(f"cfg1 {mode}: 50 apertures, F = {info.objective:.8g} (consecutive rule, oracle: {cons_gold:.8g}), "
+          f"{info.n_pg_iter_total} master iterations, pricing {1e6 * info.seconds_price / max(1, info.n_iterations):.1f} us per iteration")

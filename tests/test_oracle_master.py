@@ -187,3 +187,19 @@ def test_cfg0_runs_to_50_apertures_in_seconds(cfg0):
     assert time.time() - t < 60
     assert 1 <= len(plan.beams) <= 50
     assert plan.objective < 1.0 and all(h.kkt < 1e-8 for h in plan.history)
+
+
+def test_stored_cfg1_plan_is_converged_at_every_iteration():
+    """tests/golden/oracle_plan_cfg1.json (written by make_oracle_plan.py from oracle/ only): every master solve of
+    the stored free-running plan met the KKT conditions to 1e-8 (absolute, in units of dF/dy; F is 1e-2 .. 1 along
+    the plan), no duplicate candidate ever appeared (reading S6 never fired) and the objective fell monotonically."""
+    import json
+    import os
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "oracle_plan_cfg1.json")) as f:
+        gold = json.load(f)
+    assert len(gold["kkt"]) == gold["n_apertures"] == 50
+    assert max(gold["kkt"]) <= 1e-8
+    assert gold["n_duplicates"] == 0 and not gold["stalled"] and not gold["converged"]
+    f = np.asarray(gold["master_objective"])
+    assert (np.diff(f) < 0).all() and (np.asarray(gold["price"]) < 0).all()
+    assert gold["objective"] == pytest.approx(f[-1], rel=1e-9)
