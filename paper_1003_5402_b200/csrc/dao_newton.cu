@@ -175,7 +175,6 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
   const int AC = p.AC, WP = p.AC + 4;              // active voxels per chunk, row pitch of W (4 mod 16: conflict-free)
   const int ac_shift = 31 - __clz(AC);
   const int w_doubles = p.w_doubles;               // doubles per W tile
-  const int srow = p.srow;                         // row of W that holds the curvature weights s_a
   double *gs = reinterpret_cast<double *>(q); q += align_up_c((size_t)(T + 4) * 8, 128);
   double *ss = reinterpret_cast<double *>(q); q += align_up_c((size_t)(T + 4) * 8, 128);
   unsigned short *list = reinterpret_cast<unsigned short *>(q);
@@ -402,7 +401,7 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
         CYC_MARK(13);
         // ---- P ----
         bool act0 = false;
-        double sq0 = 0.0, gq0 = 0.0;                             // s_j = 2 c_j, pi_j / s_j
+        double sq0 = 0.0, gq0 = 0.0;                             // sqrt(s_j), s_j = 2 c_j; pi_j / sqrt(s_j)
         if (in0) {
           if (sid0 != kNoStruct) {
             StructEntry e = stab[sid0];
@@ -413,9 +412,9 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
             const double sv = 2.0 * ((un > 0.0 ? e.a : 0.0) + (ov > 0.0 ? e.b : 0.0));
             if (sv != 0.0) {
               act0 = true;
-              sq0 = sv;
+              sq0 = sqrt(sv);
               // pi / s = -(T^- - z) below the band, z - T^+ above it; both sides at once only if T^- > T^+
-              gq0 = (un > 0.0 && ov > 0.0) ? gv / sv : (un > 0.0 ? -un : ov);
+              gq0 = sq0 * ((un > 0.0 && ov > 0.0) ? gv / sv : (un > 0.0 ? -un : ov));
             }
           }
           if (!(p.debug & 8)) p.mz[vg0] = z0;
@@ -437,21 +436,21 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
         if (prof) prof_s[11] += (unsigned long long)n_act;
         fsync();
         CYC_MARK(14);
-        // ---- W: chunks of AC active voxels.  W[k][a] = A[k][v_a] in fp64 (integer pipe only), row K: pi_a / s_a,
-        //      row 8 nb_max: s_a.  The back warps scale the B fragment by s_a. ----
+        // ---- W: chunks of AC active voxels.  W[k][a] = sqrt(s_a) A[k][v_a] in fp64, row K: pi_a / sqrt(s_a), so
+        //      that W W^T = [H, grad] and both tensor-core operands come straight from W. ----
         int c0 = 0;
         do {
           const int nca = min(AC, n_act - c0), nca4 = (nca + 3) & ~3;
           if (!w_first_round) mbar_spin_wait(&wempty[wp.stage], wp.phase ^ 1u);
           CYC_MARK(5);
           double *wt = wbuf + (size_t)wp.stage * w_doubles;
-          if (tid < nca4) wt[(size_t)srow * WP + tid] = (tid < nca) ? ss[c0 + tid] : 0.0;
           if (tid < nca4) wt[(size_t)K * WP + tid] = (tid < nca) ? gs[c0 + tid] : 0.0;
           {
             // thread = (column a, row parity); the voxel of the column is looked up once
             const int a = tid & (AC - 1), kpar = tid >> ac_shift, kstep = kNwtFrontThreads >> ac_shift;
             if (a < nca4 && !(p.debug & 2)) {
               const bool live = a < nca;
+              const double sqa = live ? ss[c0 + a] : 0.0;
               const float *src = M + (live ? (int)list[c0 + a] : 0);
               double *dst = wt + a;
               for (int k = kpar; k < K; k += 4 * kstep) {
@@ -460,7 +459,7 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
                 for (int u = 0; u < 4; ++u) f[u] = src[(size_t)min(k + u * kstep, K - 1) * TP];
 #pragma unroll
                 for (int u = 0; u < 4; ++u)
-                  if (k + u * kstep < K) dst[(size_t)(k + u * kstep) * WP] = live ? cvt_pos(f[u]) : 0.0;
+                  if (k + u * kstep < K) dst[(size_t)(k + u * kstep) * WP] = sqa * cvt_pos(f[u]);
               }
             }
           }
@@ -504,21 +503,18 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
           const uint32_t wt_s = smem_addr(wt);
           for (int qd = grp; qd < ((p.debug & 1) ? 0 : nq); qd += NG) {
             const uint32_t wq = wt_s + (uint32_t)(qd * 4 + (lane & 3)) * 8u;
-            const double sv = lds_f64(wq + (uint32_t)(srow * WP) * 8u);
 #pragma unroll
             for (int s = 0; s < kNwtStrips; ++s) {
               if (s < nstr) {
-                // all fragments of the strip are requested before the first tensor-core instruction (volatile loads:
-                // left alone, the compiler sinks every load next to its predicated mma and the chain
-                // load -> scale -> mma runs once per block, 75 cycles instead of 16); a short strip re-reads
-                // its last block
+                // all fragments of the strip are requested before its first tensor-core instruction (left alone,
+                // the compiler sinks every load next to its predicated mma and the chain load -> mma runs once
+                // per block, 75 cycles instead of 16); a short strip re-reads its last block.  (All strips of a
+                // quad at once would need 36 more registers and spills inside this loop.)
                 const double fa = lds_f64(wq + (uint32_t)st_offa[s] * 8u);
                 double fb[kNwtStripLen];
 #pragma unroll
                 for (int m = 0; m < kNwtStripLen; ++m)
                   fb[m] = lds_f64(wq + (uint32_t)(st_offb[s] + min(m, st_len[s] - 1) * 8 * WP) * 8u);
-#pragma unroll
-                for (int m = 0; m < kNwtStripLen; ++m) fb[m] *= sv;
                 if (st_len[s] == kNwtStripLen) {           // full strip: straight-line tensor-core code
 #pragma unroll
                   for (int m = 0; m < kNwtStripLen; ++m) dmma884(acc[s][m][0], acc[s][m][1], fa, fb[m]);

@@ -439,6 +439,9 @@ CONFIGS = {
     "cfg4": lambda: spec_stress(2.2),
     "cfg4_literal": lambda: spec_stress(1.0),
     "mini": spec_mini,
+    # the paper's own problem size (Table 1: case P1 has 7,196 beamlets, 45,912 voxels, 2.76M
+    # non-zeros; unspecified tissue at coarse resolution): 9 fields, 6.5 mm voxels -> 7,337 beamlets, 42,898 voxels, 4.5M
+    "paper_p1": lambda: spec_prostate(2.7, n_beams=9, voxel_mm=6.5, grid=(70, 44, 32), name="paper_p1"),
     # BASELINE.json configs[3] (kernel sweep): pencil-beam matrices from ~1M to ~200M non-zeros
     "sweep_1m": lambda: spec_prostate(1.0, n_beams=5, voxel_mm=4.0, grid=(126, 126, 76), name="sweep_1m"),
     "sweep_3m": lambda: spec_prostate(1.0, n_beams=9, voxel_mm=4.0, grid=(126, 126, 76), name="sweep_3m"),

@@ -149,3 +149,42 @@ def test_pricing_many_rows_thread_per_row_kernel(D, n_rows, row_len):
     pi = orc.price(wi.astype(np.float64), brp, rbp)
     assert np.array_equal(li, pi.left) and np.array_equal(rii, pi.right) and np.array_equal(vi, pi.vstar)
     assert besti[0] == pi.best_beam
+
+
+@pytest.mark.parametrize("mode", ["consecutive", "jaws", "interdigitation", "connected"])
+def test_beam_without_leaf_rows(D, tiny, mode):
+    """A beam with zero leaf rows offers only the closed aperture: its price is 0 in every MLC mode and it never
+    wins against a beam with a negative price (the chain modes once read an unwritten table there)."""
+    ph = copy.copy(tiny)
+    ph.n_beams = tiny.n_beams + 1
+    ph.beam_row_ptr = np.r_[tiny.beam_row_ptr[:1], tiny.beam_row_ptr[:1], tiny.beam_row_ptr[1:]].astype(np.int32)   # beam 0 is empty
+    code = {"consecutive": D.MLC_CONSECUTIVE, "jaws": D.MLC_JAWS_ONLY, "interdigitation": D.MLC_INTERDIGITATION,
+            "connected": D.MLC_CONNECTED}[mode]
+    rng = np.random.default_rng(5)
+    with D.Dao(ph, mlc_mode=code, k_max=8) as d:
+        for trial in range(3):
+            w = rng.standard_normal(ph.n_bl).astype(np.float32) - 0.5
+            le, ri, vs, bp, best = (t.cpu().numpy() for t in d.price_from_w(_dev(w)))
+            assert bp[0] == 0.0 and bp[1:].min() < 0.0 and int(best[0]) == 1 + int(np.argmin(bp[1:]))
+        info = d.run(8)
+        plan = d.get_plan()
+    assert info.n_apertures >= 1 and (plan.beams != 0).all()
+    ref = orc.run(tiny, 8, mlc=mode)
+    assert abs(info.objective - ref.objective) <= 1e-3 * ref.objective      # the empty beam changes nothing
+
+
+def test_newton_master_at_its_largest_pool(D, mini):
+    """master_method = 2 up to 103 apertures (13 block rows of the Hessian; larger k_max falls back to method 1):
+    k_max = 100 on mini against the oracle's plan, and both methods against each other."""
+    ref = orc.run(mini, 100)
+    out = {}
+    for method in (1, 2):
+        with D.Dao(mini, k_max=100, master_method=method) as d:
+            info = d.run(100)
+            out[method] = info
+    for info in out.values():
+        assert info.n_apertures == len(ref.beams) and bool(info.converged) == ref.converged
+        assert abs(info.objective - ref.objective) <= 1e-3 * ref.objective
+    assert out[2].n_passes_total < out[1].n_passes_total / 5
+    print(f"mini k_max=100: {out[2].n_apertures} apertures, F m1={out[1].objective:.10g} m2={out[2].objective:.10g} oracle={ref.objective:.10g}; "
+          f"passes over A: {out[1].n_passes_total} (method 1) vs {out[2].n_passes_total} (method 2)")

@@ -194,3 +194,30 @@ def test_other_full_size_configs(D, config, n_ap):
           f"{info.seconds_total:.4f} s, F={info.objective:.8g}, pg iterations {info.n_pg_iter_total}, kkt gap {gap:.1e}; "
           "per-iteration split: " + ", ".join(f"{k} {1e6 * v / n_it:.1f} us ({v / tot:.1%})" for k, v in split.items())
           + f"; SpMV {8e-9 * ph.nnz / (split['spmv'] / n_it):.0f} GB/s, SpMV^T {8e-9 * ph.nnz / (split['spmv_t'] / n_it):.0f} GB/s (8 nnz bytes)")
+
+
+def test_paper_sized_plan_matches_oracle(D):
+    """A workload of the paper's own size (Table 1; case P1: 7,196 beamlets, 45,912 voxels): the
+    free-running 50-aperture plan against the oracle's own free-running plan, which takes seconds at this size (no
+    fixture).  This is the regime where fixed latencies, not bandwidth, decide the plan time (1.7 s on
+    a Tesla C1060 for P1 -- context only: other hardware, clinical data)."""
+    ph = phantom.make("paper_p1", seed=0)
+    ref = orc.run(ph, 50)
+    with D.Dao(ph, k_max=50) as d:
+        d.run(50); d.reset()
+        info = d.run(50)
+        plan = d.get_plan()
+        hist = d.get_vector(D.VEC_HISTORY)[:info.n_apertures]
+    assert info.n_apertures == 50 == len(ref.beams)
+    rel = abs(info.objective - ref.objective) / ref.objective
+    assert rel <= REL_OBJ, (info.objective, ref.objective)
+    n_same = sum(1 for k in range(50) if plan.beams[k] == ref.beams[k] and np.array_equal(plan.leaves(k)[0], ref.lefts[k])
+                 and np.array_equal(plan.leaves(k)[1], ref.rights[k]))
+    f_or = np.asarray([h.objective for h in ref.history])
+    assert (np.abs(hist["objective"] - f_or) <= REL_OBJ * f_or).all()
+    n_it = max(1, info.n_iterations)
+    print(f"paper_p1: V={ph.n_vox} N={ph.n_bl} nnz={ph.nnz}: F_gpu={info.objective:.10g} F_oracle={ref.objective:.10g} rel={rel:.1e} "
+          f"identical apertures {n_same}/50; plan {info.seconds_total:.4f} s; per iteration: pricing {1e6 * info.seconds_price / n_it:.1f} us "
+          f"(paper: < 100 us, PAPER.md:256), SpMV {1e6 * info.seconds_spmv / n_it:.1f}, SpMV^T {1e6 * info.seconds_spmv_t / n_it:.1f}, "
+          f"column {1e6 * info.seconds_column / n_it:.1f}, master {1e6 * info.seconds_master / n_it:.1f} us; "
+          f"{info.n_pg_iter_total} master iterations, {info.n_passes_total} passes over A")
