@@ -179,6 +179,7 @@ dao_status dao_reset(dao_ctx *ctx) {
   API_CUDA(cudaMemsetAsync(c->d.history, 0, (size_t)c->opt.k_max * sizeof(dao_iter_record), c->stream));
   API_CUDA(cudaStreamSynchronize(c->stream));
   c->K = 0;
+  c->x_current = false;
   c->have_candidate = false;
   return DAO_OK;
 }
@@ -471,6 +472,7 @@ dao_status dao_set_pool(dao_ctx *ctx, int32_t n_apertures, const int32_t *beam, 
   if (K > 0 && (!beam || !ap_row_ptr || !left || !right)) return fail(c, DAO_E_ARG, "null pool array");
   std::vector<int32_t> le((size_t)std::max(K, 1) * mr, 0), ri((size_t)std::max(K, 1) * mr, 0);
   std::vector<double> yy(DAO_MAX_APERTURES, 0.0);
+  std::vector<unsigned long long> hh((size_t)std::max(K, 1), 0ull);
   for (int32_t k = 0; k < K; ++k) {
     if (beam[k] < 0 || beam[k] >= c->n_beams) return fail(c, DAO_E_SHAPE, "aperture beam out of range");
     const int32_t r0 = c->beam_row_ptr[beam[k]], nr = c->beam_row_ptr[beam[k] + 1] - r0;
@@ -480,7 +482,9 @@ dao_status dao_set_pool(dao_ctx *ctx, int32_t n_apertures, const int32_t *beam, 
       const int32_t n = c->row_bl_ptr[r0 + m + 1] - c->row_bl_ptr[r0 + m];
       if (l < 0 || r < l || r > n) return fail(c, DAO_E_SHAPE, "leaf positions out of range");
       le[(size_t)k * mr + m] = l; ri[(size_t)k * mr + m] = r;
+      hh[k] += leaf_hash(m, l, r);
     }
+    hh[k] += beam_hash(beam[k]);
     if (y) {
       if (!(y[k] >= 0.0)) return fail(c, DAO_E_ARG, "intensities must be >= 0");
       yy[k] = y[k];
@@ -490,6 +494,7 @@ dao_status dao_set_pool(dao_ctx *ctx, int32_t n_apertures, const int32_t *beam, 
     API_CUDA(cudaMemcpyAsync(c->d.ap_beam, beam, (size_t)K * 4, cudaMemcpyHostToDevice, c->stream));
     API_CUDA(cudaMemcpyAsync(c->d.ap_left, le.data(), (size_t)K * mr * 4, cudaMemcpyHostToDevice, c->stream));
     API_CUDA(cudaMemcpyAsync(c->d.ap_right, ri.data(), (size_t)K * mr * 4, cudaMemcpyHostToDevice, c->stream));
+    API_CUDA(cudaMemcpyAsync(c->d.ap_hash, hh.data(), (size_t)K * 8, cudaMemcpyHostToDevice, c->stream));
   }
   API_CUDA(cudaMemcpyAsync(c->d.y, yy.data(), DAO_MAX_APERTURES * 8, cudaMemcpyHostToDevice, c->stream));
   k_set_pool_state<<<1, 1, 0, c->stream>>>(c->d.state, K);
@@ -504,6 +509,7 @@ dao_status dao_set_pool(dao_ctx *ctx, int32_t n_apertures, const int32_t *beam, 
   }
   API_CUDA(cudaStreamSynchronize(c->stream));   // le/ri/yy are stack-owned
   c->K = K;
+  c->x_current = false;
   c->have_candidate = false;
   return DAO_OK;
 }
@@ -512,6 +518,7 @@ dao_status dao_fmo_solve(dao_ctx *ctx, int32_t max_iter, double tol, int32_t war
   Ctx *c = reinterpret_cast<Ctx *>(ctx);
   if (!c) return DAO_E_ARG;
   if (max_iter < 0) return fail(c, DAO_E_ARG, "max_iter must be >= 0");
+  c->x_current = false;               // x becomes the FMO variable
   c->have_candidate = false;          // the pending candidate was priced at a dose that is being overwritten
   return fmo_solve(c, max_iter, tol, warm_start != 0, out);
 }

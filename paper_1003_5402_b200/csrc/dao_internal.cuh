@@ -104,6 +104,7 @@ struct DevState {
   int32_t m_passes;        // passes over A of the last master solve
   int32_t n_hit_max;       // master solves that stopped on the iteration cap since dao_create / dao_reset
   int32_t n_duplicates;
+  unsigned long long cand_hash;   // aperture_hash of the pending candidate
   int32_t price_maxlen;    // longest leaf row of caller-provided MLC tables (dao_price_from_w), decided on the device
 };
 
@@ -183,6 +184,7 @@ struct DevPtrs {
   double *beam_absmax;     // [n_beams]
   // pool
   int32_t *ap_beam;        // [k_max]
+  unsigned long long *ap_hash;   // [k_max] aperture_hash of every pool aperture (duplicate test: compare, then verify)
   int32_t *ap_left;        // [k_max * max_rows_per_beam]
   int32_t *ap_right;
   float *A;                // [k_max][n_vox_pad] aperture-major dose block
@@ -237,6 +239,8 @@ struct Ctx {
   // host bookkeeping
   int32_t K = 0;                // pool size as last seen by the host
   bool have_candidate = false;
+  bool x_current = false;       // d.x holds the beamlet intensities of the pool's current y (the Newton master writes them)
+  bool cand_appended = false;   // the last pricing launch already wrote the candidate into the pool tables
   double objective = 0.0;
   cudaEvent_t ev[8] = {};
   int64_t n_launches = 0;       // kernels launched on the hot path since dao_create (dao_run reports the difference)
@@ -258,6 +262,16 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
     }                                                                                     \
   } while (0)
 
+// Order-independent 64-bit hash of an aperture: beam + sum over its leaf rows of a mixed (row, left, right)
+__host__ __device__ __forceinline__ unsigned long long leaf_hash(int32_t m, int32_t l, int32_t r) {
+  unsigned long long z = ((unsigned long long)(uint32_t)m << 42) ^ ((unsigned long long)(uint32_t)l << 21) ^ (unsigned long long)(uint32_t)r;
+  z += 0x9e3779b97f4a7c15ull;
+  z = (z ^ (z >> 30)) * 0xbf58476d1ce4e5b9ull;
+  z = (z ^ (z >> 27)) * 0x94d049bb133111ebull;
+  return z ^ (z >> 31);
+}
+__host__ __device__ __forceinline__ unsigned long long beam_hash(int32_t b) { return leaf_hash(0x7ffff, b, b); }
+
 // kernels / launchers implemented in the .cu files --------------------------------------------
 // dao_setup.cu
 struct HostLayout;   // SELL slice table and permutation computed on the host from row_ptr
@@ -276,6 +290,9 @@ cudaError_t launch_spmv(Ctx *c, SpmvMode mode, const float *x, float *out, const
 cudaError_t launch_spmv_t(Ctx *c, const float *g, float *w_out, const int32_t *skip = nullptr);
 cudaError_t launch_intensity(Ctx *c);
 void spmv_configure(Ctx *c);
+// the column SpMV builds the candidate's 0/1 mask itself while it stages x in shared memory (every variant but the
+// one that reads x from global memory)
+inline bool spmv_builds_mask(const Ctx *c) { return c->spmv_ring_warps > 0 || c->x_in_smem; }
 
 // dao_pricing.cu
 cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, const int32_t *beam_row_ptr,

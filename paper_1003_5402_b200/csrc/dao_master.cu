@@ -794,6 +794,7 @@ cudaError_t master_configure(Ctx *c) {
 
 cudaError_t launch_master(Ctx *c, bool add_candidate) {
   if (c->opt.master_method == 2) return launch_newton(c, add_candidate);
+  c->x_current = false;                    // methods 0 / 1 leave step 1 (beamlet intensities) to k_intensity
   MasterParams p{};
   p.A = c->d.A;
   p.n_vox_pad = c->n_vox_pad;

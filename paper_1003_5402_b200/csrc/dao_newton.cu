@@ -71,6 +71,10 @@ struct NewtonParams {
   DevState *st;
   dao_iter_record *history;
   const int32_t *ap_beam;
+  // step 1 (eq. 7) of the NEXT column-generation iteration, done here: x_i = sum_{k : i in A_k} y_k
+  int32_t n_bl, max_rows;
+  const int32_t *bl_row, *row_beam, *beam_row_ptr, *row_bl_ptr, *ap_left, *ap_right;
+  float *x;
   int32_t add_candidate;
   int32_t max_iter;
   int32_t k_max;
@@ -149,8 +153,19 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
   const int cand = p.st->cand_valid;
   const int added = (p.add_candidate && cand) ? 1 : 0;
   const int K = K0 + added;
-  if ((p.add_candidate && !added) || K == 0) {     // converged, pool full or empty pool: nothing to do
+  if ((p.add_candidate && !added) || K == 0) {     // converged, pool full or empty pool: nothing to solve
     if (blockIdx.x == 0 && tid == 0) { p.st->m_added = 0; p.st->m_iters = 0; p.st->m_passes = 0; }
+    // x for the unchanged y (callers rely on the master leaving x current)
+    for (int i = (int)blockIdx.x * kMasterWorkers + tid; i < p.n_bl; i += (int)gridDim.x * kMasterWorkers) {
+      const int r = p.bl_row[i], b = p.row_beam[r];
+      const int m = r - p.beam_row_ptr[b], c = i - p.row_bl_ptr[r];
+      double acc = 0.0;
+      for (int k = 0; k < K0; ++k) {
+        if (p.ap_beam[k] != b) continue;
+        if (c >= p.ap_left[k * p.max_rows + m] && c < p.ap_right[k * p.max_rows + m]) acc += p.y[k];
+      }
+      p.x[i] = (float)acc;
+    }
     return;
   }
 
@@ -886,6 +901,17 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
       cp.advance(NS);
     }
   }
+  // beamlet intensities of the new plan (every CTA a slice; same arithmetic as k_intensity: fp64 sum in pool order)
+  for (int i = (int)blockIdx.x * kMasterWorkers + tid; i < p.n_bl; i += (int)gridDim.x * kMasterWorkers) {
+    const int r = p.bl_row[i], b = p.row_beam[r];
+    const int m = r - p.beam_row_ptr[b], c = i - p.row_bl_ptr[r];
+    double acc = 0.0;
+    for (int k = 0; k < K; ++k) {
+      if (p.ap_beam[k] != b) continue;
+      if (c >= p.ap_left[k * p.max_rows + m] && c < p.ap_right[k * p.max_rows + m]) acc += y_s[k];
+    }
+    p.x[i] = (float)acc;
+  }
   if (blockIdx.x == 0) {
     if (tid < K) p.y[tid] = y_s[tid];
     if (tid == 0) {
@@ -1006,6 +1032,10 @@ cudaError_t launch_newton(Ctx *c, bool add_candidate) {
   p.st = c->d.state;
   p.history = c->d.history;
   p.ap_beam = c->d.ap_beam;
+  p.n_bl = c->n_bl; p.max_rows = c->max_rows_per_beam;
+  p.bl_row = c->d.bl_row; p.row_beam = c->d.row_beam; p.beam_row_ptr = c->d.beam_row_ptr; p.row_bl_ptr = c->d.row_bl_ptr;
+  p.ap_left = c->d.ap_left; p.ap_right = c->d.ap_right; p.x = c->d.x;
+  c->x_current = true;                     // the kernel leaves x consistent with the y it returns
   p.add_candidate = add_candidate ? 1 : 0;
   p.max_iter = c->opt.master_max_iter;
   p.k_max = c->opt.k_max;

@@ -13,6 +13,25 @@ namespace dao {
 constexpr int kPriceSeqMaxLen = 88;    // longest leaf row the thread-per-row kernel stages
 constexpr int kPriceSeqMinRows = 32768; // below this the warp-per-row kernel has the lower latency
 
+// The tail of a pricing launch: the LAST CTA to finish (ticket counter) sums the row minima per beam (step 6a),
+// picks the beam, tests optimality and, inside dao_run / dao_price, turns the winner into the pending candidate
+// (pool tables at index K, 0/1 beamlet mask) -- one launch instead of four (row kernel, beam sums, selection,
+// append).  Every kernel that ends with it runs 256 threads per CTA and no thread leaves before the tail.
+struct PriceTail {
+  uint32_t *ticket;              // self-resetting counter (DevState.ticket_misc: free between the SpMV^T and the column)
+  int32_t do_beams;              // 1: the kernel produced row minima, the beam sums are still to do
+  int32_t n_beams, n_rows, n_bl, max_rows, k_max;
+  const int32_t *beam_row_ptr, *row_bl_ptr, *bl_row, *row_beam;
+  double *vstar, *row_absmax, *beam_price, *beam_absmax;
+  int32_t *left, *right, *best_out;
+  DevState *st;                  // null: hook call (dao_price_from_w), no candidate bookkeeping
+  double price_tol;
+  int32_t *ap_beam, *ap_left, *ap_right;
+  unsigned long long *ap_hash;
+  float *xmask;
+};
+__device__ void price_tail(const PriceTail &q);
+
 // ------------------------------------------------------------------------------------------
 // step 5.  One warp per leaf row.  With S_0 = 0 and S_r = w_1 + .. + w_r (fp64 sums of the fp32
 // inputs) the printed scan returns
@@ -23,12 +42,10 @@ constexpr int kPriceSeqMinRows = 32768; // below this the warp-per-row kernel ha
 // reduction per tile of 32 beamlets, carrying (S, max, argmax, best) between tiles.
 // Output in the ABI convention: half-open [left, right) = [l, r), closed row = (0, 0).
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_price_rows(const float *__restrict__ w,
-                                                    const int32_t *__restrict__ row_bl_ptr, int32_t n_rows,
-                                                    double *__restrict__ vstar, int32_t *__restrict__ left,
-                                                    int32_t *__restrict__ right,
-                                                    double *__restrict__ row_absmax,
-                                                    const int32_t *__restrict__ maxlen_flag) {
+__device__ __forceinline__ void price_rows_body(const float *__restrict__ w, const int32_t *__restrict__ row_bl_ptr,
+                                                int32_t n_rows, double *__restrict__ vstar, int32_t *__restrict__ left,
+                                                int32_t *__restrict__ right, double *__restrict__ row_absmax,
+                                                const int32_t *__restrict__ maxlen_flag) {
   const int lane = threadIdx.x & 31;
   const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (maxlen_flag && *maxlen_flag <= kPriceSeqMaxLen) return;     // the thread-per-row kernel takes this launch
@@ -97,6 +114,13 @@ __global__ void __launch_bounds__(256) k_price_rows(const float *__restrict__ w,
   }
 }
 
+__global__ void __launch_bounds__(256) k_price_rows(const float *w, const int32_t *row_bl_ptr, int32_t n_rows, double *vstar,
+                                                    int32_t *left, int32_t *right, double *row_absmax,
+                                                    const int32_t *maxlen_flag, PriceTail tail) {
+  price_rows_body(w, row_bl_ptr, n_rows, vstar, left, right, row_absmax, maxlen_flag);
+  if (tail.ticket) price_tail(tail);
+}
+
 // ------------------------------------------------------------------------------------------
 // step 5 for MANY leaf rows (the 10^4-10^5-row end of BASELINE.json configs[3]): thread per row, which is the
 // paper's own launch shape, but fed through shared memory: a warp copies the beamlets of its 32
@@ -151,18 +175,14 @@ __global__ void k_price_maxlen(const int32_t *__restrict__ row_bl_ptr, int32_t n
 
 // step 6a: price_b = sum over the rows of beam b of v* (PAPER.md:169).  One warp per beam,
 // lane-strided partial sums in row order, then a fixed shuffle tree.
-__global__ void __launch_bounds__(256) k_price_beams(const double *__restrict__ vstar,
-                                                     const double *__restrict__ row_absmax,
-                                                     const int32_t *__restrict__ beam_row_ptr, int32_t n_beams,
-                                                     double *__restrict__ beam_price,
-                                                     double *__restrict__ beam_absmax) {
+__device__ __forceinline__ void price_beam_body(int b, const double *vstar, const double *row_absmax,
+                                                const int32_t *__restrict__ beam_row_ptr, double *beam_price,
+                                                double *beam_absmax) {
   const int lane = threadIdx.x & 31;
-  const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  if (b >= n_beams) return;
   double s = 0.0, a = 0.0;
   for (int32_t r = beam_row_ptr[b] + lane; r < beam_row_ptr[b + 1]; r += 32) {
-    s += vstar[r];
-    a = fmax(a, row_absmax[r]);
+    s += __ldcg(vstar + r);
+    a = fmax(a, __ldcg(row_absmax + r));
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
@@ -173,6 +193,13 @@ __global__ void __launch_bounds__(256) k_price_beams(const double *__restrict__ 
     beam_price[b] = s;
     beam_absmax[b] = a;
   }
+}
+
+__global__ void __launch_bounds__(256) k_price_beams(const double *vstar, const double *row_absmax,
+                                                     const int32_t *beam_row_ptr, int32_t n_beams, double *beam_price,
+                                                     double *beam_absmax) {
+  const int b = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (b < n_beams) price_beam_body(b, vstar, row_absmax, beam_row_ptr, beam_price, beam_absmax);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -186,7 +213,7 @@ __global__ void __launch_bounds__(256) k_price_beams(const double *__restrict__ 
 // Outputs per row: the rectangle clipped to the row's beamlets as half-open leaves inside the row, and the
 // sum of w over them.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_price_jaws(const float *__restrict__ w, const int32_t *__restrict__ beam_row_ptr,
+__device__ __forceinline__ void price_jaws_body(const float *__restrict__ w, const int32_t *__restrict__ beam_row_ptr,
                                                     const int32_t *__restrict__ row_bl_ptr,
                                                     const int32_t *__restrict__ row_col0, int32_t width,
                                                     double *__restrict__ vstar, int32_t *__restrict__ left,
@@ -255,6 +282,14 @@ __global__ void __launch_bounds__(256) k_price_jaws(const float *__restrict__ w,
   }
 }
 
+__global__ void __launch_bounds__(256) k_price_jaws(const float *w, const int32_t *beam_row_ptr, const int32_t *row_bl_ptr,
+                                                    const int32_t *row_col0, int32_t width, double *vstar, int32_t *left,
+                                                    int32_t *right, double *beam_price, double *beam_absmax,
+                                                    PriceTail tail) {
+  price_jaws_body(w, beam_row_ptr, row_bl_ptr, row_col0, width, vstar, left, right, beam_price, beam_absmax);
+  if (tail.ticket) price_tail(tail);
+}
+
 // ------------------------------------------------------------------------------------------
 // Interdigitation (reading J2) and connectedness (reading J3) pricing (PAPER.md:260 names the constraints):
 // the feasible apertures of a beam are chains over its leaf rows, so the best one is a shortest path through
@@ -269,7 +304,7 @@ __global__ void __launch_bounds__(256) k_price_jaws(const float *__restrict__ w,
 //   J3: the open rows are consecutive and adjacent open intervals share a lateral position.
 // An open row stays inside its own beamlets.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_price_chain(int32_t mode, const float *__restrict__ w,
+__device__ __forceinline__ void price_chain_body(int32_t mode, const float *__restrict__ w,
                                                      const int32_t *__restrict__ beam_row_ptr,
                                                      const int32_t *__restrict__ row_bl_ptr,
                                                      const int32_t *__restrict__ row_col0, int32_t width, int32_t max_rows,
@@ -411,17 +446,25 @@ __global__ void __launch_bounds__(256) k_price_chain(int32_t mode, const float *
   }
 }
 
+__global__ void __launch_bounds__(256) k_price_chain(int32_t mode, const float *w, const int32_t *beam_row_ptr,
+                                                     const int32_t *row_bl_ptr, const int32_t *row_col0, int32_t width,
+                                                     int32_t max_rows, int32_t *from_g, double *vstar, int32_t *left,
+                                                     int32_t *right, double *beam_price, double *beam_absmax,
+                                                     PriceTail tail) {
+  price_chain_body(mode, w, beam_row_ptr, row_bl_ptr, row_col0, width, max_rows, from_g, vstar, left, right, beam_price,
+                   beam_absmax);
+  if (tail.ticket) price_tail(tail);
+}
+
 // step 6b: b* = argmin_b price_b (ties: smallest b), optimality test (reading S3), candidate
 // bookkeeping.  One CTA.
-__global__ void __launch_bounds__(256) k_price_select(const double *__restrict__ beam_price,
-                                                      const double *__restrict__ beam_absmax, int32_t n_beams,
-                                                      const int32_t *__restrict__ beam_row_ptr,
-                                                      const int32_t *__restrict__ left,
-                                                      const int32_t *__restrict__ right, int32_t *best_out,
-                                                      DevState *st, double price_tol, int32_t k_max,
-                                                      int32_t max_rows, const int32_t *__restrict__ ap_beam,
-                                                      const int32_t *__restrict__ ap_left,
-                                                      const int32_t *__restrict__ ap_right) {
+// (a device function run by one CTA of 256 threads: the tail of the pricing launch, or k_price_select; what other
+// CTAs of the same launch wrote is read with __ldcg)
+__device__ void price_select_body(const double *beam_price, const double *beam_absmax, int32_t n_beams,
+                                  const int32_t *__restrict__ beam_row_ptr, const int32_t *left, const int32_t *right,
+                                  int32_t *best_out, DevState *st, double price_tol, int32_t k_max, int32_t max_rows,
+                                  const int32_t *ap_beam, const int32_t *ap_left, const int32_t *ap_right,
+                                  const unsigned long long *ap_hash) {
   __shared__ double sv[256];
   __shared__ int32_t sb[256];
   __shared__ double sa[256];
@@ -430,9 +473,9 @@ __global__ void __launch_bounds__(256) k_price_select(const double *__restrict__
   double bv = CUDART_INF, am = 0.0;
   int32_t bb = 0x7fffffff;
   for (int32_t b = t; b < n_beams; b += 256) {
-    const double v = beam_price[b];
+    const double v = __ldcg(beam_price + b);
     if (v < bv) { bv = v; bb = b; }     // ascending b within a thread: ties keep the smaller b
-    am = fmax(am, beam_absmax[b]);
+    am = fmax(am, __ldcg(beam_absmax + b));
   }
   sv[t] = bv; sb[t] = bb; sa[t] = am;
   __syncthreads();
@@ -452,25 +495,33 @@ __global__ void __launch_bounds__(256) k_price_select(const double *__restrict__
   if (st == nullptr) return;
   // candidate bookkeeping
   const int32_t r0 = beam_row_ptr[best], r1 = beam_row_ptr[best + 1];
+  __shared__ unsigned long long s_hash[256];
   int32_t cnt = 0;
-  for (int32_t r = r0 + t; r < r1; r += 256) cnt += right[r] - left[r];
+  unsigned long long hsh = 0ull;
+  for (int32_t r = r0 + t; r < r1; r += 256) {
+    const int32_t l = __ldcg(left + r), rr = __ldcg(right + r);
+    cnt += rr - l;
+    hsh += leaf_hash(r - r0, l, rr);
+  }
   s_cnt[t] = cnt;
+  s_hash[t] = hsh;
   __syncthreads();
   for (int o = 128; o > 0; o >>= 1) {
-    if (t < o) s_cnt[t] += s_cnt[t + o];
+    if (t < o) { s_cnt[t] += s_cnt[t + o]; s_hash[t] += s_hash[t + o]; }
     __syncthreads();
   }
+  const unsigned long long cand_hash = s_hash[0] + beam_hash(best);
   // duplicate of an aperture already in the pool? (reading S6: counted; it ends the column generation, see below)
   __shared__ int32_t s_dup;
   if (t == 0) s_dup = 0;
   __syncthreads();
   const int32_t K = st->K;
   for (int32_t k = 0; k < K; ++k) {
-    if (ap_beam[k] != best) continue;
+    if (ap_beam[k] != best || ap_hash[k] != cand_hash) continue;     // hash first (uniform), then verify leaf by leaf
     int32_t diff = 0;
     for (int32_t r = r0 + t; r < r1; r += 256) {
       const int32_t m = r - r0;
-      diff |= (ap_left[k * max_rows + m] != left[r]) | (ap_right[k * max_rows + m] != right[r]);
+      diff |= (ap_left[k * max_rows + m] != __ldcg(left + r)) | (ap_right[k * max_rows + m] != __ldcg(right + r));
     }
     const int any = __syncthreads_or(diff);
     if (!any && t == 0) s_dup = 1;
@@ -490,6 +541,7 @@ __global__ void __launch_bounds__(256) k_price_select(const double *__restrict__
     if (improving && s_dup) done = (!st->m_hit_max && -price <= 10.0 * fmax(st->m_kkt, tol_abs)) ? 1 : 2;
     if (s_dup) st->n_duplicates += 1;
     st->cand_beam = best;
+    st->cand_hash = cand_hash;
     st->cand_price = price;
     st->w_abs_max = absmax;
     st->cand_nopen = s_cnt[0];
@@ -497,6 +549,68 @@ __global__ void __launch_bounds__(256) k_price_select(const double *__restrict__
     st->done = done;
     st->cand_valid = (done == 0 && K < k_max) ? 1 : 0;
   }
+}
+
+__global__ void __launch_bounds__(256) k_price_select(const double *beam_price, const double *beam_absmax, int32_t n_beams,
+                                                      const int32_t *beam_row_ptr, const int32_t *left,
+                                                      const int32_t *right, int32_t *best_out, DevState *st,
+                                                      double price_tol, int32_t k_max, int32_t max_rows,
+                                                      const int32_t *ap_beam, const int32_t *ap_left,
+                                                      const int32_t *ap_right, const unsigned long long *ap_hash) {
+  price_select_body(beam_price, beam_absmax, n_beams, beam_row_ptr, left, right, best_out, st, price_tol, k_max, max_rows,
+                    ap_beam, ap_left, ap_right, ap_hash);
+}
+
+// the candidate becomes column K of the pool tables; its 0/1 beamlet mask is the x of step 7 (a_K = D 1_A)
+__device__ void append_body(int32_t i0, int32_t stride, const DevState *st, int32_t n_bl, int32_t max_rows,
+                            const int32_t *__restrict__ bl_row, const int32_t *__restrict__ row_beam,
+                            const int32_t *__restrict__ beam_row_ptr, const int32_t *__restrict__ row_bl_ptr,
+                            const int32_t *left, const int32_t *right, int32_t *ap_beam, int32_t *ap_left,
+                            int32_t *ap_right, unsigned long long *ap_hash, float *xmask) {
+  if (!st->cand_valid) return;
+  const int32_t K = st->K, b = st->cand_beam;
+  const int32_t r0 = beam_row_ptr[b], nr = beam_row_ptr[b + 1] - r0;
+  const int32_t n = (xmask != nullptr && n_bl > max_rows) ? n_bl : max_rows;
+  for (int32_t i = i0; i < n; i += stride) {
+    if (xmask != nullptr && i < n_bl) {
+      const int32_t r = bl_row[i];
+      float m = 0.f;
+      if (row_beam[r] == b) {
+        const int32_t c = i - row_bl_ptr[r];
+        m = (c >= __ldcg(left + r) && c < __ldcg(right + r)) ? 1.f : 0.f;
+      }
+      xmask[i] = m;
+    }
+    if (i == 0) { ap_beam[K] = b; ap_hash[K] = st->cand_hash; }
+    if (i < max_rows) {
+      ap_left[K * max_rows + i] = i < nr ? __ldcg(left + r0 + i) : 0;
+      ap_right[K * max_rows + i] = i < nr ? __ldcg(right + r0 + i) : 0;
+    }
+  }
+}
+
+__device__ void price_tail(const PriceTail &q) {
+  __shared__ bool s_last;
+  const int t = threadIdx.x;
+  __threadfence();
+  __syncthreads();
+  if (t == 0) s_last = atomicAdd(q.ticket, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!s_last) return;
+  if (t == 0) *q.ticket = 0u;
+  __threadfence();
+  if (q.do_beams) {
+    for (int b = t >> 5; b < q.n_beams; b += 8) price_beam_body(b, q.vstar, q.row_absmax, q.beam_row_ptr, q.beam_price, q.beam_absmax);
+    __threadfence_block();
+    __syncthreads();
+  }
+  price_select_body(q.beam_price, q.beam_absmax, q.n_beams, q.beam_row_ptr, q.left, q.right, q.best_out, q.st, q.price_tol,
+                    q.k_max, q.max_rows, q.ap_beam, q.ap_left, q.ap_right, q.ap_hash);
+  if (q.st == nullptr) return;
+  __threadfence_block();
+  __syncthreads();
+  append_body(t, 256, q.st, q.n_bl, q.max_rows, q.bl_row, q.row_beam, q.beam_row_ptr, q.row_bl_ptr, q.left, q.right, q.ap_beam,
+              q.ap_left, q.ap_right, q.ap_hash, q.xmask);
 }
 
 size_t chain_pricing_smem(int32_t max_rows, int32_t width) {
@@ -509,6 +623,17 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
                            double *row_absmax, double *beam_price, double *beam_absmax, int32_t *best_out,
                            bool update_state, int32_t max_row_len) {
   const int wpb = 8;
+  PriceTail tl{};
+  tl.ticket = &c->d.state->ticket_misc;
+  tl.n_beams = n_beams; tl.n_rows = n_rows; tl.n_bl = c->n_bl; tl.max_rows = c->max_rows_per_beam; tl.k_max = c->opt.k_max;
+  tl.beam_row_ptr = beam_row_ptr; tl.row_bl_ptr = row_bl_ptr; tl.bl_row = c->d.bl_row; tl.row_beam = c->d.row_beam;
+  tl.vstar = vstar; tl.row_absmax = row_absmax; tl.beam_price = beam_price; tl.beam_absmax = beam_absmax;
+  tl.left = left; tl.right = right; tl.best_out = best_out;
+  tl.st = update_state ? c->d.state : nullptr;
+  tl.price_tol = c->opt.price_tol;
+  tl.ap_beam = c->d.ap_beam; tl.ap_left = c->d.ap_left; tl.ap_right = c->d.ap_right; tl.ap_hash = c->d.ap_hash;
+  tl.xmask = spmv_builds_mask(c) ? nullptr : c->d.xmask;
+  c->cand_appended = false;
   if (c->opt.mlc_mode == DAO_MLC_JAWS_ONLY) {
     // the context's own MLC tables only (dao_price_from_w refuses caller tables in this mode)
     const size_t smem = (size_t)c->max_rows_per_beam * (size_t)(c->max_beam_width + 1) * sizeof(double);
@@ -516,56 +641,68 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
     if (e != cudaSuccess) return e;
     ++c->n_launches;
     k_price_jaws<<<n_beams, 256, smem, c->stream>>>(w, beam_row_ptr, row_bl_ptr, c->d.row_col0, c->max_beam_width, vstar,
-                                                    left, right, beam_price, beam_absmax);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-  } else if (c->opt.mlc_mode == DAO_MLC_INTERDIGITATION || c->opt.mlc_mode == DAO_MLC_CONNECTED) {
+                                                    left, right, beam_price, beam_absmax, tl);
+    c->cand_appended = update_state;
+    return cudaGetLastError();
+  }
+  if (c->opt.mlc_mode == DAO_MLC_INTERDIGITATION || c->opt.mlc_mode == DAO_MLC_CONNECTED) {
     const size_t smem = chain_pricing_smem(c->max_rows_per_beam, c->max_beam_width);
     cudaError_t e = cudaFuncSetAttribute(k_price_chain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     ++c->n_launches;
     k_price_chain<<<n_beams, 256, smem, c->stream>>>(c->opt.mlc_mode, w, beam_row_ptr, row_bl_ptr, c->d.row_col0,
                                                      c->max_beam_width, c->max_rows_per_beam, c->d.chain_from, vstar, left, right,
-                                                     beam_price, beam_absmax);
+                                                     beam_price, beam_absmax, tl);
+    c->cand_appended = update_state;
+    return cudaGetLastError();
+  }
+  // max_row_len > 0: known on the host (the context's own tables); < 0: caller tables, decided on the device
+  const bool seq_possible = n_rows >= kPriceSeqMinRows && max_row_len != 0;
+  if (!seq_possible && n_rows > 0) {
+    // the usual case (a few hundred leaf rows): ONE launch, warp per row + the tail in the last CTA
+    tl.do_beams = 1;
+    ++c->n_launches;
+    k_price_rows<<<(n_rows + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(w, row_bl_ptr, n_rows, vstar, left, right, row_absmax,
+                                                                      nullptr, tl);
+    c->cand_appended = update_state;
+    return cudaGetLastError();
+  }
+  // many rows (the 10^4-10^5-row end of configs[3]): thread-per-row kernel where the rows are short enough, separate
+  // beam-sum and selection launches
+  PriceTail none{};
+  const int32_t *flag = nullptr;
+  if (seq_possible && max_row_len < 0) {
+    int32_t *f = &c->d.state->price_maxlen;
+    cudaError_t e = cudaMemsetAsync(f, 0, sizeof(int32_t), c->stream);
+    if (e != cudaSuccess) return e;
+    ++c->n_launches;
+    k_price_maxlen<<<std::min((n_rows + 255) / 256, c->n_sm * 4), 256, 0, c->stream>>>(row_bl_ptr, n_rows, f);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-  } else {
-    // max_row_len > 0: known on the host (the context's own tables); < 0: caller tables, decided on the device
-    const bool seq_possible = n_rows >= kPriceSeqMinRows && max_row_len != 0;
-    const int32_t *flag = nullptr;
-    if (seq_possible && max_row_len < 0) {
-      int32_t *f = &c->d.state->price_maxlen;
-      cudaError_t e = cudaMemsetAsync(f, 0, sizeof(int32_t), c->stream);
-      if (e != cudaSuccess) return e;
-      ++c->n_launches;
-      k_price_maxlen<<<std::min((n_rows + 255) / 256, c->n_sm * 4), 256, 0, c->stream>>>(row_bl_ptr, n_rows, f);
-      e = cudaGetLastError();
-      if (e != cudaSuccess) return e;
-      flag = f;
-    }
-    if (seq_possible && (flag || max_row_len <= kPriceSeqMaxLen)) {
-      ++c->n_launches;
-      k_price_rows_seq<<<(n_rows + 127) / 128, 128, 0, c->stream>>>(w, row_bl_ptr, n_rows, vstar, left, right, row_absmax, flag);
-      cudaError_t e = cudaGetLastError();
-      if (e != cudaSuccess) return e;
-    }
-    if (n_rows > 0 && (!seq_possible || flag || max_row_len > kPriceSeqMaxLen)) {
-      ++c->n_launches;
-      k_price_rows<<<(n_rows + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(w, row_bl_ptr, n_rows, vstar, left,
-                                                                        right, row_absmax, flag);
-      cudaError_t e = cudaGetLastError();
-      if (e != cudaSuccess) return e;
-    }
+    flag = f;
+  }
+  if (seq_possible && (flag || max_row_len <= kPriceSeqMaxLen)) {
     ++c->n_launches;
-    k_price_beams<<<(n_beams + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(vstar, row_absmax, beam_row_ptr, n_beams,
-                                                                         beam_price, beam_absmax);
+    k_price_rows_seq<<<(n_rows + 127) / 128, 128, 0, c->stream>>>(w, row_bl_ptr, n_rows, vstar, left, right, row_absmax, flag);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  if (n_rows > 0 && (!seq_possible || flag || max_row_len > kPriceSeqMaxLen)) {
+    ++c->n_launches;
+    k_price_rows<<<(n_rows + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(w, row_bl_ptr, n_rows, vstar, left, right, row_absmax,
+                                                                      flag, none);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }
   ++c->n_launches;
+  k_price_beams<<<(n_beams + wpb - 1) / wpb, wpb * 32, 0, c->stream>>>(vstar, row_absmax, beam_row_ptr, n_beams, beam_price,
+                                                                       beam_absmax);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  ++c->n_launches;
   k_price_select<<<1, 256, 0, c->stream>>>(beam_price, beam_absmax, n_beams, beam_row_ptr, left, right, best_out,
                                            update_state ? c->d.state : nullptr, c->opt.price_tol, c->opt.k_max,
-                                           c->max_rows_per_beam, c->d.ap_beam, c->d.ap_left, c->d.ap_right);
+                                           c->max_rows_per_beam, c->d.ap_beam, c->d.ap_left, c->d.ap_right, c->d.ap_hash);
   return cudaGetLastError();
 }
 
@@ -573,41 +710,26 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
 // Append the pending candidate to the pool tables at index K and write its 0/1 beamlet mask
 // (the x of step 7, a_K = D 1_A).  The pool size itself is advanced by the master kernel.
 // ------------------------------------------------------------------------------------------
-__global__ void k_append_candidate(const DevState *__restrict__ st, int32_t n_bl, int32_t max_rows,
-                                   const int32_t *__restrict__ bl_row, const int32_t *__restrict__ row_beam,
-                                   const int32_t *__restrict__ beam_row_ptr,
-                                   const int32_t *__restrict__ row_bl_ptr, const int32_t *__restrict__ left,
-                                   const int32_t *__restrict__ right, int32_t *__restrict__ ap_beam,
-                                   int32_t *__restrict__ ap_left, int32_t *__restrict__ ap_right,
-                                   float *__restrict__ xmask) {
-  if (!st->cand_valid) return;
-  const int32_t K = st->K, b = st->cand_beam;
-  const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n_bl) {
-    const int32_t r = bl_row[i];
-    float m = 0.f;
-    if (row_beam[r] == b) {
-      const int32_t c = i - row_bl_ptr[r];
-      m = (c >= left[r] && c < right[r]) ? 1.f : 0.f;
-    }
-    xmask[i] = m;
-  }
-  const int32_t r0 = beam_row_ptr[b], nr = beam_row_ptr[b + 1] - r0;
-  if (i == 0) ap_beam[K] = b;
-  if (i < max_rows) {
-    ap_left[K * max_rows + i] = i < nr ? left[r0 + i] : 0;
-    ap_right[K * max_rows + i] = i < nr ? right[r0 + i] : 0;
-  }
+__global__ void k_append_candidate(const DevState *st, int32_t n_bl, int32_t max_rows, const int32_t *bl_row,
+                                   const int32_t *row_beam, const int32_t *beam_row_ptr, const int32_t *row_bl_ptr,
+                                   const int32_t *left, const int32_t *right, int32_t *ap_beam, int32_t *ap_left,
+                                   int32_t *ap_right, unsigned long long *ap_hash, float *xmask) {
+  append_body(blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, st, n_bl, max_rows, bl_row, row_beam,
+              beam_row_ptr, row_bl_ptr, left, right, ap_beam, ap_left, ap_right, ap_hash, xmask);
 }
 
 cudaError_t launch_append_candidate(Ctx *c) {
+  if (c->cand_appended) {                 // the pricing launch already appended its winner (price_tail)
+    c->cand_appended = false;
+    return cudaSuccess;
+  }
   const int t = 128;
   const int n = c->n_bl > c->max_rows_per_beam ? c->n_bl : c->max_rows_per_beam;
   ++c->n_launches;
   k_append_candidate<<<(n + t - 1) / t, t, 0, c->stream>>>(c->d.state, c->n_bl, c->max_rows_per_beam, c->d.bl_row,
                                                            c->d.row_beam, c->d.beam_row_ptr, c->d.row_bl_ptr,
                                                            c->d.left, c->d.right, c->d.ap_beam, c->d.ap_left,
-                                                           c->d.ap_right, c->d.xmask);
+                                                           c->d.ap_right, c->d.ap_hash, c->d.xmask);
   return cudaGetLastError();
 }
 

@@ -142,6 +142,7 @@ static void carve_workspace(Carver &cv, const Dims &dm, const HostLayout &L, Dev
   d->beam_price = cv.take<double>((size_t)dm.n_beams);
   d->beam_absmax = cv.take<double>((size_t)dm.n_beams);
   d->ap_beam = cv.take<int32_t>((size_t)dm.k_max);
+  d->ap_hash = cv.take<unsigned long long>((size_t)dm.k_max);
   d->ap_left = cv.take<int32_t>((size_t)dm.k_max * dm.max_rows);
   d->ap_right = cv.take<int32_t>((size_t)dm.k_max * dm.max_rows);
   const NewtonLayout nl = layout_of_master(dm, L.n_vox_pad);
@@ -775,6 +776,7 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   SETUP_CUDA(cudaMemsetAsync(d.m_epoch, 0, 64 * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.m_prof, 0, kMasterProfSlots * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.ap_beam, 0, (size_t)dm.k_max * 4, q));
+  SETUP_CUDA(cudaMemsetAsync(d.ap_hash, 0, (size_t)dm.k_max * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.ap_left, 0, (size_t)dm.k_max * dm.max_rows * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.ap_right, 0, (size_t)dm.k_max * dm.max_rows * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.history, 0, (size_t)dm.k_max * sizeof(dao_iter_record), q));

@@ -35,6 +35,7 @@ __global__ void k_intensity(const DevState *__restrict__ st, int32_t n_bl, int32
 }
 
 cudaError_t launch_intensity(Ctx *c) {
+  if (c->x_current) return cudaSuccess;   // the master kernel already wrote x for this y
   const int t = 128;
   ++c->n_launches;
   k_intensity<<<(c->n_bl + t - 1) / t, t, 0, c->stream>>>(c->d.state, c->n_bl, c->max_rows_per_beam,
@@ -72,7 +73,22 @@ struct SpmvParams {
   // column mode: layout of the dose block A (a_index) and the column to write (< 0: the pool size K)
   int32_t a_T, a_TP, a_col;
   int64_t a_stride;
+  // column mode with a_col < 0: x is the 0/1 mask of the pending candidate, built while x is staged (no mask array,
+  // no extra pass): beamlet i is open iff its leaf row belongs to the candidate's beam and i lies in [left, right)
+  const int32_t *bl_row, *row_beam, *row_bl_ptr, *left, *right;
+  int32_t mask_from_candidate;
 };
+
+template <int MODE>
+__device__ __forceinline__ float spmv_x_of(const SpmvParams &p, int i, int cand_beam) {
+  if (MODE == kSpmvColumn && p.mask_from_candidate) {
+    const int32_t r = p.bl_row[i];
+    if (p.row_beam[r] != cand_beam) return 0.f;
+    const int32_t c = i - p.row_bl_ptr[r];
+    return (c >= p.left[r] && c < p.right[r]) ? 1.f : 0.f;
+  }
+  return p.x[i];
+}
 
 // per-row epilogue: objective / gradient (step 3) or plain store
 template <int MODE>
@@ -215,7 +231,10 @@ __global__ void __launch_bounds__(kSpmvRingThreads, 1) k_spmv_ring(SpmvParams p)
   for (int s = 0; s < kRingStages; ++s) issue();
 
   // x and the penalty table are staged while the first chunks are in flight
-  for (int i = threadIdx.x; i < p.n_bl; i += blockDim.x) xs[i] = p.x[i];
+  {
+    const int cand_beam = (MODE == kSpmvColumn && p.mask_from_candidate) ? p.st->cand_beam : 0;
+    for (int i = threadIdx.x; i < p.n_bl; i += blockDim.x) xs[i] = spmv_x_of<MODE>(p, i, cand_beam);
+  }
   if (MODE == kSpmvObjective) {
     for (int i = threadIdx.x; i < 256; i += blockDim.x) stab_s[i] = p.stab[i];
   }
@@ -266,7 +285,8 @@ __global__ void __launch_bounds__(kSpmvThreads, 2) k_spmv_sell(SpmvParams p) {
     }
   }
   if (XS) {
-    for (int i = threadIdx.x; i < p.n_bl; i += blockDim.x) xs[i] = p.x[i];
+    const int cand_beam = (MODE == kSpmvColumn && p.mask_from_candidate) ? p.st->cand_beam : 0;
+    for (int i = threadIdx.x; i < p.n_bl; i += blockDim.x) xs[i] = spmv_x_of<MODE>(p, i, cand_beam);
   }
   if (MODE == kSpmvObjective) {
     for (int i = threadIdx.x; i < 256; i += blockDim.x) stab_s[i] = p.stab[i];
@@ -329,6 +349,8 @@ static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out, const in
   p.skip = skip;
   p.a_T = c->nwt.T; p.a_TP = c->nwt.TP; p.a_stride = c->nwt.tile_stride; p.a_col = a_col;
   if (MODE == kSpmvColumn) p.out = c->d.A;
+  p.bl_row = c->d.bl_row; p.row_beam = c->d.row_beam; p.row_bl_ptr = c->d.row_bl_ptr; p.left = c->d.left; p.right = c->d.right;
+  p.mask_from_candidate = (MODE == kSpmvColumn && a_col < 0 && spmv_builds_mask(c)) ? 1 : 0;
   ++c->n_launches;
   if (c->spmv_ring_warps > 0) {
     const int nw = c->spmv_ring_warps;
