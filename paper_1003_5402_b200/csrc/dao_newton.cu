@@ -7,16 +7,20 @@
 // (the optimal value) is unique by convexity, and the stopping test is the one of methods 0/1 and of the
 // oracle (reading S2), so parity is unaffected by the choice of method.
 //
-// ONE persistent cooperative kernel, one CTA per SM (16 worker warps + 1 producer warp).  The dose
-// block is stored tiled (NewtonLayout): the K live columns of a tile of T voxels are one contiguous
-// range, fetched by ONE cp.async.bulk (1-D TMA) into a stage of a shared-memory ring.  With all K
-// columns of a tile resident, one pass computes EVERYTHING at a trial point y:
+// ONE persistent cooperative kernel, one CTA per SM, 16 warps (128 registers each).  The dose block is
+// stored tiled (NewtonLayout): the K live columns of a tile of T voxels are one contiguous range,
+// fetched by ONE cp.async.bulk (1-D TMA) into a stage of a shared-memory ring (issued by lane 0 of an
+// otherwise idle back warp).  With all K columns of a tile resident, one pass computes EVERYTHING at a
+// trial point y; the warps are specialised:
+//  front warps (8):
 //   Z  z_j = sum_k y_k A[k][j]                        (fp64, thread per voxel and k-slice)
 //   P  F, pi_j = dF/dz_j, s_j = 2 c_j, list of the active voxels (s_j != 0) of the tile
-//   H  the augmented Gram matrix  [A; pi/s]-style:  H[k1][k2] += sum_j A[k1][j] s_j A[k2][j]  and
-//      grad[k1] += sum_j A[k1][j] pi_j  as one extra column, over the ACTIVE voxels only, on the fp64
-//      tensor cores (mma.sync m8n8k4 f64: 8x8 blocks of H, 4 voxels per instruction; every warp owns a
-//      fixed set of blocks whose accumulators stay in registers for the whole pass)
+//   W  the fp64 tile  W[k][a] = sqrt(s_a) A[k][a]  (k < K),  W[K][a] = pi_a / sqrt(s_a)  over chunks of AC
+//      ACTIVE voxels (fp32 -> fp64 on the integer pipe), double buffered in shared memory
+//  back warps (8):
+//   H  [H, grad] += W W^T on the fp64 tensor cores (mma.sync m8n8k4 f64: 8x8 blocks, 4 voxels per
+//      instruction; every warp owns fixed strips of 1x5 blocks whose accumulators stay in registers for
+//      the whole pass).  H[k1][k2] = sum_j A[k1][j] s_j A[k2][j],  grad[k] = sum_j A[k][j] pi_j (row K).
 // then one grid reduction of (H, grad, F) through flagged slots (dao_grid_reduce.cuh), and every CTA
 // computes the same Newton step on the free set {k : y_k > 0 or grad_k < 0} by an LDL^T factorisation
 // in shared memory.  The trial point y + t d (t = 1 unless a bound is hit first) is accepted on
@@ -55,9 +59,7 @@ struct NewtonParams {
   int32_t lbuf_doubles;      // capacity of the factorisation buffer (also holds the W tile)
   int32_t AC;                // active voxels per chunk of the H phase (power of two)
   int32_t w_doubles;         // doubles per W tile: (8 nb_max + 1) (AC + 4)
-  int32_t srow;              // 8 nb_max
   int32_t ks_shift;          // log2 of the k-slices per voxel of the dose loop: T << ks_shift = 256 front threads
-  int32_t debug;             // timing experiments only (dao_options.reserved >> 3): 1 no DMMA, 2 no W conversion, 4 no Z loop
   int32_t n_struct;
   const uint8_t *sid;
   const float *vt;           // per-voxel thresholds T_j (re-optimisation mode) or null
@@ -332,8 +334,8 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
         if (ti_ < ntl) {
           const int vg = (tb0 + (rev ? ntl - 1 - ti_ : ti_) * tstep) * T + v0;
           if (zsl == 0 && vg < p.n_vox_pad) {
-            if (p.debug & 16) sid_n = (vg & 7) == 0 ? 0 : kNoStruct;      // timing experiment: no global load
-            else { sid_n = p.sid[vg]; if (p.vt) vt_n = p.vt[vg]; }
+            sid_n = p.sid[vg];
+            if (p.vt) vt_n = p.vt[vg];
           }
         }
       };
@@ -368,7 +370,7 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
           const double *py = yv + zsl;
           float f[4];
           double yk[4];
-          if (!(p.debug & 4)) {
+          {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
               const int ii = max(min(u, nI - 1), 0);
@@ -432,7 +434,7 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
               gq0 = sq0 * ((un > 0.0 && ov > 0.0) ? gv / sv : (un > 0.0 ? -un : ov));
             }
           }
-          if (!(p.debug & 8)) p.mz[vg0] = z0;
+          p.mz[vg0] = z0;
         }
         const unsigned m0 = __ballot_sync(0xffffffffu, act0);
         if (lane == 0) wcnt_s[warp] = __popc(m0);
@@ -463,7 +465,7 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
           {
             // thread = (column a, row parity); the voxel of the column is looked up once
             const int a = tid & (AC - 1), kpar = tid >> ac_shift, kstep = kNwtFrontThreads >> ac_shift;
-            if (a < nca4 && !(p.debug & 2)) {
+            if (a < nca4) {
               const bool live = a < nca;
               const double sqa = live ? ss[c0 + a] : 0.0;
               const float *src = M + (live ? (int)list[c0 + a] : 0);
@@ -516,7 +518,7 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
           const int nq = (meta & 0xffff) >> 2;
           const double *wt = wbuf + (size_t)wp.stage * w_doubles;
           const uint32_t wt_s = smem_addr(wt);
-          for (int qd = grp; qd < ((p.debug & 1) ? 0 : nq); qd += NG) {
+          for (int qd = grp; qd < nq; qd += NG) {
             const uint32_t wq = wt_s + (uint32_t)(qd * 4 + (lane & 3)) * 8u;
 #pragma unroll
             for (int s = 0; s < kNwtStrips; ++s) {
@@ -1015,8 +1017,6 @@ cudaError_t launch_newton(Ctx *c, bool add_candidate) {
   p.lbuf_doubles = L.lbuf_doubles;
   p.AC = L.AC;
   p.w_doubles = (8 * L.nb_max + 1) * (L.AC + 4);
-  p.srow = 8 * L.nb_max;
-  p.debug = c->opt.reserved >> 3;
   p.ks_shift = 0;
   while ((L.T << p.ks_shift) < kNwtFrontThreads) ++p.ks_shift;
   p.n_struct = std::max(c->n_struct, 1);

@@ -125,7 +125,7 @@ __global__ void __launch_bounds__(256) k_price_rows(const float *w, const int32_
 // step 5 for MANY leaf rows (the 10^4-10^5-row end of BASELINE.json configs[3]): thread per row, which is the
 // paper's own launch shape, but fed through shared memory: a warp copies the beamlets of its 32
 // consecutive rows (one contiguous slice of w) with coalesced loads, then every lane runs the printed scan
-// over its own row sequentially in fp64 -- literally the oracle's loop, strict comparisons
+// over its own row sequentially in fp64 -- the paper's loop as printed, strict comparisons
 // included, so ties and sums agree bit for bit.  The warp-per-row kernel above stays in use for few rows
 // (lower latency) and for rows too long for the staging buffer.
 // ------------------------------------------------------------------------------------------
