@@ -134,9 +134,12 @@ typedef struct {
   int32_t master_method;     /* 0 = plain gradient projection, 1 = gradient projection with conjugate
                                 (Polak-Ribiere+) directions on the free face, 2 = projected Newton on the free
                                 variables (exact Hessian A^T diag(2c) A of the piecewise-quadratic F on the fp64
-                                tensor cores, one pass over A per iteration; default 2; pools of more than 103
-                                apertures use method 1).  Same stopping test and the same (unique) optimal
-                                value for all three; reading S2 */
+                                tensor cores, one pass over A per iteration), 3 = the same projected Newton method
+                                with the Hessian on the 5th-generation tensor cores (tcgen05, TF32 hi/lo split,
+                                TMEM accumulators: H to ~2^-21 relative; dose, objective and gradient -- all
+                                that enters the stopping test -- stay fp64); pools of more than 103 apertures
+                                use method 1.  Same stopping test and the same (unique) optimal value for all
+                                four; reading S2 */
   int32_t sell_sigma;        /* sorting window (rows) of the internal sliced-ELL layout of D; 1 = keep the
                                 caller's voxel order; 0 = library default */
   int32_t timers;            /* non-zero: CUDA-event timers per kernel class in dao_run (default 1) */

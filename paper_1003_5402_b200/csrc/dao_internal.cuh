@@ -66,6 +66,14 @@ struct NewtonLayout {
   int32_t AC = 0;           // active voxels per chunk of the Hessian phase
   int32_t lbuf_doubles = 0; // shared buffer of the LDL^T factorisation and of the fp64 tile W of the Hessian phase
   size_t smem = 0;          // dynamic shared memory of k_master_newton
+  // master_method = 3: the Hessian on the 5th-generation tensor cores (tcgen05, TF32 hi/lo split, TMEM accumulators)
+  int32_t tc = 0;           // 1: k_master_newton<true>
+  int32_t kp = 0;           // rows of one half (hi or lo) of the operand tile: 64 (k_max <= 56) or 128
+  int32_t lbo = 0;          // bytes between the two 16-byte K-halves of an MMA k-step (core matrices adjacent along the voxels)
+  int32_t sbo = 0;          // bytes between groups of 8 operand rows
+  int32_t w_bytes = 0;      // bytes of one operand tile: (2 kp / 8) sbo
+  int32_t tmem_cols = 0;    // TMEM columns allocated per CTA (power of two >= 32)
+  int32_t meta_rows = 0;    // rows of TP floats at the head of every tile (structure ids, thresholds) before column 0
 };
 
 // ------------------------------------------------------------------------------------------
@@ -310,9 +318,10 @@ cudaError_t master_configure(Ctx *c);
 cudaError_t launch_master(Ctx *c, bool add_candidate);
 
 // dao_newton.cu (method 2)
-NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct);   // host only, no device query
+NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct, bool tc);   // host only, no device query
 cudaError_t newton_configure(Ctx *c);
 cudaError_t launch_newton(Ctx *c, bool add_candidate);
+cudaError_t newton_fill_tile_meta(Ctx *c);   // method 3: writes the meta rows of the tiled dose block (after sid / vt are set)
 
 // Position of (internal voxel i, aperture column k) in the dose block A (floats)
 __host__ __device__ __forceinline__ size_t a_index(int32_t tile_T, int32_t tile_TP, int64_t tile_stride,

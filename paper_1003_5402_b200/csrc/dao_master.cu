@@ -753,7 +753,7 @@ static size_t master_fixed_smem(const Ctx *c, int n_stages) {
 }
 
 cudaError_t master_configure(Ctx *c) {
-  if (c->opt.master_method == 2) return newton_configure(c);
+  if (c->opt.master_method >= 2) return newton_configure(c);
   c->master_grid = std::min(c->n_sm * kMasterCtasPerSm, kMasterMaxGrid);
   int slab = (c->n_vox_pad + c->master_grid - 1) / c->master_grid;
   slab = (slab + 127) / 128 * 128;
@@ -793,7 +793,7 @@ cudaError_t master_configure(Ctx *c) {
 }
 
 cudaError_t launch_master(Ctx *c, bool add_candidate) {
-  if (c->opt.master_method == 2) return launch_newton(c, add_candidate);
+  if (c->opt.master_method >= 2) return launch_newton(c, add_candidate);
   c->x_current = false;                    // methods 0 / 1 leave step 1 (beamlet intensities) to k_intensity
   MasterParams p{};
   p.A = c->d.A;

@@ -33,6 +33,8 @@
 #include <math_constants.h>
 
 #include <algorithm>
+#include <cstdlib>
+#include <cstdio>
 
 namespace dao {
 
@@ -46,6 +48,21 @@ constexpr int kNwtMinStages = DAO_NWT_MIN_STAGES;   // ring stages a layout must
 constexpr int kNwtFront = 8;             // front warps: dose, penalty, active list, fp64 tile W
 constexpr int kNwtBack = kNW - kNwtFront;   // back warps: H += W W^T on the fp64 tensor cores
 constexpr int kNwtFrontThreads = kNwtFront * 32;
+// master_method = 3 (tensor cores): tiles of 128 voxels, a GROUP of 4 warps per tile (lane = voxel), 4 groups per CTA.
+// A group appends its active voxels to an operand slab of two HALVES of 16 voxels each (filled alternately); a half
+// = rows [Wh (64); Wl (64)] x 16 voxels, K-major core matrices (8 rows x 16 bytes): 128 bytes between voxel quads
+// (LBO), 512 bytes between groups of 8 rows (SBO).  The tile starts with two META rows (structure ids, per-voxel
+// thresholds) so that one bulk copy brings everything a tile needs.
+constexpr int kTcT = 128;
+constexpr int kTcGroupWarps = kTcT / 32;
+constexpr int kTcGroups = kNW / kTcGroupWarps;
+constexpr int kTcHV = 16;                // voxels per half = two MMA k-steps
+constexpr uint32_t kTcLbo = 128, kTcSbo = (kTcHV / 4) * kTcLbo, kTcHalfBytes = 16 * kTcSbo;
+constexpr uint32_t kTcCols = 64;         // TMEM columns: one 128 x 64 fp32 accumulator
+constexpr int kTcMaxK = 56;              // 8 block rows of the augmented Hessian fit the 64 rows of one operand half
+constexpr int kTcMaxStages = 12;
+constexpr int kTcMetaRows = 2;
+constexpr int kNwtAcc = 7;               // gradient accumulators per thread: rows r, r + 8, ... < 56
 
 struct NewtonParams {
   const float *A;            // tiled dose block
@@ -81,10 +98,12 @@ struct NewtonParams {
   int32_t max_iter;
   int32_t k_max;
   double tol;
+  int32_t dbg;
 };
 
 // barrier over the front warps
 __device__ __forceinline__ void fsync() { asm volatile("bar.sync 2, %0;" ::"n"(kNwtFrontThreads) : "memory"); }
+// master_method = 3: every worker warp is a front warp
 
 // fp32 -> fp64 of a finite value >= 0 on the integer pipe (F2F.F64.F32 runs at 16 per clock and SM with ~90
 // cycles of latency, measured): exact for normal numbers; +0 maps to 2^-127 -- the dose loop subtracts exactly
@@ -117,6 +136,53 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                : "d"(a), "d"(b));
 }
 
+// ---- tcgen05 (5th-generation tensor cores): shared-memory operand descriptors, MMA issue, TMEM access ----
+// Operand tiles are K-major ("K" = the contraction index = the voxels of a chunk) without swizzling: a core matrix
+// is 8 rows x 16 bytes stored contiguously (row r at +16 r); `lbo` bytes separate core matrices adjacent along the
+// voxels, `sbo` bytes separate groups of 8 rows.  One kind::tf32 MMA consumes 8 voxels = two core matrices.
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+  return (uint64_t)((saddr >> 4) & 0x3fffu) | ((uint64_t)((lbo >> 4) & 0x3fffu) << 16) |
+         ((uint64_t)((sbo >> 4) & 0x3fffu) << 32) | ((uint64_t)1 << 46);   // descriptor version 1 (sm_100), no swizzle
+}
+// D[tmem] (+)= A[smem] B[smem]^T, M = 128 rows of A, N rows of B (idesc), 8 voxels; fp32 accumulation in TMEM
+__device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// arrives on `bar` when every MMA issued so far by this thread has completed (implies fence::before_thread_sync)
+__device__ __forceinline__ void umma_commit(uint64_t *bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// generic-proxy writes to shared memory become visible to the async proxy (the tensor core reads operands through it)
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// 16 consecutive TMEM columns of this thread's lane (warp w may touch lanes 32 (w % 4) .. + 31 only)
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
+  uint32_t r[16];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n\t"
+      "tcgen05.wait::ld.sync.aligned;"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr)
+      : "memory");
+#pragma unroll
+  for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+__device__ __forceinline__ float tf32_rna(float x) {
+  uint32_t r;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+  return __uint_as_float(r);
+}
+__device__ __forceinline__ void sts_f32(uint32_t addr, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory"); }
+
+// rows of the operand tile a worker thread handles are kpar, kpar + kstep, ...: kstep = 512 / AC
+__device__ __forceinline__ int kstep_of(int ac_shift) { return kMasterWorkers >> ac_shift; }
+
 // index of block (I, J), I <= J < nb, in the row-major enumeration of the upper block triangle
 __host__ __device__ __forceinline__ int blk_index(int nb, int I, int J) { return I * nb - (I * (I - 1)) / 2 + (J - I); }
 
@@ -132,7 +198,14 @@ __device__ __forceinline__ int lidx(int i, int j) { return (i * (i + 1)) / 2 + j
 
 // 16 warps exactly: a 17th (a dedicated producer warp, as in k_master) would be allocated as 20 warps and cap the
 // kernel at 96 registers, which made the compiler serialise the tensor-core loop through one temporary register.
-__global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParams p) {
+// master_method = 3 (TC = true): every worker warp is a front warp and the Hessian runs on the 5th-generation tensor
+// cores -- the front warps write the chunk of active voxels as a TF32 hi/lo operand tile, a 17th CONTROL warp (one
+// thread) feeds the A ring and issues tcgen05.mma (accumulators in TMEM for the whole pass); the gradient A^T pi is
+// accumulated in fp64 by the threads that write the tile.  Only H (which steers the Newton direction and never enters
+// the stopping test) is computed in reduced precision: ~2^-21 relative (3 x TF32), see DESIGN.md section 6.
+constexpr int kNwtTcThreads = kMasterWorkers + 64;   // + the control warp and the feeder warp
+template <bool TC>
+__global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_master_newton(NewtonParams p) {
   extern __shared__ __align__(128) unsigned char dyn_smem[];
   __shared__ double y_s[DAO_MAX_APERTURES];        // accepted point
   __shared__ double ytr_s[DAO_MAX_APERTURES];      // trial point of the current pass
@@ -149,7 +222,18 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
   __shared__ volatile int wmeta_s[2];              // per W buffer: columns (multiple of 4) | last chunk of its tile << 16
   __shared__ double fred_s[kNW];
   __shared__ unsigned long long prof_s[kMasterProfSlots];
+  __shared__ uint32_t tmem_base_s;                 // TC: base address of the TMEM allocation
+  __shared__ volatile int ctrl_cmd_s;              // TC: 1 = another pass follows, 0 = the solve is over
+  __shared__ double ycur_s[DAO_MAX_APERTURES];     // TC: the point of the current pass
+  __shared__ volatile int smeta_s[kTcGroups][2];   // TC: per half message: bit 0 = it holds voxels, bit 1 = last of the pass
+  __shared__ volatile int gcnt_s[kTcGroups][2][kTcGroupWarps];   // TC: active voxels of a tile per warp (double buffered)
+  __shared__ volatile int stop_s;                  // TC: the feeder warp stops issuing
+  __shared__ volatile int wdone_s[kNW];            // TC: tiles this warp has finished since the kernel started
+  __shared__ volatile int gen_s[16];               // TC: copies issued into ring stage s so far (a group may run several uses of
+                                                   // a stage ahead of the feeder: a parity wait alone would alias)
+  __shared__ volatile long long total_tiles_s;     // TC: tiles consumed when the solve ended
 
+  constexpr int NF = kNwtFront;                    // front warps (method 2)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int K0 = p.st->K;
   const int cand = p.st->cand_valid;
@@ -158,7 +242,7 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
   if ((p.add_candidate && !added) || K == 0) {     // converged, pool full or empty pool: nothing to solve
     if (blockIdx.x == 0 && tid == 0) { p.st->m_added = 0; p.st->m_iters = 0; p.st->m_passes = 0; }
     // x for the unchanged y (callers rely on the master leaving x current)
-    for (int i = (int)blockIdx.x * kMasterWorkers + tid; i < p.n_bl; i += (int)gridDim.x * kMasterWorkers) {
+    for (int i = (int)blockIdx.x * kMasterWorkers + tid; tid < kMasterWorkers && i < p.n_bl; i += (int)gridDim.x * kMasterWorkers) {
       const int r = p.bl_row[i], b = p.row_beam[r];
       const int m = r - p.beam_row_ptr[b], c = i - p.row_bl_ptr[r];
       double acc = 0.0;
@@ -185,9 +269,27 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
   uint64_t *full = reinterpret_cast<uint64_t *>(q); q += 128;
   uint64_t *empty = reinterpret_cast<uint64_t *>(q); q += 128;
   uint64_t *wfull = empty + 8, *wempty = empty + 10;   // the two W buffers (n_stages <= 6)
+  // TC: up to 16 stages; per-warp slab barriers; accumulators of a pass complete; next command
+  uint64_t *sfull = nullptr, *sempty = nullptr, *acc_full = nullptr, *go = nullptr;
+  unsigned char *slabs = nullptr, *cl_s = nullptr;
+  double *cpi_s = nullptr, *gpart = nullptr;
+  float *csq_s = nullptr, *lh_s = nullptr;
+  if constexpr (TC) {
+    sfull = reinterpret_cast<uint64_t *>(q); q += 128;
+    sempty = reinterpret_cast<uint64_t *>(q); q += 128;
+    acc_full = reinterpret_cast<uint64_t *>(q); go = acc_full + 1; q += 128;
+    cpi_s = reinterpret_cast<double *>(q); q += kNW * 32 * 8;
+    csq_s = reinterpret_cast<float *>(q); q += kNW * 32 * 4;
+    cl_s = q; q += kNW * 32;
+  }
   StructEntry *stab = reinterpret_cast<StructEntry *>(q); q += align_up_c((size_t)p.n_struct * sizeof(StructEntry), 128);
+  if constexpr (TC) { slabs = q; }                 // 16 slabs; idle between the passes: hred, lbuf, lh, gradient partials live here
   double *hred = reinterpret_cast<double *>(q); q += align_up_c((size_t)p.n_red_cap * 8, 128);
   double *lbuf = reinterpret_cast<double *>(q); q += align_up_c((size_t)p.lbuf_doubles * 8, 128);
+  if constexpr (TC) {
+    lh_s = reinterpret_cast<float *>(q); q += align_up_c((size_t)64 * 65 * 4, 128);
+    gpart = reinterpret_cast<double *>(q); q += (size_t)kNW * 64 * 8;
+  }
   double *wbuf = lbuf;                             // the two W tiles of the H phase share the factorisation buffer
   const int AC = p.AC, WP = p.AC + 4;              // active voxels per chunk, row pitch of W (4 mod 16: conflict-free)
   const int ac_shift = 31 - __clz(AC);
@@ -197,12 +299,151 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
   unsigned short *list = reinterpret_cast<unsigned short *>(q);
 
   if (tid == 0) {
-    for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], kNwtFront); }
-    for (int s = 0; s < 2; ++s) { mbar_init(&wfull[s], kNwtFront); mbar_init(&wempty[s], kNwtBack); }
+    if constexpr (TC) {
+      for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], kTcGroupWarps); }
+      for (int h = 0; h < 2 * kTcGroups; ++h) { mbar_init(&sfull[h], kTcGroupWarps); mbar_init(&sempty[h], 1); }
+      mbar_init(acc_full, 1);
+      mbar_init(go, 1);
+      stop_s = 0;
+      for (int w = 0; w < kNW; ++w) { wdone_s[w] = 0; gen_s[w] = 0; }
+    } else {
+      for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NF); }
+      for (int s = 0; s < 2; ++s) { mbar_init(&wfull[s], NF); mbar_init(&wempty[s], kNwtBack); }
+    }
     for (int i = 0; i < kMasterProfSlots; ++i) prof_s[i] = 0ull;
   }
   fence_mbar_init();
+  if constexpr (TC) {
+    if (warp == kNW) {                             // the control warp owns the TMEM allocation
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_addr(&tmem_base_s)), "r"(kTcCols) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+  }
   __syncthreads();
+  if constexpr (TC) tc_fence_after();
+  const uint32_t tmem_base = TC ? tmem_base_s : 0u;
+
+  // =============================== control and feeder warps (TC) ================================
+  // Warp 16, one thread: takes the operand halves of the groups in a FIXED order (message m of group 0, 1, 2, 3, then
+  // m + 1: independent of timing, so the accumulation order in TMEM is the same in every run) and issues the
+  // tcgen05.mma of each (two k-steps of 8 voxels); tcgen05.commit hands the half back to its group and, after the
+  // last message of a pass, publishes the accumulators (acc_full).  `go` / ctrl_cmd_s: does another pass follow?
+  // Warp 17: lane l owns ring stage l and streams the tiles l, l + NS, ... of the CTA's sequence (one bulk copy per
+  // tile: meta rows + the K live columns); it runs ahead into the next pass and is stopped by stop_s.
+  if constexpr (TC) {
+    if (warp == kNW) {
+      if (lane == 0) {
+        // instruction descriptor: D = F32, A = B = TF32, both K-major, N = 64, M = 128
+        const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((64u >> 3) << 17) | ((128u >> 4) << 24);
+        const uint64_t desc0 = umma_desc(smem_addr(slabs), kTcLbo, kTcSbo);
+        const bool cprof = (p.prof != nullptr) && blockIdx.x == 0;
+        uint32_t par = 0u, go_phase = 0u;            // bit (2 g + b): parity of the next message on half b of group g
+        uint32_t seq = 0u;                           // bit g: which half group g sends next
+        int tiles_seen[kTcGroups];                   // tiles of group g whose halves have all been taken
+#pragma unroll
+        for (int g = 0; g < kTcGroups; ++g) tiles_seen[g] = 0;
+        bool any_mma = false;
+        // one half of group g: meta, the two MMAs, hand the half back; returns true for the last message of the pass
+        auto take = [&](int g) -> bool {
+          const int b = (seq >> g) & 1u, hb = 2 * g + b;
+          par ^= 1u << hb;
+          seq ^= 1u << g;
+          const int meta = smeta_s[g][b];
+          if ((p.dbg & 64) && blockIdx.x == 0) printf("ctl take g %d b %d meta 0x%x seen %d\n", g, b, meta, tiles_seen[g]);
+          if ((meta & 1) && !(p.dbg & 1)) {
+            tc_fence_after();
+            const uint64_t d = desc0 + (uint64_t)((uint32_t)hb * (kTcHalfBytes >> 4));
+            umma_tf32(tmem_base, d, d, idesc, any_mma ? 1u : 0u);
+            umma_tf32(tmem_base, d + (uint64_t)((2u * kTcLbo) >> 4), d + (uint64_t)((2u * kTcLbo) >> 4), idesc, 1u);
+            any_mma = true;
+            umma_commit(&sempty[hb]);
+          } else {
+            mbar_arrive(&sempty[hb]);
+          }
+          if (cprof) prof_s[7] += 1ull;
+          return (meta & 2) != 0;
+        };
+        for (;;) {
+          any_mma = false;
+          // tile rounds: the halves group g completed while it handled its u-th tile of the pass, g = 0, 1, 2, 3 --
+          // the order in which the ring hands out the tiles, so nobody waits for a stage that waits for us
+          for (int u = 0; u * kTcGroups < ntl; ++u) {
+#pragma unroll
+            for (int g = 0; g < kTcGroups; ++g) {
+              if (g + kTcGroups * u >= ntl) break;
+              long long tcp = cprof ? clock64() : 0ll;
+              const int want = tiles_seen[g] + 1;
+              for (;;) {
+                bool done = true;
+#pragma unroll
+                for (int w = 0; w < kTcGroupWarps; ++w) done = done && (wdone_s[g * kTcGroupWarps + w] >= want);
+                const int b = (seq >> g) & 1u, hb = 2 * g + b;
+                if (mbar_test_wait(&sfull[hb], (par >> hb) & 1u)) {
+                  // a half completed during a LATER tile of the group stays for that tile's round (the order of the
+                  // MMAs must not depend on how far ahead the group runs)
+                  if ((smeta_s[g][b] >> 8) >= want) break;
+                  take(g);
+                  continue;
+                }
+                if (done) break;
+              }
+              tiles_seen[g] = want;
+              if (cprof) prof_s[0] += (unsigned long long)(clock64() - tcp);
+            }
+          }
+          // the last message of every group: its partial half (or an empty message)
+#pragma unroll
+          for (int g = 0; g < kTcGroups; ++g) {
+            const int hb = 2 * g + ((seq >> g) & 1u);
+            mbar_wait(&sfull[hb], (par >> hb) & 1u);
+            take(g);
+          }
+          if (any_mma) umma_commit(acc_full);
+          else mbar_arrive(acc_full);
+          mbar_wait(go, go_phase);
+          go_phase ^= 1u;
+          if (!ctrl_cmd_s) break;
+          tc_fence_after();
+        }
+      }
+      __syncwarp();
+      __syncthreads();                               // the final barrier of the workers
+      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTcCols) : "memory");
+      return;
+    }
+    if (warp == kNW + 1) {
+      if (lane < NS && ntl > 0 && !((p.dbg & 4) && lane > 0 && false)) {
+        const int Kc = p.st->K + ((p.add_candidate && p.st->cand_valid) ? 1 : 0);
+        const uint32_t bytes = (uint32_t)(Kc + kTcMetaRows) * (uint32_t)TP * 4u;
+        long long c = lane, last_issued = -1;
+        int j = lane, pi = 0;                        // tile j of pass pi
+        while (j >= ntl) { j -= ntl; ++pi; }
+        for (;;) {
+          bool ok = c < NS, stop = false;
+          while (!ok) {
+            if (stop_s) { stop = true; break; }
+            ok = mbar_test_wait(&empty[lane], (uint32_t)(((c / NS) - 1) & 1));
+          }
+          if (stop) break;
+          const int tile = tb0 + ((pi & 1) ? ntl - 1 - j : j) * tstep;
+          mbar_arrive_expect_tx(&full[lane], bytes);
+          bulk_g2s(ring + (size_t)lane * p.stage_bytes, p.A + (size_t)tile * (size_t)p.tile_stride, bytes, &full[lane]);
+          __threadfence_block();
+          gen_s[lane] = (int)(c / NS) + 1;
+          last_issued = c;
+          c += NS;
+          j += NS;
+          while (j >= ntl) { j -= ntl; ++pi; }
+        }
+        // drain: a copy issued for a tile that is never consumed must land before the CTA may exit
+        if (last_issued >= total_tiles_s) mbar_wait(&full[lane], (uint32_t)((last_issued / NS) & 1));
+      }
+      __syncwarp();
+      __syncthreads();
+      return;
+    }
+  }
 
   // =============================== worker warps =================================================
   const int nb = (K + 1 + 7) >> 3;                 // 8x8 block rows of the augmented matrix (K columns + gradient)
@@ -237,7 +478,7 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
   int NC = 1;
   while (NC < kNwtBack && ((nstrips + NC - 1) / NC > kNwtStrips || kNwtBack % NC != 0)) ++NC;
   const int NG = kNwtBack / NC;
-  const bool is_front = warp < kNwtFront;
+  const bool is_front = TC || warp < kNwtFront;
   const int bw = is_front ? 0 : warp - kNwtFront;
   const int cls = bw % NC, grp = bw / NC;
   int nstr = 0;
@@ -587,6 +828,308 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
     PROF_MARK(2);
   };
 
+  // ---- the same pass with the Hessian on the 5th-generation tensor cores (master_method = 3) ----
+  // No CTA-wide step inside the pass: a tile of 128 voxels belongs to a GROUP of four warps (lane = voxel), the 4
+  // groups walk the CTA's tiles independently and meet only on mbarriers.  Per tile and warp:
+  //  Z  z_j = sum_k y_k A[k][j]  (fp64, 4 chains);  P  F, pi_j, s_j = 2 c_j, ballot of the active voxels; the four
+  //     counts of the group are exchanged through shared memory (one named barrier per tile and group);
+  //  W  the group APPENDS its active voxels, in voxel order, to its operand slab: two halves of 16 voxels, rows
+  //     [Wh (64); Wl (64)], Wh + Wl = fp32(sqrt(s) A[k][j]) split into two TF32 values (K-major core matrices); lane
+  //     (q, r) converts rows r, r + 8, ... of the warp's active voxels q and q + 4 of a chunk of 8 and adds
+  //     pi_j A[k][j] to its fp64 gradient accumulators.  A complete half is handed to the control warp (every warp
+  //     of the group arrives once per half, after its own writes), which issues [hh; lh] += [Wh; Wl] Wh^T into TMEM.
+  // After the last tile the partial half is padded with zeros and sent as the group's last message of the pass; then
+  // H = hh + lh + lh^T (the lo x lo term, 2^-22 relative, is dropped), gradient, F -> hred, grid reduction.
+  uint32_t acc_phase = 0u;
+  long long cbase = 0;                                   // tiles of the earlier passes (position in the A stream)
+  unsigned half_base = 0u;                               // halves this group has sent in the earlier passes
+  int tiles_done = 0;                                    // tiles this warp has finished
+  auto pass_tc = [&](const double *yv) {
+    double f_acc = 0.0;
+    const bool rev = (pass_no++ & 1u) != 0u;
+    double gacc[kNwtAcc];
+#pragma unroll
+    for (int i = 0; i < kNwtAcc; ++i) gacc[i] = 0.0;
+    if (tid < K) ycur_s[tid] = yv[tid];
+    if (tid == 0) si[10] = 0;
+    wsync();
+    const int grp = warp / kTcGroupWarps, wg = warp % kTcGroupWarps;
+    unsigned fill = 0u;                                  // active voxels the group has appended in this pass
+    {
+      // what the +0 -> 2^-127 of cvt_pos adds to a dose, accumulated exactly like the dose itself
+      double zc;
+      {
+        double c[4] = {0.0, 0.0, 0.0, 0.0};
+        int k = 0;
+        for (; k + 3 < K; k += 4) {
+#pragma unroll
+          for (int u = 0; u < 4; ++u) c[u] = fma(ycur_s[k + u], kTiny, c[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < 3; ++u)
+          if (k + u < K) c[u] = fma(ycur_s[k + u], kTiny, c[u]);
+        zc = (c[0] + c[1]) + (c[2] + c[3]);
+      }
+      const int v = wg * 32 + lane;                      // voxel of the tile
+      const int q4 = lane & 3, rp = lane >> 2;           // W: active voxels q4 and q4 + 4 of a chunk, rows rp + 8 i
+      const uint32_t slab = smem_addr(slabs) + (uint32_t)grp * 2u * kTcHalfBytes + (uint32_t)rp * 16u;
+      unsigned char *my_cl = cl_s + warp * 32;
+      double *my_cpi = cpi_s + warp * 32;
+      float *my_csq = csq_s + warp * 32;
+      // half h (running index of the group) may be written once the message that last used its buffer is consumed
+      unsigned verified = half_base;                     // halves below this index are known to be free for writing
+      unsigned arrived = half_base;                      // halves below this index: this warp has arrived on sfull
+      // this warp is done with every half below `upto` that the group has completed: hand them over
+      auto verify_upto = [&](unsigned upto) {
+        while (verified < upto) {
+          if (verified >= 2u) mbar_wait(&sempty[2 * grp + (verified & 1u)], ((verified >> 1) - 1u) & 1u);
+          ++verified;
+        }
+      };
+      auto arrive_upto = [&](unsigned upto) {
+        while (arrived < upto) {
+          verify_upto(arrived + 1u);                     // the previous phase of this half's barrier must be complete
+          fence_async_smem();
+          __syncwarp();
+          if (lane == 0) {
+            if (wg == 0) smeta_s[grp][arrived & 1u] = 1 | (tiles_done << 8);
+            mbar_arrive(&sfull[2 * grp + (arrived & 1u)]);
+          }
+          ++arrived;
+        }
+      };
+      int tix = 0;
+      for (int j = grp; j < ntl; j += kTcGroups, ++tix) {
+        const long long c = cbase + j;
+        const int stg = (int)(c % NS);
+        const uint32_t par = (uint32_t)((c / NS) & 1);
+        const int tile = tb0 + (rev ? ntl - 1 - j : j) * tstep;
+        long long tc = prof ? clock64() : 0ll;
+#define CYC_MARK(slot)                                    \
+  do {                                                    \
+    if (prof) {                                           \
+      const long long now_ = clock64();                   \
+      prof_s[slot] += (unsigned long long)(now_ - tc);    \
+      tc = now_;                                          \
+    }                                                     \
+  } while (0)
+        while (gen_s[stg] <= (int)(c / NS)) {}            // the copy of THIS use of the stage has been issued
+        mbar_wait(&full[stg], par);
+        CYC_MARK(12);
+        const unsigned char *stage = ring + (size_t)stg * p.stage_bytes;
+        const float *M = reinterpret_cast<const float *>(stage) + kTcMetaRows * TP;   // column 0 of the tile
+        // ---- Z ----
+        double z0;
+        {
+          double a4[4] = {0.0, 0.0, 0.0, 0.0};
+          const float *pa = M + v;
+          float f[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) f[u] = pa[(size_t)min(u, K - 1) * TP];
+          int k = 0;
+          for (; k + 7 < K; k += 4) {                    // the next group exists in full
+            float n[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) n[u] = pa[(size_t)(k + 4 + u) * TP];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) a4[u] = fma(ycur_s[k + u], cvt_pos(f[u]), a4[u]);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) f[u] = n[u];
+          }
+          if (k + 3 < K) {                               // one more full group; its successor is partial
+            float n[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) n[u] = pa[(size_t)min(k + 4 + u, K - 1) * TP];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) a4[u] = fma(ycur_s[k + u], cvt_pos(f[u]), a4[u]);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) f[u] = n[u];
+            k += 4;
+          }
+#pragma unroll
+          for (int u = 0; u < 3; ++u)
+            if (k + u < K) a4[u] = fma(ycur_s[k + u], cvt_pos(f[u]), a4[u]);
+          z0 = ((a4[0] + a4[1]) + (a4[2] + a4[3])) - zc;
+        }
+        CYC_MARK(13);
+        // ---- P ----
+        bool act0 = false;
+        float sq0 = 0.f;
+        double gv0 = 0.0;                                 // sqrt(s_j) (fp32), pi_j
+        {
+          const int sid0 = stage[v];
+          if (sid0 != kNoStruct) {
+            StructEntry e = stab[sid0];
+            if (p.vt) e.tm = e.tp = (double)reinterpret_cast<const float *>(stage)[TP + v];
+            const double un = fmax(e.tm - z0, 0.0), ov = fmax(z0 - e.tp, 0.0);
+            f_acc += e.a * un * un + e.b * ov * ov;
+            const double sv = 2.0 * ((un > 0.0 ? e.a : 0.0) + (ov > 0.0 ? e.b : 0.0));
+            if (sv != 0.0) {
+              act0 = true;
+              gv0 = -2.0 * e.a * un + 2.0 * e.b * ov;
+              sq0 = sqrtf((float)sv);
+            }
+          }
+          p.mz[(size_t)tile * T + v] = z0;
+        }
+        const unsigned m0 = __ballot_sync(0xffffffffu, act0);
+        const int n_w = __popc(m0);
+        if (act0) {
+          const int i = __popc(m0 & ((1u << lane) - 1u));
+          my_cl[i] = (unsigned char)v; my_cpi[i] = gv0; my_csq[i] = sq0;
+        }
+        if (lane == 0) gcnt_s[grp][tix & 1][wg] = n_w;
+        asm volatile("bar.sync %0, %1;" ::"r"(3 + grp), "n"(kTcGroupWarps * 32) : "memory");
+        unsigned off_w = 0u, n_t = 0u;
+#pragma unroll
+        for (int w = 0; w < kTcGroupWarps; ++w) {
+          const unsigned cn = (unsigned)gcnt_s[grp][tix & 1][w];
+          if (w < wg) off_w += cn;
+          n_t += cn;
+        }
+        if (prof) prof_s[11] += (unsigned long long)n_t;
+        CYC_MARK(14);
+        // ---- W: this warp's active voxels go to the positions fill + off_w ... of the group's stream ----
+        const unsigned pos_w = fill + off_w;
+        const unsigned done_after = half_base + (fill + n_t) / kTcHV;     // halves complete once this tile is in
+        for (int c0 = 0; c0 < n_w; c0 += 8) {
+          const unsigned h_first = half_base + (pos_w + c0) / kTcHV;
+          const unsigned h_last = half_base + (pos_w + min(c0 + 7, n_w - 1)) / kTcHV;
+          arrive_upto(min(h_first, done_after));
+          verify_upto(h_last + 1u);
+          CYC_MARK(5);
+          const int a0 = c0 + q4, a1 = a0 + 4;
+          const bool l0 = a0 < n_w, l1 = a1 < n_w;
+          const float s0 = l0 ? my_csq[a0] : 0.f, s1 = l1 ? my_csq[a1] : 0.f;
+          const double p0 = l0 ? my_cpi[a0] : 0.0, p1 = l1 ? my_cpi[a1] : 0.0;
+          const float *src0 = M + (l0 ? (int)my_cl[a0] : 0), *src1 = M + (l1 ? (int)my_cl[a1] : 0);
+          const unsigned ps0 = pos_w + a0, ps1 = pos_w + a1;             // position in the group's stream
+          const uint32_t o0 = slab + (((half_base + ps0 / kTcHV) & 1u) ? kTcHalfBytes : 0u) + ((ps0 % kTcHV) >> 2) * kTcLbo + (ps0 & 3u) * 4u;
+          const uint32_t o1 = slab + (((half_base + ps1 / kTcHV) & 1u) ? kTcHalfBytes : 0u) + ((ps1 % kTcHV) >> 2) * kTcLbo + (ps1 & 3u) * 4u;
+          float f0[kNwtAcc], f1[kNwtAcc];
+#pragma unroll
+          for (int i = 0; i < kNwtAcc; ++i) {
+            const size_t ro = (size_t)min(rp + 8 * i, K - 1) * TP;
+            f0[i] = src0[ro];
+            f1[i] = src1[ro];
+          }
+#pragma unroll
+          for (int i = 0; i < kNwtAcc; ++i) {
+            if (rp + 8 * i < K) {
+              const float w0 = s0 * f0[i], w1 = s1 * f1[i];
+              const float h0 = tf32_rna(w0), h1 = tf32_rna(w1);
+              if (l0 && !(p.dbg & 2)) {
+                sts_f32(o0 + (uint32_t)i * kTcSbo, h0);
+                sts_f32(o0 + (uint32_t)(i + 8) * kTcSbo, tf32_rna(w0 - h0));
+              }
+              if (l1 && !(p.dbg & 2)) {
+                sts_f32(o1 + (uint32_t)i * kTcSbo, h1);
+                sts_f32(o1 + (uint32_t)(i + 8) * kTcSbo, tf32_rna(w1 - h1));
+              }
+              gacc[i] = fma(p0, cvt_pos(f0[i]), gacc[i]);
+              gacc[i] = fma(p1, cvt_pos(f1[i]), gacc[i]);
+            }
+          }
+          CYC_MARK(6);
+        }
+        if ((p.dbg & 64) && blockIdx.x == 0 && lane == 0) printf("w %d tile j %d tix %d n_w %d off %u n_t %u fill %u hb %u done_after %u arrived %u verified %u\n", warp, j, tix, n_w, off_w, n_t, fill, half_base, done_after, arrived, verified);
+        fill += n_t;
+        arrive_upto(done_after);                         // every half this tile completed (also those without a voxel of this warp)
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(&empty[stg]);
+          __threadfence_block();
+          wdone_s[warp] = ++tiles_done;                  // after the arrivals above: the control warp counts on that order
+        }
+      }
+      // ---- last message of the pass: the partial half, its unused voxels zeroed (warp 0 of the group) ----
+      {
+        const unsigned h = half_base + fill / kTcHV, used = fill % kTcHV;
+        if ((p.dbg & 64) && blockIdx.x == 0 && lane == 0) printf("w %d flush h %u used %u arrived %u verified %u\n", warp, h, used, arrived, verified);
+        verify_upto(h + 1u);
+        if (wg == 0 && used > 0u) {
+          for (unsigned cc = used + (unsigned)q4; cc < (unsigned)kTcHV; cc += 4u) {
+            const uint32_t o = slab + ((h & 1u) ? kTcHalfBytes : 0u) + (cc >> 2) * kTcLbo + (cc & 3u) * 4u;
+#pragma unroll
+            for (int i = 0; i < kNwtAcc; ++i) {
+              if (rp + 8 * i < K) {
+                sts_f32(o + (uint32_t)i * kTcSbo, 0.f);
+                sts_f32(o + (uint32_t)(i + 8) * kTcSbo, 0.f);
+              }
+            }
+          }
+        }
+        fence_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+          if (wg == 0) smeta_s[grp][h & 1u] = (used > 0u ? 1 : 0) | 2 | (tiles_done << 8);
+          mbar_arrive(&sfull[2 * grp + (h & 1u)]);
+        }
+        half_base = h + 1u;
+        if (fill > 0u) si[10] = 1;                       // this CTA issued at least one MMA: the accumulators are live
+      }
+#undef CYC_MARK
+    }
+    cbase += ntl;
+    // the slab area is recycled below (lh, gradient partials, hred): every warp must be past its last write
+    wsync();
+    PROF_MARK(1);
+    mbar_wait(acc_full, acc_phase);
+    acc_phase ^= 1u;
+    tc_fence_after();
+    // ---- gradient: lanes (q, r) -> r; rows r + 8 i.  Per-warp partials, added in warp order below ----
+#pragma unroll
+    for (int i = 0; i < kNwtAcc; ++i) {
+      double g = gacc[i];
+      g += __shfl_xor_sync(0xffffffffu, g, 1);
+      g += __shfl_xor_sync(0xffffffffu, g, 2);
+      if ((lane & 3) == 0) gpart[warp * 64 + (lane >> 2) + 8 * i] = g;
+    }
+    {
+      const double fs = warp_sum_f64(f_acc);
+      if (lane == 0) fred_s[warp] = fs;
+    }
+    // ---- accumulators: TMEM lanes 0..63 hold hh, lanes 64..127 lh (columns 0..63); lh goes through shared memory ----
+    const int lq = warp & 3, cs0 = (warp >> 2) * 16;   // lane quarter, first of the 16 columns of this warp
+    const int row = 32 * (lq & 1) + lane;
+    const bool any_h = si[10] != 0 && !(p.dbg & 8);
+    if (any_h && lq >= 2) {
+      float vv[16];
+      tmem_ld16(tmem_base + ((uint32_t)(32 * lq) << 16) + (uint32_t)cs0, vv);
+#pragma unroll
+      for (int jj = 0; jj < 16; ++jj) lh_s[row * 65 + cs0 + jj] = vv[jj];
+    }
+    wsync();
+    if (lq < 2 && row - lane < 8 * nb) {               // warp-uniform: tcgen05.ld is a warp-wide instruction
+      float vv[16];
+      if (any_h) tmem_ld16(tmem_base + ((uint32_t)(32 * lq) << 16) + (uint32_t)cs0, vv);
+#pragma unroll
+      for (int jj = 0; jj < 16; ++jj) {
+        const int col = cs0 + jj;
+        if (row < 8 * nb && col < 8 * nb && (row >> 3) <= (col >> 3)) {
+          double h = 0.0;
+          if (row < K && col < K) {
+            if (any_h) h = ((double)vv[jj] + (double)lh_s[row * 65 + col]) + (double)lh_s[col * 65 + row];
+          } else if (col == K && row < K) {            // gradient column of the augmented matrix
+            double g = 0.0;
+            for (int w = 0; w < kNW; ++w) g += gpart[w * 64 + row];
+            h = g;
+          }
+          hred[(size_t)blk_index(nb, row >> 3, col >> 3) * 64 + (row & 7) * 8 + (col & 7)] = h;
+        }
+      }
+    }
+    tc_fence_before();
+    if (tid == 0) {
+      double s = 0.0;
+      for (int w = 0; w < kNW; ++w) s += fred_s[w];
+      hred[nblocks * 64] = s;
+    }
+    wsync();
+    red.ranges(n_red, hred, hred, lbuf);
+    PROF_MARK(2);
+  };
+
   // ---- the first pass evaluates everything at the warm start (previous optimum, new column at 0), every later
   //      one at a trial point.  pass() has ONE call site: inlined several times the kernel outgrew the instruction
   //      cache and everything that runs once per iteration ran from L2 (5x slower, measured). ----
@@ -596,9 +1139,15 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
   const double *cur = y_s;
 
   for (;;) {
-    pass(cur);
+    if constexpr (TC) {
+      if (passes > 0 && tid == 0) { ctrl_cmd_s = 1; mbar_arrive(go); }   // the control warp starts the next pass
+      pass_tc(cur);
+    } else {
+      pass(cur);
+    }
     ++passes;
     if (passes == 1) F = hred[nblocks * 64];
+    if ((p.dbg & 128) && blockIdx.x == 0 && tid == 0) printf("pass %d K %d H00 %.10e g0 %.10e F %.10e\n", passes, K, hred[0], h_at(hred, nb, 0, K), hred[nblocks * 64]);
     if (restoring) have_dir = false;
     // ================= decision on the pass just made (warp 0; identical in every CTA) =================
     if (warp == 0) {
@@ -895,12 +1444,22 @@ __global__ void __launch_bounds__(kMasterWorkers, 1) k_master_newton(NewtonParam
 
   // ---- publish ----
   // drain: every issued stage must have landed before the CTA may exit
-  if (is_issuer) si[9] = issued_total;
-  wsync();
-  if (tid == 0) {
-    for (const int n_issued = si[9]; consumed_total < n_issued; ++consumed_total) {
-      mbar_wait(&full[cp.stage], cp.phase);
-      cp.advance(NS);
+  if constexpr (TC) {
+    if (tid == 0) {                                          // the feeder drains the ring, the control warp frees the TMEM
+      total_tiles_s = cbase;
+      __threadfence_block();
+      stop_s = 1;
+      ctrl_cmd_s = 0;
+      mbar_arrive(go);
+    }
+  } else {
+    if (is_issuer) si[9] = issued_total;
+    wsync();
+    if (tid == 0) {
+      for (const int n_issued = si[9]; consumed_total < n_issued; ++consumed_total) {
+        mbar_wait(&full[cp.stage], cp.phase);
+        cp.advance(NS);
+      }
     }
   }
   // beamlet intensities of the new plan (every CTA a slice; same arithmetic as k_intensity: fp64 sum in pool order)
@@ -964,12 +1523,34 @@ static size_t newton_fixed_smem(int32_t k_max, int32_t T, int32_t n_struct, int3
          align_up((size_t)(T + 8) * 2, 128);
 }
 
-NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct) {
+NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct, bool tc) {
   NewtonLayout L;
   L.nb_max = (k_max + 1 + 7) / 8;
   L.n_red = L.nb_max * (L.nb_max + 1) / 2 * 64 + 8;
   // 227 KB opt-in maximum per CTA on sm_100; ~9 KB of static tables, 1 KB reserved by the system
-  const size_t budget = (size_t)227 * 1024 - (size_t)10 * 1024;
+  const size_t budget = (size_t)227 * 1024 - (size_t)11 * 1024;
+  if (tc && k_max <= kTcMaxK) {
+    // master_method = 3: tiles of 128 voxels (a group of four warps each); a stage = the two meta rows (structure
+    // ids, per-voxel thresholds) + the k_max columns of a tile; as many stages as fit beside the operand slabs (whose
+    // 64 KB also hold hred, the factorisation buffer, lh and the gradient partials between the passes)
+    L.tc = 1;
+    L.kp = 64; L.lbo = (int32_t)kTcLbo; L.sbo = (int32_t)kTcSbo; L.w_bytes = (int32_t)kTcHalfBytes; L.tmem_cols = (int32_t)kTcCols;
+    L.meta_rows = kTcMetaRows;
+    L.T = kTcT; L.TP = kTcT + 4; L.AC = 64;
+    L.lbuf_doubles = std::max((k_max + 1) * (k_max + 2) / 2 + 8, kNW * 32);
+    L.stage_bytes = (int32_t)align_up((size_t)(k_max + kTcMetaRows) * L.TP * 4, 128);
+    const size_t recycled = align_up((size_t)L.n_red * 8, 128) + align_up((size_t)L.lbuf_doubles * 8, 128) +
+                            align_up((size_t)64 * 65 * 4, 128) + (size_t)kNW * 64 * 8;
+    const size_t fixed = 5 * 128 + (size_t)kNW * 32 * 13 + align_up((size_t)std::max(n_struct, 1) * sizeof(StructEntry), 128) +
+                         std::max(recycled, (size_t)kTcGroups * 2 * kTcHalfBytes);
+    int32_t stages = 2;
+    while (stages < kTcMaxStages && fixed + (size_t)(stages + 1) * L.stage_bytes <= budget) ++stages;
+    L.n_stages = stages;
+    L.smem = fixed + (size_t)stages * L.stage_bytes;
+    L.n_tiles = (n_vox_pad + L.T - 1) / L.T;
+    L.tile_stride = (int64_t)(k_max + kTcMetaRows) * L.TP;
+    return L;
+  }
   static const int32_t cand_t[] = {256, 128, 64, 32};        // T x k-slices = 256 front threads
   static const int32_t cand_ac[] = {64, 32, 16};
   for (int32_t T : cand_t) {
@@ -994,13 +1575,35 @@ NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct) {
   return L;
 }
 
+// master_method = 3: the structure id and the threshold of every voxel of a tile, in the tile's two meta rows
+__global__ void k_newton_tile_meta(float *A, int32_t n_tiles, int32_t T, int32_t TP, int64_t tile_stride, const uint8_t *sid,
+                                   const float *vt, int32_t n_vox_pad) {
+  const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x);
+  if (i >= n_tiles * T) return;
+  const int t = i / T, v = i - t * T;
+  float *tile = A + (size_t)t * (size_t)tile_stride;
+  reinterpret_cast<uint8_t *>(tile)[v] = (i < n_vox_pad) ? sid[i] : (uint8_t)kNoStruct;
+  tile[TP + v] = (vt != nullptr && i < n_vox_pad) ? vt[i] : 0.f;
+}
+
+cudaError_t newton_fill_tile_meta(Ctx *c) {
+  const NewtonLayout &L = c->nwt;
+  if (!L.tc) return cudaSuccess;
+  const int n = L.n_tiles * L.T;
+  k_newton_tile_meta<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d.A, L.n_tiles, L.T, L.TP, L.tile_stride, c->d.sid,
+                                                           c->has_vt ? c->d.vt : nullptr, c->n_vox_pad);
+  return cudaGetLastError();
+}
+
 cudaError_t newton_configure(Ctx *c) {
   c->master_grid = std::min(c->n_sm, kMasterMaxGrid);
+  { const char *e = getenv("DAO_GRID"); if (e) c->master_grid = atoi(e); }
   const NewtonLayout &L = c->nwt;
-  cudaError_t e = cudaFuncSetAttribute(k_master_newton, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem);
+  const void *fn = L.tc ? (const void *)k_master_newton<true> : (const void *)k_master_newton<false>;
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem);
   if (e != cudaSuccess) return e;
   int nbk = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nbk, k_master_newton, kMasterWorkers, L.smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nbk, fn, L.tc ? kNwtTcThreads : kMasterWorkers, L.smem);
   if (e != cudaSuccess) return e;
   if (nbk < 1) return cudaErrorLaunchOutOfResources;
   return cudaSuccess;
@@ -1018,7 +1621,8 @@ cudaError_t launch_newton(Ctx *c, bool add_candidate) {
   p.AC = L.AC;
   p.w_doubles = (8 * L.nb_max + 1) * (L.AC + 4);
   p.ks_shift = 0;
-  while ((L.T << p.ks_shift) < kNwtFrontThreads) ++p.ks_shift;
+  while ((L.T << p.ks_shift) < (L.tc ? kMasterWorkers : kNwtFrontThreads)) ++p.ks_shift;
+
   p.n_struct = std::max(c->n_struct, 1);
   p.sid = c->d.sid;
   p.vt = c->has_vt ? c->d.vt : nullptr;
@@ -1040,10 +1644,16 @@ cudaError_t launch_newton(Ctx *c, bool add_candidate) {
   p.max_iter = c->opt.master_max_iter;
   p.k_max = c->opt.k_max;
   p.tol = c->opt.master_tol;
+  { const char *e = getenv("DAO_DEBUG"); p.dbg = e ? atoi(e) : 0; }
   void *args[] = {&p};
   ++c->n_launches;
-  return cudaLaunchCooperativeKernel((void *)k_master_newton, dim3(c->master_grid), dim3(kMasterWorkers), args, L.smem,
-                                     c->stream);
+  if (p.dbg & 16) return cudaStreamSynchronize(c->stream);
+  if (p.dbg & 32) { cudaError_t e0 = cudaStreamSynchronize(c->stream); if (e0 != cudaSuccess) { fprintf(stderr, "before newton: %s\n", cudaGetErrorString(e0)); return e0; } }
+  if (L.tc)
+    return cudaLaunchCooperativeKernel((void *)k_master_newton<true>, dim3(c->master_grid), dim3(kNwtTcThreads), args,
+                                       L.smem, c->stream);
+  return cudaLaunchCooperativeKernel((void *)k_master_newton<false>, dim3(c->master_grid), dim3(kMasterWorkers), args,
+                                     L.smem, c->stream);
 }
 
 }  // namespace dao

@@ -100,7 +100,7 @@ struct Dims {
 
 // layout of the dose block and of the grid-reduction slots, decided by the master method alone
 static NewtonLayout layout_of_master(const Dims &dm, int32_t n_vox_pad) {
-  if (dm.master_method == 2) return newton_layout(dm.k_max, n_vox_pad, dm.n_struct);
+  if (dm.master_method >= 2) return newton_layout(dm.k_max, n_vox_pad, dm.n_struct, dm.master_method == 3);
   return NewtonLayout{};
 }
 
@@ -229,7 +229,7 @@ static dao_status check_args(const dao_csr *D, const dao_mlc *mlc, const dao_str
   if (opt->k_max < 1) { *err = "k_max must be >= 1"; return DAO_E_ARG; }
   if (opt->k_max > DAO_MAX_APERTURES) { *err = "k_max > DAO_MAX_APERTURES"; return DAO_E_UNSUPPORTED; }
   if (opt->master_max_iter < 0 || !(opt->master_tol >= 0.0) || !(opt->price_tol >= 0.0) ||
-      (opt->master_method < 0 || opt->master_method > 2) || opt->sell_sigma < 0 ||
+      (opt->master_method < 0 || opt->master_method > 3) || opt->sell_sigma < 0 ||
       !(opt->master_ls_tol > 0.0) || !(opt->master_ls_tol < 1.0) ||
       (opt->mlc_mode < DAO_MLC_CONSECUTIVE || opt->mlc_mode > DAO_MLC_CONNECTED)) {
     *err = "bad option value"; return DAO_E_ARG;
@@ -256,7 +256,7 @@ static dao_status check_args(const dao_csr *D, const dao_mlc *mlc, const dao_str
   dm->n_beams = mlc->n_beams; dm->n_rows = mlc->n_rows; dm->k_max = opt->k_max;
   dm->max_rows = std::max(max_rows, 1);
   // the projected-Newton master handles pools up to kNewtonMaxK apertures; larger pools use method 1
-  dm->master_method = (opt->master_method == 2 && opt->k_max > kNewtonMaxK) ? 1 : opt->master_method;
+  dm->master_method = (opt->master_method >= 2 && opt->k_max > kNewtonMaxK) ? 1 : opt->master_method;
   dm->n_struct = s->n_struct;
   dm->chain_states = 0;
   if (opt->mlc_mode == DAO_MLC_INTERDIGITATION || opt->mlc_mode == DAO_MLC_CONNECTED) {
@@ -773,6 +773,7 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   }
   // the tiled dose block is read with its padding (tile tails, the 4 pad floats of every column): finite zeros
   if (c->nwt.T) SETUP_CUDA(cudaMemsetAsync(d.A, 0, (size_t)c->nwt.n_tiles * (size_t)c->nwt.tile_stride * 4, q));
+  SETUP_CUDA(newton_fill_tile_meta(c));
   SETUP_CUDA(cudaMemsetAsync(d.m_epoch, 0, 64 * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.m_prof, 0, kMasterProfSlots * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.ap_beam, 0, (size_t)dm.k_max * 4, q));

@@ -348,7 +348,7 @@ static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out, const in
   p.st = c->d.state;
   p.skip = skip;
   p.a_T = c->nwt.T; p.a_TP = c->nwt.TP; p.a_stride = c->nwt.tile_stride; p.a_col = a_col;
-  if (MODE == kSpmvColumn) p.out = c->d.A;
+  if (MODE == kSpmvColumn) p.out = c->d.A + (size_t)c->nwt.meta_rows * (size_t)c->nwt.TP;   // column 0 of tile 0
   p.bl_row = c->d.bl_row; p.row_beam = c->d.row_beam; p.row_bl_ptr = c->d.row_bl_ptr; p.left = c->d.left; p.right = c->d.right;
   p.mask_from_candidate = (MODE == kSpmvColumn && a_col < 0 && spmv_builds_mask(c)) ? 1 : 0;
   ++c->n_launches;
