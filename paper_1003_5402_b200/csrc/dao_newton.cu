@@ -34,7 +34,6 @@
 
 #include <algorithm>
 #include <cstdlib>
-#include <cstdio>
 
 namespace dao {
 
@@ -58,7 +57,7 @@ constexpr int kTcGroupWarps = kTcT / 32;
 constexpr int kTcGroups = kNW / kTcGroupWarps;
 constexpr int kTcHV = 16;                // voxels per half = two MMA k-steps
 constexpr uint32_t kTcLbo = 128, kTcSbo = (kTcHV / 4) * kTcLbo, kTcHalfBytes = 16 * kTcSbo;
-constexpr uint32_t kTcCols = 64;         // TMEM columns: one 128 x 64 fp32 accumulator
+constexpr uint32_t kTcCols = 64 * kTcGroups;   // TMEM columns: one 128 x 64 fp32 accumulator per group
 constexpr int kTcMaxK = 56;              // 8 block rows of the augmented Hessian fit the 64 rows of one operand half
 constexpr int kTcMaxStages = 12;
 constexpr int kTcMetaRows = 2;
@@ -98,7 +97,6 @@ struct NewtonParams {
   int32_t max_iter;
   int32_t k_max;
   double tol;
-  int32_t dbg;
 };
 
 // barrier over the front warps
@@ -203,7 +201,7 @@ __device__ __forceinline__ int lidx(int i, int j) { return (i * (i + 1)) / 2 + j
 // thread) feeds the A ring and issues tcgen05.mma (accumulators in TMEM for the whole pass); the gradient A^T pi is
 // accumulated in fp64 by the threads that write the tile.  Only H (which steers the Newton direction and never enters
 // the stopping test) is computed in reduced precision: ~2^-21 relative (3 x TF32), see DESIGN.md section 6.
-constexpr int kNwtTcThreads = kMasterWorkers + 64;   // + the control warp and the feeder warp
+constexpr int kNwtTcThreads = kMasterWorkers + 96;   // + two control warps and the feeder warp
 template <bool TC>
 __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_master_newton(NewtonParams p) {
   extern __shared__ __align__(128) unsigned char dyn_smem[];
@@ -228,7 +226,7 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
   __shared__ volatile int smeta_s[kTcGroups][2];   // TC: per half message: bit 0 = it holds voxels, bit 1 = last of the pass
   __shared__ volatile int gcnt_s[kTcGroups][2][kTcGroupWarps];   // TC: active voxels of a tile per warp (double buffered)
   __shared__ volatile int stop_s;                  // TC: the feeder warp stops issuing
-  __shared__ volatile int wdone_s[kNW];            // TC: tiles this warp has finished since the kernel started
+  __shared__ volatile int live_s[kTcGroups];       // TC: the group issued an MMA in this pass (its accumulator is live)
   __shared__ volatile int gen_s[16];               // TC: copies issued into ring stage s so far (a group may run several uses of
                                                    // a stage ahead of the feeder: a parity wait alone would alias)
   __shared__ volatile long long total_tiles_s;     // TC: tiles consumed when the solve ended
@@ -302,10 +300,10 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
     if constexpr (TC) {
       for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], kTcGroupWarps); }
       for (int h = 0; h < 2 * kTcGroups; ++h) { mbar_init(&sfull[h], kTcGroupWarps); mbar_init(&sempty[h], 1); }
-      mbar_init(acc_full, 1);
+      mbar_init(acc_full, 2);
       mbar_init(go, 1);
       stop_s = 0;
-      for (int w = 0; w < kNW; ++w) { wdone_s[w] = 0; gen_s[w] = 0; }
+      for (int w = 0; w < 16; ++w) gen_s[w] = 0;
     } else {
       for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NF); }
       for (int s = 0; s < 2; ++s) { mbar_init(&wfull[s], NF); mbar_init(&wempty[s], kNwtBack); }
@@ -325,81 +323,56 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
   const uint32_t tmem_base = TC ? tmem_base_s : 0u;
 
   // =============================== control and feeder warps (TC) ================================
-  // Warp 16, one thread: takes the operand halves of the groups in a FIXED order (message m of group 0, 1, 2, 3, then
-  // m + 1: independent of timing, so the accumulation order in TMEM is the same in every run) and issues the
-  // tcgen05.mma of each (two k-steps of 8 voxels); tcgen05.commit hands the half back to its group and, after the
-  // last message of a pass, publishes the accumulators (acc_full).  `go` / ctrl_cmd_s: does another pass follow?
-  // Warp 17: lane l owns ring stage l and streams the tiles l, l + NS, ... of the CTA's sequence (one bulk copy per
-  // tile: meta rows + the K live columns); it runs ahead into the next pass and is stopped by stop_s.
+  // Warps 16 and 17, one thread each: control warp c serves the groups 2c and 2c + 1.  It takes whichever of their
+  // operand halves is ready and issues its two tcgen05.mma (k-steps of 8 voxels) into the accumulator OF THAT GROUP
+  // (TMEM columns 64 g ...): the halves of a group arrive in the group's own fixed order and the four accumulators are
+  // added in a fixed order afterwards, so the result does not depend on timing.  tcgen05.commit hands the half back
+  // to its group; after the last message of both groups the accumulators are published (acc_full).  `go` /
+  // ctrl_cmd_s: does another pass follow?
+  // Warp 18, one thread: streams the tiles of the CTA's sequence into the ring (one bulk copy per tile: meta rows +
+  // the K live columns); it runs ahead into the next pass and is stopped by stop_s.
   if constexpr (TC) {
-    if (warp == kNW) {
+    if (warp == kNW || warp == kNW + 1) {
       if (lane == 0) {
+        const int cw = warp - kNW;
         // instruction descriptor: D = F32, A = B = TF32, both K-major, N = 64, M = 128
         const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((64u >> 3) << 17) | ((128u >> 4) << 24);
         const uint64_t desc0 = umma_desc(smem_addr(slabs), kTcLbo, kTcSbo);
-        const bool cprof = (p.prof != nullptr) && blockIdx.x == 0;
-        uint32_t par = 0u, go_phase = 0u;            // bit (2 g + b): parity of the next message on half b of group g
-        uint32_t seq = 0u;                           // bit g: which half group g sends next
-        int tiles_seen[kTcGroups];                   // tiles of group g whose halves have all been taken
-#pragma unroll
-        for (int g = 0; g < kTcGroups; ++g) tiles_seen[g] = 0;
-        bool any_mma = false;
-        // one half of group g: meta, the two MMAs, hand the half back; returns true for the last message of the pass
-        auto take = [&](int g) -> bool {
-          const int b = (seq >> g) & 1u, hb = 2 * g + b;
-          par ^= 1u << hb;
-          seq ^= 1u << g;
-          const int meta = smeta_s[g][b];
-          if ((p.dbg & 64) && blockIdx.x == 0) printf("ctl take g %d b %d meta 0x%x seen %d\n", g, b, meta, tiles_seen[g]);
-          if ((meta & 1) && !(p.dbg & 1)) {
-            tc_fence_after();
-            const uint64_t d = desc0 + (uint64_t)((uint32_t)hb * (kTcHalfBytes >> 4));
-            umma_tf32(tmem_base, d, d, idesc, any_mma ? 1u : 0u);
-            umma_tf32(tmem_base, d + (uint64_t)((2u * kTcLbo) >> 4), d + (uint64_t)((2u * kTcLbo) >> 4), idesc, 1u);
-            any_mma = true;
-            umma_commit(&sempty[hb]);
-          } else {
-            mbar_arrive(&sempty[hb]);
-          }
-          if (cprof) prof_s[7] += 1ull;
-          return (meta & 2) != 0;
-        };
+        const bool cprof = (p.prof != nullptr) && blockIdx.x == 0 && cw == 0;
+        uint32_t par = 0u, go_phase = 0u;            // bit (2 gi + b): parity of the next message on half b of group 2 cw + gi
+        uint32_t seq = 0u;                           // bit gi: which half the group sends next
         for (;;) {
-          any_mma = false;
-          // tile rounds: the halves group g completed while it handled its u-th tile of the pass, g = 0, 1, 2, 3 --
-          // the order in which the ring hands out the tiles, so nobody waits for a stage that waits for us
-          for (int u = 0; u * kTcGroups < ntl; ++u) {
+          uint32_t live = 3u, mma_any = 0u;          // groups that have not sent their last message; groups with an MMA
+          long long tcp = cprof ? clock64() : 0ll;
+          while (live) {
+            bool idle = true;
 #pragma unroll
-            for (int g = 0; g < kTcGroups; ++g) {
-              if (g + kTcGroups * u >= ntl) break;
-              long long tcp = cprof ? clock64() : 0ll;
-              const int want = tiles_seen[g] + 1;
-              for (;;) {
-                bool done = true;
-#pragma unroll
-                for (int w = 0; w < kTcGroupWarps; ++w) done = done && (wdone_s[g * kTcGroupWarps + w] >= want);
-                const int b = (seq >> g) & 1u, hb = 2 * g + b;
-                if (mbar_test_wait(&sfull[hb], (par >> hb) & 1u)) {
-                  // a half completed during a LATER tile of the group stays for that tile's round (the order of the
-                  // MMAs must not depend on how far ahead the group runs)
-                  if ((smeta_s[g][b] >> 8) >= want) break;
-                  take(g);
-                  continue;
-                }
-                if (done) break;
+            for (int gi = 0; gi < 2; ++gi) {
+              if (!((live >> gi) & 1u)) continue;
+              const int g = 2 * cw + gi, b = (seq >> gi) & 1u, hb = 2 * g + b, pb = 2 * gi + b;
+              if (!mbar_test_wait(&sfull[hb], (par >> pb) & 1u)) continue;
+              idle = false;
+              if (cprof) { const long long n_ = clock64(); prof_s[0] += (unsigned long long)(n_ - tcp); tcp = n_; }
+              par ^= 1u << pb;
+              seq ^= 1u << gi;
+              const int meta = smeta_s[g][b];
+              if (meta & 1) {
+                tc_fence_after();
+                const uint64_t d = desc0 + (uint64_t)((uint32_t)hb * (kTcHalfBytes >> 4));
+                const uint32_t acc = tmem_base + (uint32_t)g * 64u;
+                umma_tf32(acc, d, d, idesc, (mma_any >> gi) & 1u);
+                umma_tf32(acc, d + (uint64_t)((2u * kTcLbo) >> 4), d + (uint64_t)((2u * kTcLbo) >> 4), idesc, 1u);
+                mma_any |= 1u << gi;
+                umma_commit(&sempty[hb]);
+              } else {
+                mbar_arrive(&sempty[hb]);
               }
-              tiles_seen[g] = want;
-              if (cprof) prof_s[0] += (unsigned long long)(clock64() - tcp);
+              if (meta & 2) live &= ~(1u << gi);
+              if (cprof) { const long long n_ = clock64(); prof_s[15] += (unsigned long long)(n_ - tcp); prof_s[7] += 1ull; tcp = n_; }
             }
+            if (idle) __nanosleep(32);
           }
-          // the last message of every group: its partial half (or an empty message)
-#pragma unroll
-          for (int g = 0; g < kTcGroups; ++g) {
-            const int hb = 2 * g + ((seq >> g) & 1u);
-            mbar_wait(&sfull[hb], (par >> hb) & 1u);
-            take(g);
-          }
-          if (any_mma) umma_commit(acc_full);
+          if (mma_any) umma_commit(acc_full);
           else mbar_arrive(acc_full);
           mbar_wait(go, go_phase);
           go_phase ^= 1u;
@@ -409,35 +382,37 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
       }
       __syncwarp();
       __syncthreads();                               // the final barrier of the workers
-      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTcCols) : "memory");
+      if (warp == kNW)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTcCols) : "memory");
       return;
     }
-    if (warp == kNW + 1) {
-      if (lane < NS && ntl > 0 && !((p.dbg & 4) && lane > 0 && false)) {
+    if (warp == kNW + 2) {
+      if (lane == 0 && ntl > 0) {
         const int Kc = p.st->K + ((p.add_candidate && p.st->cand_valid) ? 1 : 0);
         const uint32_t bytes = (uint32_t)(Kc + kTcMetaRows) * (uint32_t)TP * 4u;
-        long long c = lane, last_issued = -1;
-        int j = lane, pi = 0;                        // tile j of pass pi
-        while (j >= ntl) { j -= ntl; ++pi; }
+        RingPos ipc{0, 0u};
+        long long c = 0;
+        int j = 0;
+        bool rv = false, stop = false;
         for (;;) {
-          bool ok = c < NS, stop = false;
-          while (!ok) {
-            if (stop_s) { stop = true; break; }
-            ok = mbar_test_wait(&empty[lane], (uint32_t)(((c / NS) - 1) & 1));
+          if (c >= NS) {
+            while (!mbar_test_wait(&empty[ipc.stage], ipc.phase ^ 1u)) {
+              if (stop_s) { stop = true; break; }
+              __nanosleep(64);
+            }
           }
           if (stop) break;
-          const int tile = tb0 + ((pi & 1) ? ntl - 1 - j : j) * tstep;
-          mbar_arrive_expect_tx(&full[lane], bytes);
-          bulk_g2s(ring + (size_t)lane * p.stage_bytes, p.A + (size_t)tile * (size_t)p.tile_stride, bytes, &full[lane]);
+          const int tile = tb0 + (rv ? ntl - 1 - j : j) * tstep;
+          mbar_arrive_expect_tx(&full[ipc.stage], bytes);
+          bulk_g2s(ring + (size_t)ipc.stage * p.stage_bytes, p.A + (size_t)tile * (size_t)p.tile_stride, bytes, &full[ipc.stage]);
           __threadfence_block();
-          gen_s[lane] = (int)(c / NS) + 1;
-          last_issued = c;
-          c += NS;
-          j += NS;
-          while (j >= ntl) { j -= ntl; ++pi; }
+          gen_s[ipc.stage] = (int)(c / NS) + 1;
+          ipc.advance(NS);
+          ++c;
+          if (++j == ntl) { j = 0; rv = !rv; }
         }
-        // drain: a copy issued for a tile that is never consumed must land before the CTA may exit
-        if (last_issued >= total_tiles_s) mbar_wait(&full[lane], (uint32_t)((last_issued / NS) & 1));
+        // drain: copies issued for tiles that are never consumed must land before the CTA may exit
+        for (long long cc = total_tiles_s; cc < c; ++cc) mbar_wait(&full[(int)(cc % NS)], (uint32_t)((cc / NS) & 1));
       }
       __syncwarp();
       __syncthreads();
@@ -843,15 +818,15 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
   uint32_t acc_phase = 0u;
   long long cbase = 0;                                   // tiles of the earlier passes (position in the A stream)
   unsigned half_base = 0u;                               // halves this group has sent in the earlier passes
-  int tiles_done = 0;                                    // tiles this warp has finished
   auto pass_tc = [&](const double *yv) {
     double f_acc = 0.0;
     const bool rev = (pass_no++ & 1u) != 0u;
     double gacc[kNwtAcc];
 #pragma unroll
     for (int i = 0; i < kNwtAcc; ++i) gacc[i] = 0.0;
+    const long long t_head = prof ? clock64() : 0ll;
     if (tid < K) ycur_s[tid] = yv[tid];
-    if (tid == 0) si[10] = 0;
+    if (tid < kTcGroups) live_s[tid] = 0;
     wsync();
     const int grp = warp / kTcGroupWarps, wg = warp % kTcGroupWarps;
     unsigned fill = 0u;                                  // active voxels the group has appended in this pass
@@ -892,12 +867,13 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
           fence_async_smem();
           __syncwarp();
           if (lane == 0) {
-            if (wg == 0) smeta_s[grp][arrived & 1u] = 1 | (tiles_done << 8);
+            if (wg == 0) smeta_s[grp][arrived & 1u] = 1;
             mbar_arrive(&sfull[2 * grp + (arrived & 1u)]);
           }
           ++arrived;
         }
       };
+      if (prof) prof_s[10] += (unsigned long long)(clock64() - t_head);   // EXPERIMENT: head of the pass
       int tix = 0;
       for (int j = grp; j < ntl; j += kTcGroups, ++tix) {
         const long long c = cbase + j;
@@ -913,7 +889,7 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
       tc = now_;                                          \
     }                                                     \
   } while (0)
-        while (gen_s[stg] <= (int)(c / NS)) {}            // the copy of THIS use of the stage has been issued
+        while (gen_s[stg] <= (int)(c / NS)) __nanosleep(32);   // the copy of THIS use of the stage has been issued
         mbar_wait(&full[stg], par);
         CYC_MARK(12);
         const unsigned char *stage = ring + (size_t)stg * p.stage_bytes;
@@ -1018,11 +994,11 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
             if (rp + 8 * i < K) {
               const float w0 = s0 * f0[i], w1 = s1 * f1[i];
               const float h0 = tf32_rna(w0), h1 = tf32_rna(w1);
-              if (l0 && !(p.dbg & 2)) {
+              if (l0) {
                 sts_f32(o0 + (uint32_t)i * kTcSbo, h0);
                 sts_f32(o0 + (uint32_t)(i + 8) * kTcSbo, tf32_rna(w0 - h0));
               }
-              if (l1 && !(p.dbg & 2)) {
+              if (l1) {
                 sts_f32(o1 + (uint32_t)i * kTcSbo, h1);
                 sts_f32(o1 + (uint32_t)(i + 8) * kTcSbo, tf32_rna(w1 - h1));
               }
@@ -1032,20 +1008,14 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
           }
           CYC_MARK(6);
         }
-        if ((p.dbg & 64) && blockIdx.x == 0 && lane == 0) printf("w %d tile j %d tix %d n_w %d off %u n_t %u fill %u hb %u done_after %u arrived %u verified %u\n", warp, j, tix, n_w, off_w, n_t, fill, half_base, done_after, arrived, verified);
         fill += n_t;
         arrive_upto(done_after);                         // every half this tile completed (also those without a voxel of this warp)
         __syncwarp();
-        if (lane == 0) {
-          mbar_arrive(&empty[stg]);
-          __threadfence_block();
-          wdone_s[warp] = ++tiles_done;                  // after the arrivals above: the control warp counts on that order
-        }
+        if (lane == 0) mbar_arrive(&empty[stg]);
       }
       // ---- last message of the pass: the partial half, its unused voxels zeroed (warp 0 of the group) ----
       {
         const unsigned h = half_base + fill / kTcHV, used = fill % kTcHV;
-        if ((p.dbg & 64) && blockIdx.x == 0 && lane == 0) printf("w %d flush h %u used %u arrived %u verified %u\n", warp, h, used, arrived, verified);
         verify_upto(h + 1u);
         if (wg == 0 && used > 0u) {
           for (unsigned cc = used + (unsigned)q4; cc < (unsigned)kTcHV; cc += 4u) {
@@ -1062,19 +1032,23 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
         fence_async_smem();
         __syncwarp();
         if (lane == 0) {
-          if (wg == 0) smeta_s[grp][h & 1u] = (used > 0u ? 1 : 0) | 2 | (tiles_done << 8);
+          if (wg == 0) smeta_s[grp][h & 1u] = (used > 0u ? 1 : 0) | 2;
           mbar_arrive(&sfull[2 * grp + (h & 1u)]);
         }
         half_base = h + 1u;
-        if (fill > 0u) si[10] = 1;                       // this CTA issued at least one MMA: the accumulators are live
+        if (fill > 0u && wg == 0 && lane == 0) live_s[grp] = 1;   // the group's accumulator is live in this pass
       }
 #undef CYC_MARK
     }
     cbase += ntl;
     // the slab area is recycled below (lh, gradient partials, hred): every warp must be past its last write
+    const long long t_tail = prof ? clock64() : 0ll;
     wsync();
+    if (prof) prof_s[8] += (unsigned long long)(clock64() - t_tail);     // EXPERIMENT: wait for the other warps
     PROF_MARK(1);
+    const long long t_acc = prof ? clock64() : 0ll;
     mbar_wait(acc_full, acc_phase);
+    if (prof) prof_s[9] += (unsigned long long)(clock64() - t_acc);      // EXPERIMENT: wait for the accumulators
     acc_phase ^= 1u;
     tc_fence_after();
     // ---- gradient: lanes (q, r) -> r; rows r + 8 i.  Per-warp partials, added in warp order below ----
@@ -1092,24 +1066,46 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
     // ---- accumulators: TMEM lanes 0..63 hold hh, lanes 64..127 lh (columns 0..63); lh goes through shared memory ----
     const int lq = warp & 3, cs0 = (warp >> 2) * 16;   // lane quarter, first of the 16 columns of this warp
     const int row = 32 * (lq & 1) + lane;
-    const bool any_h = si[10] != 0 && !(p.dbg & 8);
-    if (any_h && lq >= 2) {
-      float vv[16];
-      tmem_ld16(tmem_base + ((uint32_t)(32 * lq) << 16) + (uint32_t)cs0, vv);
+    bool any_h = false;
 #pragma unroll
-      for (int jj = 0; jj < 16; ++jj) lh_s[row * 65 + cs0 + jj] = vv[jj];
+    for (int g = 0; g < kTcGroups; ++g) any_h = any_h || (live_s[g] != 0);
+    if (any_h && lq >= 2) {
+      float acc[16];
+#pragma unroll
+      for (int jj = 0; jj < 16; ++jj) acc[jj] = 0.f;
+#pragma unroll
+      for (int g = 0; g < kTcGroups; ++g) {
+        if (live_s[g]) {
+          float vv[16];
+          tmem_ld16(tmem_base + ((uint32_t)(32 * lq) << 16) + (uint32_t)(64 * g + cs0), vv);
+#pragma unroll
+          for (int jj = 0; jj < 16; ++jj) acc[jj] += vv[jj];
+        }
+      }
+#pragma unroll
+      for (int jj = 0; jj < 16; ++jj) lh_s[row * 65 + cs0 + jj] = acc[jj];
     }
     wsync();
     if (lq < 2 && row - lane < 8 * nb) {               // warp-uniform: tcgen05.ld is a warp-wide instruction
-      float vv[16];
-      if (any_h) tmem_ld16(tmem_base + ((uint32_t)(32 * lq) << 16) + (uint32_t)cs0, vv);
+      double hh[16];
+#pragma unroll
+      for (int jj = 0; jj < 16; ++jj) hh[jj] = 0.0;
+#pragma unroll
+      for (int g = 0; g < kTcGroups; ++g) {
+        if (live_s[g]) {
+          float vv[16];
+          tmem_ld16(tmem_base + ((uint32_t)(32 * lq) << 16) + (uint32_t)(64 * g + cs0), vv);
+#pragma unroll
+          for (int jj = 0; jj < 16; ++jj) hh[jj] += (double)vv[jj];
+        }
+      }
 #pragma unroll
       for (int jj = 0; jj < 16; ++jj) {
         const int col = cs0 + jj;
         if (row < 8 * nb && col < 8 * nb && (row >> 3) <= (col >> 3)) {
           double h = 0.0;
           if (row < K && col < K) {
-            if (any_h) h = ((double)vv[jj] + (double)lh_s[row * 65 + col]) + (double)lh_s[col * 65 + row];
+            if (any_h) h = (hh[jj] + (double)lh_s[row * 65 + col]) + (double)lh_s[col * 65 + row];
           } else if (col == K && row < K) {            // gradient column of the augmented matrix
             double g = 0.0;
             for (int w = 0; w < kNW; ++w) g += gpart[w * 64 + row];
@@ -1147,7 +1143,6 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
     }
     ++passes;
     if (passes == 1) F = hred[nblocks * 64];
-    if ((p.dbg & 128) && blockIdx.x == 0 && tid == 0) printf("pass %d K %d H00 %.10e g0 %.10e F %.10e\n", passes, K, hred[0], h_at(hred, nb, 0, K), hred[nblocks * 64]);
     if (restoring) have_dir = false;
     // ================= decision on the pass just made (warp 0; identical in every CTA) =================
     if (warp == 0) {
@@ -1445,7 +1440,7 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
   // ---- publish ----
   // drain: every issued stage must have landed before the CTA may exit
   if constexpr (TC) {
-    if (tid == 0) {                                          // the feeder drains the ring, the control warp frees the TMEM
+    if (tid == 0) {                                          // the feeder drains the ring, a control warp frees the TMEM
       total_tiles_s = cbase;
       __threadfence_block();
       stop_s = 1;
@@ -1644,11 +1639,8 @@ cudaError_t launch_newton(Ctx *c, bool add_candidate) {
   p.max_iter = c->opt.master_max_iter;
   p.k_max = c->opt.k_max;
   p.tol = c->opt.master_tol;
-  { const char *e = getenv("DAO_DEBUG"); p.dbg = e ? atoi(e) : 0; }
   void *args[] = {&p};
   ++c->n_launches;
-  if (p.dbg & 16) return cudaStreamSynchronize(c->stream);
-  if (p.dbg & 32) { cudaError_t e0 = cudaStreamSynchronize(c->stream); if (e0 != cudaSuccess) { fprintf(stderr, "before newton: %s\n", cudaGetErrorString(e0)); return e0; } }
   if (L.tc)
     return cudaLaunchCooperativeKernel((void *)k_master_newton<true>, dim3(c->master_grid), dim3(kNwtTcThreads), args,
                                        L.smem, c->stream);
