@@ -146,7 +146,8 @@ typedef struct {
   int32_t mlc_mode;          /* dao_mlc_mode (default DAO_MLC_CONSECUTIVE) */
   int32_t reserved;          /* test/bench hooks, 0 in production: bit 0 forces the direct-load SpMV variant,
                                 bit 1 turns on the master's phase timers (DAO_VEC_MASTER_PHASES), bit 2 forces the span variant
-                                of the transposed SpMV even for short beamlet rows */
+                                of the transposed SpMV even for short beamlet rows, bit 4 runs the Newton master
+                                (methods 2, 3) on 8 CTAs so that small inputs exercise many tiles per CTA */
   int32_t pad_;              /* keep 0 */
 } dao_options;
 

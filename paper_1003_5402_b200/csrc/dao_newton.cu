@@ -33,7 +33,6 @@
 #include <math_constants.h>
 
 #include <algorithm>
-#include <cstdlib>
 
 namespace dao {
 
@@ -824,7 +823,6 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
     double gacc[kNwtAcc];
 #pragma unroll
     for (int i = 0; i < kNwtAcc; ++i) gacc[i] = 0.0;
-    const long long t_head = prof ? clock64() : 0ll;
     if (tid < K) ycur_s[tid] = yv[tid];
     if (tid < kTcGroups) live_s[tid] = 0;
     wsync();
@@ -873,7 +871,6 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
           ++arrived;
         }
       };
-      if (prof) prof_s[10] += (unsigned long long)(clock64() - t_head);   // EXPERIMENT: head of the pass
       int tix = 0;
       for (int j = grp; j < ntl; j += kTcGroups, ++tix) {
         const long long c = cbase + j;
@@ -1042,13 +1039,9 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
     }
     cbase += ntl;
     // the slab area is recycled below (lh, gradient partials, hred): every warp must be past its last write
-    const long long t_tail = prof ? clock64() : 0ll;
     wsync();
-    if (prof) prof_s[8] += (unsigned long long)(clock64() - t_tail);     // EXPERIMENT: wait for the other warps
     PROF_MARK(1);
-    const long long t_acc = prof ? clock64() : 0ll;
     mbar_wait(acc_full, acc_phase);
-    if (prof) prof_s[9] += (unsigned long long)(clock64() - t_acc);      // EXPERIMENT: wait for the accumulators
     acc_phase ^= 1u;
     tc_fence_after();
     // ---- gradient: lanes (q, r) -> r; rows r + 8 i.  Per-warp partials, added in warp order below ----
@@ -1592,7 +1585,7 @@ cudaError_t newton_fill_tile_meta(Ctx *c) {
 
 cudaError_t newton_configure(Ctx *c) {
   c->master_grid = std::min(c->n_sm, kMasterMaxGrid);
-  { const char *e = getenv("DAO_GRID"); if (e) c->master_grid = atoi(e); }
+  if (c->opt.reserved & 16) c->master_grid = std::min(c->master_grid, 8);   // test hook: many tiles per CTA on small inputs
   const NewtonLayout &L = c->nwt;
   const void *fn = L.tc ? (const void *)k_master_newton<true> : (const void *)k_master_newton<false>;
   cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.smem);

@@ -258,7 +258,11 @@ __global__ void __launch_bounds__(kSpmvRingThreads, 1) k_spmv_ring(SpmvParams p)
         for (int k = 0; k < kn; ++k) acc = fma((double)sv[k * 32], (double)xs[sc[k * 32]], acc);
       }
       ++n_consumed;
-      __syncwarp();                          // every lane is done with the stage before it is refilled
+      // every lane is done with the stage before it is refilled; the proxy fence orders the lanes' generic-proxy
+      // reads before the bulk copy (async proxy) -- without it a refill was seen to overtake reads still queued
+      // (k_spmvt_ring, where the values are consumed after the refill is issued)
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      __syncwarp();
       issue();
     }
     spmv_store<MODE>(p, out, stab_s, slice * 32 + lane, acc, f_acc, kcol);

@@ -107,15 +107,17 @@ def test_cfg1_lockstep_first_iterations(D, cfg1):
             assert -1e-5 <= rel <= REL_OBJ, (it, m.objective, res.objective)
 
 
-def test_cfg1_plan_50_apertures(D, cfg1):
+@pytest.mark.parametrize("method", [2, 3])
+def test_cfg1_plan_50_apertures(D, cfg1, method):
     """The north-star target: a free-running 50-aperture plan of configs[1], run exactly as bench.py
     runs it, against (i) the oracle's own free-running plan (stored fixture), (ii) the oracle's
-    recomputation of dose / objective / reduced costs from the GPU's plan."""
+    recomputation of dose / objective / reduced costs from the GPU's plan.  Method 2 (the default; exact Hessian on
+    the fp64 tensor cores) and method 3 (Hessian on tcgen05 in split TF32)."""
     ph = cfg1
     with open(os.path.join(GOLDEN, "oracle_plan_cfg1.json")) as f:
         gold = json.load(f)
     assert (gold["n_vox"], gold["n_bl"], gold["nnz"]) == (ph.n_vox, ph.n_bl, ph.nnz)
-    with D.Dao(ph, k_max=50) as d:
+    with D.Dao(ph, k_max=50, master_method=method) as d:
         info = d.run(50)
         plan = d.get_plan()
         hist = d.get_vector(D.VEC_HISTORY)[:info.n_apertures]
@@ -145,7 +147,7 @@ def test_cfg1_plan_50_apertures(D, cfg1):
     assert gap <= REL_OBJ * F_o, (gap, F_o)
     f = np.r_[hist["objective_before"][:1], hist["objective"]]
     assert (np.diff(f) <= 1e-9 * f[:-1]).all() and (hist["price"] < 0).all() and (plan.intensity >= 0).all()
-    print(f"cfg1: F_gpu={info.objective:.12g} F_oracle={gold['objective']:.12g} rel={rel:.2e} same beams {n_same}/50 "
+    print(f"cfg1 method {method}: F_gpu={info.objective:.12g} F_oracle={gold['objective']:.12g} rel={rel:.2e} same beams {n_same}/50 "
           f"pg iterations {info.n_pg_iter_total} kkt gap {gap:.2e}")
 
 
