@@ -116,6 +116,11 @@ typedef struct {
                                     T_s^+ of voxel j's structure (finite values) */
   int32_t per_voxel_weights;     /* 0: weights alpha_s / |v_s|, beta_s / |v_s| (eq. 9-10); 1: alpha_s, beta_s are the
                                     per-voxel weights alpha_j, beta_j of eq. 3-4 as they are (no division by |v_s|) */
+  /* Voxel-row slab: when D holds only a slab of the voxel rows of a larger problem, |v_s| of eq. 9-10
+     is the structure's voxel count in the WHOLE problem, not in the slab.  Optional [n_struct] host array; NULL:
+     the context counts its own voxels.  With it, dao_eval_x returns the slab's share of F, dao_spmv_t the slab's
+     partial sum of w = D^T pi (eq. 8): the caller adds the shares over the slabs in slab order. */
+  const int64_t *struct_count;
 } dao_structs;
 
 /* Options.  Zero-initialise, then dao_default_options, then override. */

@@ -641,7 +641,8 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   {
     std::vector<StructEntry> tab(256, StructEntry{0.0, 0.0, 0.0, 0.0});
     for (int i = 0; i < s->n_struct; ++i) {
-      const double n = (double)h_flags[1 + i];
+      // |v_s|: the context's own count, or the caller's count over the whole problem (voxel-row slab)
+      const double n = s->struct_count ? (double)s->struct_count[i] : (double)h_flags[1 + i];
       const double div = s->per_voxel_weights ? 1.0 : n;       // eq. 3-4 as given, or eq. 9-10 per |v_s|
       tab[i].a = n > 0 ? (double)s->w_under[i] / div : 0.0;
       tab[i].b = n > 0 ? (double)s->w_over[i] / div : 0.0;

@@ -52,7 +52,7 @@ class CMlc(C.Structure):
 class CStructs(C.Structure):
     _fields_ = [("n_struct", C.c_int32), ("vox_struct", C.c_void_p), ("t_under", C.c_void_p),
                 ("w_under", C.c_void_p), ("t_over", C.c_void_p), ("w_over", C.c_void_p),
-                ("vox_threshold", C.c_void_p), ("per_voxel_weights", C.c_int32)]
+                ("vox_threshold", C.c_void_p), ("per_voxel_weights", C.c_int32), ("struct_count", C.c_void_p)]
 
 
 class COptions(C.Structure):
@@ -219,6 +219,14 @@ class Dao:
             else:
                 self._keep.append(vt)
                 st.vox_threshold = _np_ptr(vt)
+        # voxel-row slab: |v_s| of the whole problem, see paper_1003_5402_b200.sharded
+        sc = getattr(ph, "struct_count", None)
+        if sc is not None:
+            sc = np.ascontiguousarray(sc, dtype=np.int64)
+            if sc.size != tu.size:
+                raise ValueError("struct_count must have n_struct entries")
+            self._keep.append(sc)
+            st.struct_count = _np_ptr(sc)
         mlc = CMlc(self.n_beams, self.n_rows, _np_ptr(brp), _np_ptr(rbp))
         rc0 = getattr(ph, "row_col0", None)
         if rc0 is not None:

@@ -40,7 +40,7 @@ def test_default_options_and_struct_layout(lib):
     assert (o.k_max, o.master_max_iter, o.master_method, o.timers) == (50, 2000, 2, 1)
     assert o.master_tol == 1e-7 and o.price_tol == 1e-6 and o.master_ls_tol == 0.01
     # sizes the C side was compiled with (natural alignment, no packing)
-    assert C.sizeof(dao.COptions) == 56 and C.sizeof(dao.CMlc) == 32 and C.sizeof(dao.CStructs) == 64 and C.sizeof(dao.CCsr) == 48 and C.sizeof(dao.CPriceInfo) == 48
+    assert C.sizeof(dao.COptions) == 56 and C.sizeof(dao.CMlc) == 32 and C.sizeof(dao.CStructs) == 72 and C.sizeof(dao.CCsr) == 48 and C.sizeof(dao.CPriceInfo) == 48
     assert C.sizeof(dao.CMasterInfo) == 48 and C.sizeof(dao.CIterRecord) == 56 == dao.ITER_RECORD_DTYPE.itemsize
     assert C.sizeof(dao.CRunInfo) == 112 and C.sizeof(dao.CPlan) == 64 and C.sizeof(dao.CDims) == 56
 
