@@ -117,7 +117,7 @@ def master_alg_bytes(method: int, V: int, K: int, n_iter: int, n_passes: int) ->
     """Algorithmic bytes of one master solve.  Methods 0/1: per projected-gradient
     iteration 2*4*V*K (two passes over A) + (n_ls + 3)*8*V with n_ls = the repeated gradient passes per iteration.
     Method 2: every pass reads A once (4*V*K), reads sid (V) and writes the fp64 dose (8*V)."""
-    if method == 2:
+    if method >= 2:      # 3: the same pass with the Hessian on tcgen05; sid and thresholds ride in the tile (2 meta rows)
         return float(n_passes) * (4.0 * V * K + 9.0 * V)
     n_ls = max(0, n_passes - (2 * n_iter + 1))
     return n_iter * (2.0 * 4.0 * V * K + 3.0 * 8.0 * V) + n_ls * (4.0 * V * K + 8.0 * V)
@@ -324,9 +324,11 @@ def main():
     ap.add_argument("--apertures", type=int, default=N_APERTURES, help="apertures per plan (50; configs[4] asks for 100)")
     ap.add_argument("--ref-apertures", type=int, default=0,
                     help="apertures of the oracle run behind cpu_baseline / --impl reference (0 = the full plan; fewer = a scaled prefix)")
-    ap.add_argument("--master-method", type=int, default=2, help="dao_options.master_method (2 = projected Newton, 1 = conjugated gradient projection)")
+    ap.add_argument("--master-method", type=int, default=2, help="dao_options.master_method (2 = projected Newton, exact Hessian on the fp64 tensor cores; 3 = the same with the Hessian on tcgen05 in split TF32; 1 = conjugated gradient projection)")
     ap.add_argument("--split-steps", type=int, default=2, help="plans of the separate per-kernel-class timing pass")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="skip the plan times of paper_p1 / configs[2] / configs[4] and of master_method = 3 that the default run appends")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[3] kernel sweep (markdown table)")
     ap.add_argument("--widened", action="store_true", help="measure the SURVEY 8(f) rows (FMO, re-optimisation, MLC modes)")
@@ -453,9 +455,9 @@ def main():
         "regimes": regimes})
     plan_bytes = N_APERTURES * (ab["spmv"] + ab["spmv_t"] + ab["price"] + ab["column"]) + master_bytes_plan
 
-    master_kernel = "k_master_newton" if method == 2 else "k_master"
+    master_kernel = "k_master_newton" if method >= 2 else "k_master"
     master_model = ("per pass over A: 4*V*K (A read once) + V (sid) + 8*V (fp64 dose written); a solve makes `passes` passes"
-                    if method == 2 else
+                    if method >= 2 else
                     "SURVEY 8(d): per projected-gradient iteration 2*4*V*K + (n_ls+3)*8*V, n_ls = repeated gradient passes")
 
     def traffic_of(kernel, alg_of_launch):
@@ -523,6 +525,37 @@ def main():
         e2e = {"value": e / world, "unit": "s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                "includes": f"dao_create from pinned host CSR (H2D + sliced-ELL + transpose build), dao_run({N_APERTURES}), dao_get_plan"}
 
+    # ---- the other BASELINE.json configs and master_method = 3, plan time only (rank 0, N = 1; bounded) ----
+    others = None
+    if rank == 0 and world == 1 and args.config == "cfg1" and not args.no_other_configs:
+        others = {}
+        t_budget = time.perf_counter()
+
+        def plan_time(ph_o, n_ap, **o):
+            with dao.Dao(ph_o, timers=0, k_max=n_ap, **o) as d3:
+                for _ in range(3):
+                    d3.reset()
+                    inf3 = d3.run(n_ap)
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for _ in range(3):
+                    d3.reset()
+                    inf3 = d3.run(n_ap)
+                e1.record()
+                torch.cuda.synchronize()
+                return {"seconds_per_plan": e0.elapsed_time(e1) * 1e-3 / 3, "apertures": int(inf3.n_apertures),
+                        "objective": inf3.objective, "master_passes_over_A": int(inf3.n_passes_total),
+                        "master_method": int(d3.opt.master_method), "n_vox": int(ph_o.n_vox), "n_bl": int(ph_o.n_bl),
+                        "nnz": int(ph_o.nnz)}
+
+        others["cfg1_master_method_3"] = plan_time(ph, N_APERTURES, master_method=3)
+        for name, n_ap in (("paper_p1", 50), ("cfg2", 50), ("cfg4", 100)):
+            if time.perf_counter() - t_budget > 150.0:
+                others[name] = {"skipped": "time budget of the default run"}
+                continue
+            others[name] = plan_time(phantom.make(name, 0), n_ap, master_method=args.master_method)
+
     # ---- CPU baseline: the oracle as it stands, one full plan, rank 0, N = 1 only ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -534,7 +567,7 @@ def main():
                "scaling": "weak", "vs_baseline": None, "dtype": "f32 storage, f64 accumulate", "data": "synthetic",
                "config": workload_config(ph, args), "clocks": clocks, "e2e": e2e,
                "gpu_launches": int(launches), "roofline": roofline, "roofline_kernels": roofline_kernels,
-               "roofline_master": master_roofline, "cpu_baseline": cpu, "kernels": kernels,
+               "roofline_master": master_roofline, "cpu_baseline": cpu, "kernels": kernels, "other_configs": others,
                "plan": {"objective": last.objective, "apertures": last.n_apertures, "cg_iterations_per_s": n_it / elapsed,
                         "master_iterations": int(last.n_pg_iter_total), "master_passes_over_A": int(last.n_passes_total),
                         "master_hit_max_iter": int(last.n_hit_max_iter), "converged": int(last.converged),

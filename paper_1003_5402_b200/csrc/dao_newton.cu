@@ -59,7 +59,7 @@ constexpr uint32_t kTcLbo = 128, kTcSbo = (kTcHV / 4) * kTcLbo, kTcHalfBytes = 1
 constexpr uint32_t kTcCols = 64 * kTcGroups;   // TMEM columns: one 128 x 64 fp32 accumulator per group
 constexpr int kTcMaxK = 56;              // 8 block rows of the augmented Hessian fit the 64 rows of one operand half
 constexpr int kTcMaxStages = 12;
-constexpr int kTcMetaRows = 2;
+constexpr int kNwtMetaRows = 2;
 constexpr int kNwtAcc = 7;               // gradient accumulators per thread: rows r, r + 8, ... < 56
 
 struct NewtonParams {
@@ -388,7 +388,7 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
     if (warp == kNW + 2) {
       if (lane == 0 && ntl > 0) {
         const int Kc = p.st->K + ((p.add_candidate && p.st->cand_valid) ? 1 : 0);
-        const uint32_t bytes = (uint32_t)(Kc + kTcMetaRows) * (uint32_t)TP * 4u;
+        const uint32_t bytes = (uint32_t)(Kc + kNwtMetaRows) * (uint32_t)TP * 4u;
         RingPos ipc{0, 0u};
         long long c = 0;
         int j = 0;
@@ -492,7 +492,7 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
   int issued_total = 0, consumed_total = 0, issue_ti = 0;
   bool issue_rev = false;
   const bool is_issuer = tid == kMasterWorkers - 32;
-  const uint32_t tile_bytes = (uint32_t)K * (uint32_t)TP * 4u;
+  const uint32_t tile_bytes = (uint32_t)(K + kNwtMetaRows) * (uint32_t)TP * 4u;   // two meta rows + the K live columns
   auto feed = [&]() {                      // issue copies while stages are free; never blocks
     while (ntl > 0) {
       // the stage was used before: all front warps must have released it (try_wait would block for ~0.5 us)
@@ -540,21 +540,6 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
           if (i + u < nI) c[u] = fma(yv[zsl + ((i + u) << ks_shift)], kTiny, c[u]);
         zc = (c[0] + c[1]) + (c[2] + c[3]);
       }
-      // structure id / threshold of this thread's voxel, fetched one tile ahead (an L2 round trip is longer than Z)
-      int sid_n = kNoStruct;
-      float vt_n = 0.f;
-      auto fetch_sid = [&](int ti_) {
-        sid_n = kNoStruct;
-        vt_n = 0.f;
-        if (ti_ < ntl) {
-          const int vg = (tb0 + (rev ? ntl - 1 - ti_ : ti_) * tstep) * T + v0;
-          if (zsl == 0 && vg < p.n_vox_pad) {
-            sid_n = p.sid[vg];
-            if (p.vt) vt_n = p.vt[vg];
-          }
-        }
-      };
-      fetch_sid(0);
       for (int ti = 0; ti < ntl; ++ti) {
         const int tile = tb0 + (rev ? ntl - 1 - ti : ti) * tstep;
         long long tc = prof ? clock64() : 0ll;
@@ -566,15 +551,16 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
       tc = now_;                                          \
     }                                                     \
   } while (0)
-        // structure id / threshold of this thread's voxel: issued before the wait, used after the Z loop
         const int vg0 = tile * T + v0;
         const bool in0 = zsl == 0 && vg0 < p.n_vox_pad;
-        const int sid0 = sid_n;
-        const float vt0 = vt_n;
-        fetch_sid(ti + 1);
         mbar_wait(&full[cp.stage], cp.phase);
         CYC_MARK(12);
-        const float *M = reinterpret_cast<const float *>(ring + (size_t)cp.stage * p.stage_bytes);
+        // the tile starts with two meta rows: the structure ids and the per-voxel thresholds of its voxels (the front
+        // warps used to fetch them from global memory: an exposed L2 round trip per tile)
+        const unsigned char *stage = ring + (size_t)cp.stage * p.stage_bytes;
+        const float *M = reinterpret_cast<const float *>(stage) + kNwtMetaRows * TP;
+        const int sid0 = stage[v0];
+        const float vt0 = reinterpret_cast<const float *>(stage)[TP + v0];
         // ---- Z ----
         double z0;
         {
@@ -890,7 +876,7 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
         mbar_wait(&full[stg], par);
         CYC_MARK(12);
         const unsigned char *stage = ring + (size_t)stg * p.stage_bytes;
-        const float *M = reinterpret_cast<const float *>(stage) + kTcMetaRows * TP;   // column 0 of the tile
+        const float *M = reinterpret_cast<const float *>(stage) + kNwtMetaRows * TP;   // column 0 of the tile
         // ---- Z ----
         double z0;
         {
@@ -1523,10 +1509,10 @@ NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct, b
     // 64 KB also hold hred, the factorisation buffer, lh and the gradient partials between the passes)
     L.tc = 1;
     L.kp = 64; L.lbo = (int32_t)kTcLbo; L.sbo = (int32_t)kTcSbo; L.w_bytes = (int32_t)kTcHalfBytes; L.tmem_cols = (int32_t)kTcCols;
-    L.meta_rows = kTcMetaRows;
+    L.meta_rows = kNwtMetaRows;
     L.T = kTcT; L.TP = kTcT + 4; L.AC = 64;
     L.lbuf_doubles = std::max((k_max + 1) * (k_max + 2) / 2 + 8, kNW * 32);
-    L.stage_bytes = (int32_t)align_up((size_t)(k_max + kTcMetaRows) * L.TP * 4, 128);
+    L.stage_bytes = (int32_t)align_up((size_t)(k_max + kNwtMetaRows) * L.TP * 4, 128);
     const size_t recycled = align_up((size_t)L.n_red * 8, 128) + align_up((size_t)L.lbuf_doubles * 8, 128) +
                             align_up((size_t)64 * 65 * 4, 128) + (size_t)kNW * 64 * 8;
     const size_t fixed = 5 * 128 + (size_t)kNW * 32 * 13 + align_up((size_t)std::max(n_struct, 1) * sizeof(StructEntry), 128) +
@@ -1536,7 +1522,7 @@ NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct, b
     L.n_stages = stages;
     L.smem = fixed + (size_t)stages * L.stage_bytes;
     L.n_tiles = (n_vox_pad + L.T - 1) / L.T;
-    L.tile_stride = (int64_t)(k_max + kTcMetaRows) * L.TP;
+    L.tile_stride = (int64_t)(k_max + kNwtMetaRows) * L.TP;
     return L;
   }
   static const int32_t cand_t[] = {256, 128, 64, 32};        // T x k-slices = 256 front threads
@@ -1545,7 +1531,7 @@ NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct, b
     for (int32_t AC : cand_ac) {
       const int32_t lbuf = std::max((k_max + 1) * (k_max + 2) / 2 + 8, 2 * (8 * L.nb_max + 1) * (AC + 4));
       const int32_t TP = T + 4;
-      const int32_t stage = (int32_t)align_up((size_t)k_max * TP * 4, 128);
+      const int32_t stage = (int32_t)align_up((size_t)(k_max + kNwtMetaRows) * TP * 4, 128);
       const size_t fixed = newton_fixed_smem(k_max, T, n_struct, L.n_red, lbuf);
       if (fixed + (size_t)kNwtMinStages * stage > budget && !(AC == 16 && T == 32)) continue;
       if (AC == 16 && T > 32) continue;                      // rather a smaller tile than 4-quad chunks
@@ -1558,8 +1544,9 @@ NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct, b
     }
     if (L.T) break;
   }
+  L.meta_rows = kNwtMetaRows;
   L.n_tiles = (n_vox_pad + L.T - 1) / L.T;
-  L.tile_stride = (int64_t)k_max * L.TP;
+  L.tile_stride = (int64_t)(k_max + kNwtMetaRows) * L.TP;
   return L;
 }
 
@@ -1576,7 +1563,7 @@ __global__ void k_newton_tile_meta(float *A, int32_t n_tiles, int32_t T, int32_t
 
 cudaError_t newton_fill_tile_meta(Ctx *c) {
   const NewtonLayout &L = c->nwt;
-  if (!L.tc) return cudaSuccess;
+  if (!L.meta_rows) return cudaSuccess;
   const int n = L.n_tiles * L.T;
   k_newton_tile_meta<<<(n + 255) / 256, 256, 0, c->stream>>>(c->d.A, L.n_tiles, L.T, L.TP, L.tile_stride, c->d.sid,
                                                            c->has_vt ? c->d.vt : nullptr, c->n_vox_pad);
