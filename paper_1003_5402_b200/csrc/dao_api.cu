@@ -30,13 +30,15 @@ static dao_status fail(Ctx *c, dao_status st, const char *msg) {
 // ------------------------------------------------------------------------------------------
 namespace dao {
 
+// tile_T > 0: `in` is in the tiled order of the Newton master (voxel i at slot i / n_tiles of tile i mod n_tiles)
 template <typename T>
 __global__ void k_to_user_order(int32_t n_vox_pad, const int32_t *__restrict__ perm, const T *__restrict__ in,
-                                T *__restrict__ out) {
+                                T *__restrict__ out, int32_t tile_T, int32_t n_tiles) {
   const int32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_vox_pad) return;
   const int32_t j = perm[i];
-  if (j >= 0) out[j] = in[i];
+  if (j < 0) return;
+  out[j] = tile_T > 0 ? in[(size_t)(i % n_tiles) * tile_T + (size_t)(i / n_tiles)] : in[i];
 }
 
 // 0/1 beamlet mask of pool aperture k (for dao_set_pool)
@@ -382,7 +384,7 @@ dao_status dao_get_vector(dao_ctx *ctx, int32_t which, void *dst, dao_memspace m
     case DAO_VEC_G: src = c->d.g; bytes = (size_t)c->n_vox * 4; break;
     case DAO_VEC_MASTER_Z: {
       double *tmp = reinterpret_cast<double *>(c->d.io_scratch);
-      k_to_user_order<double><<<gv, t, 0, c->stream>>>(c->n_vox_pad, c->d.perm, c->d.mz, tmp);
+      k_to_user_order<double><<<gv, t, 0, c->stream>>>(c->n_vox_pad, c->d.perm, c->d.mz, tmp, c->nwt.T, c->nwt.n_tiles);
       API_CUDA(cudaGetLastError());
       src = tmp; bytes = (size_t)c->n_vox * 8;
       break;

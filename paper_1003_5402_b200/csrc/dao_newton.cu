@@ -555,8 +555,8 @@ __global__ void __launch_bounds__(TC ? kNwtTcThreads : kMasterWorkers, 1) k_mast
       tc = now_;                                          \
     }                                                     \
   } while (0)
-        const int vg0 = tile * T + v0;
-        const bool in0 = zsl == 0 && vg0 < p.n_vox_pad;
+        const int vg0 = tile * T + v0;                 // position of the voxel in the tiled order (mz is kept in it)
+        const bool in0 = zsl == 0;                       // slots without a voxel carry kNoStruct and zero columns
         mbar_wait(&full[cp.stage], cp.phase);
         CYC_MARK(12);
         // the tile starts with two meta rows: the structure ids and the per-voxel thresholds of its voxels (the front
@@ -1540,9 +1540,10 @@ NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct, b
 // master_method = 3: the structure id and the threshold of every voxel of a tile, in the tile's two meta rows
 __global__ void k_newton_tile_meta(float *A, int32_t n_tiles, int32_t T, int32_t TP, int64_t tile_stride, const uint8_t *sid,
                                    const float *vt, int32_t n_vox_pad) {
-  const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x);
-  if (i >= n_tiles * T) return;
-  const int t = i / T, v = i - t * T;
+  const int pos = (int)(blockIdx.x * blockDim.x + threadIdx.x);
+  if (pos >= n_tiles * T) return;
+  const int t = pos / T, v = pos - t * T;
+  const int i = v * n_tiles + t;                     // the voxel at slot v of tile t (a_index)
   float *tile = A + (size_t)t * (size_t)tile_stride;
   reinterpret_cast<uint8_t *>(tile)[v] = (i < n_vox_pad) ? sid[i] : (uint8_t)kNoStruct;
   tile[TP + v] = (vt != nullptr && i < n_vox_pad) ? vt[i] : 0.f;

@@ -148,7 +148,7 @@ static void carve_workspace(Carver &cv, const Dims &dm, const HostLayout &L, Dev
   const NewtonLayout nl = layout_of_master(dm, L.n_vox_pad);
   d->A = cv.take<float>(nl.T ? (size_t)nl.n_tiles * (size_t)nl.tile_stride : (size_t)dm.k_max * vp);
   d->y = cv.take<double>((size_t)DAO_MAX_APERTURES);
-  d->mz = cv.take<double>(vp);
+  d->mz = cv.take<double>(nl.T ? (size_t)nl.n_tiles * (size_t)nl.T : vp);   // the Newton master keeps it in the tiled order
   d->mdz = cv.take<double>(vp);
   {
     const size_t g = (size_t)std::min(n_sm * kMasterCtasPerSm, kMasterMaxGrid);
@@ -763,10 +763,10 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   SETUP_CUDA(cudaMemsetAsync(d.g, 0, vp * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.w, 0, (size_t)dm.n_bl * 4, q));
   SETUP_CUDA(cudaMemsetAsync(d.y, 0, DAO_MAX_APERTURES * 8, q));
-  SETUP_CUDA(cudaMemsetAsync(d.mz, 0, vp * 8, q));
   SETUP_CUDA(cudaMemsetAsync(d.mdz, 0, vp * 8, q));
   c->nwt = layout_of_master(dm, L.n_vox_pad);
   c->red_stride = c->nwt.T ? c->nwt.n_red : kMaxRedux;
+  SETUP_CUDA(cudaMemsetAsync(d.mz, 0, (c->nwt.T ? (size_t)c->nwt.n_tiles * (size_t)c->nwt.T : vp) * 8, q));
   {
     const size_t g = (size_t)std::min(c->n_sm * kMasterCtasPerSm, kMasterMaxGrid);
     SETUP_CUDA(cudaMemsetAsync(d.ll_part, 0, 2 * g * (size_t)c->red_stride * sizeof(uint4), q));

@@ -71,7 +71,7 @@ struct SpmvParams {
   DevState *st;
   const int32_t *skip;       // device flag (may be null): non-zero -> the launch does nothing
   // column mode: layout of the dose block A (a_index) and the column to write (< 0: the pool size K)
-  int32_t a_T, a_TP, a_col;
+  int32_t a_T, a_TP, a_col, a_ntiles;
   int64_t a_stride;
   // column mode with a_col < 0: x is the 0/1 mask of the pending candidate, built while x is staged (no mask array,
   // no extra pass): beamlet i is open iff its leaf row belongs to the candidate's beam and i lies in [left, right)
@@ -114,7 +114,7 @@ __device__ __forceinline__ void spmv_store(const SpmvParams &p, float *out, cons
     const int32_t j = p.perm[i];
     if (j >= 0) out[j] = (float)acc;
   } else if (MODE == kSpmvColumn) {
-    out[a_index(p.a_T, p.a_TP, p.a_stride, p.n_vox_pad, i, kcol)] = (float)acc;
+    out[a_index(p.a_T, p.a_TP, p.a_stride, p.n_vox_pad, p.a_ntiles, i, kcol)] = (float)acc;
   } else {
     out[i] = (float)acc;
   }
@@ -351,7 +351,7 @@ static cudaError_t launch_spmv_mode(Ctx *c, const float *x, float *out, const in
   p.f_part = c->d.f_part;
   p.st = c->d.state;
   p.skip = skip;
-  p.a_T = c->nwt.T; p.a_TP = c->nwt.TP; p.a_stride = c->nwt.tile_stride; p.a_col = a_col;
+  p.a_T = c->nwt.T; p.a_TP = c->nwt.TP; p.a_stride = c->nwt.tile_stride; p.a_col = a_col; p.a_ntiles = c->nwt.n_tiles;
   if (MODE == kSpmvColumn) p.out = c->d.A + (size_t)c->nwt.meta_rows * (size_t)c->nwt.TP;   // column 0 of tile 0
   p.bl_row = c->d.bl_row; p.row_beam = c->d.row_beam; p.row_bl_ptr = c->d.row_bl_ptr; p.left = c->d.left; p.right = c->d.right;
   p.mask_from_candidate = (MODE == kSpmvColumn && a_col < 0 && spmv_builds_mask(c)) ? 1 : 0;
