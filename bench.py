@@ -92,7 +92,7 @@ def algorithmic_bytes(ph, sell_elems=None):
     }
 
 
-TRAFFIC_CSV = os.path.join("profiles", "r02_traffic.csv")   # one `ncu --set full` capture per kernel; see profiles/r02_traffic.md
+TRAFFIC_CSV = os.path.join("profiles", "r02b_traffic.csv")   # one `ncu --set full` capture per kernel; see profiles/r02b_traffic.md
 
 
 def ncu_traffic(kernel: str):
@@ -485,7 +485,7 @@ def main():
     # the master's roofline object: the HBM regime when the plan has one (A streams from DRAM), else the L2 regime
     hb = regimes.get("hbm")
     head = hb or regimes.get("l2") or {}
-    mtr, mtrd = traffic_of(master_kernel, lambda t: master_alg_bytes(method, V, t["K"], t["pg_iterations"], t["passes"]))
+    mtr, mtrd = traffic_of(master_kernel + ("@method3" if method == 3 else ""), lambda t: master_alg_bytes(method, V, t["K"], t["pg_iterations"], t["passes"]))
     n_head = max(1, head.get("solves", 1))
     master_roofline = {
         "kernel": f"{master_kernel} (restricted master problem over the dense block A, method {method})",
