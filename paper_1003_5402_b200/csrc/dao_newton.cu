@@ -1,4 +1,4 @@
-// dao_newton.cu -- step 8 with master_method = 2: the restricted master problem  min_{y >= 0} F(A y)
+// dao_newton.cu -- step 8 with master_method = 2 and 3: the restricted master problem  min_{y >= 0} F(A y)
 // by PROJECTED NEWTON on the free variables.  F is a convex piecewise quadratic
 // (eq. 3-5, 9-10), so on a fixed voxel active set its Hessian  H = A^T diag(2 c) A,
 // c_j = a_j [z_j < T_j^-] + b_j [z_j > T_j^+],  is exact and a Newton step lands on the minimiser of the
@@ -8,9 +8,10 @@
 // oracle (reading S2), so parity is unaffected by the choice of method.
 //
 // ONE persistent cooperative kernel, one CTA per SM, 16 warps (128 registers each).  The dose block is
-// stored tiled (NewtonLayout): the K live columns of a tile of T voxels are one contiguous range,
-// fetched by ONE cp.async.bulk (1-D TMA) into a stage of a shared-memory ring (issued by lane 0 of an
-// otherwise idle back warp).  With all K columns of a tile resident, one pass computes EVERYTHING at a
+// stored tiled (NewtonLayout; the voxels are spread over the tiles, a_index): two meta rows (structure ids,
+// thresholds) and the K live columns of a tile of T voxels are one contiguous range, fetched by ONE
+// cp.async.bulk (1-D TMA) into a stage of a shared-memory ring (issued by lane 0 of an otherwise idle back
+// warp).  With all K columns of a tile resident, one pass computes EVERYTHING at a
 // trial point y; the warps are specialised:
 //  front warps (8):
 //   Z  z_j = sum_k y_k A[k][j]                        (fp64, thread per voxel and k-slice)
@@ -26,6 +27,10 @@
 // in shared memory.  The trial point y + t d (t = 1 unless a bound is hit first) is accepted on
 // sufficient decrease of F -- the next pass IS the evaluation -- else t is shortened by the secant
 // of phi'(t) = d . grad(y + t d).  All sums fp64 in a fixed order: bit-reproducible.
+//
+// master_method = 3 is the same kernel template with TC = true: the Hessian on the 5th-generation tensor cores
+// (tcgen05.mma kind::tf32 on a hi/lo split of sqrt(s) A, accumulators in TMEM); see the comments at the control
+// warps and at pass_tc below, and DESIGN.md sections 6 and 13.
 #include "dao_internal.cuh"
 #include "dao_ptx.cuh"
 #include "dao_grid_reduce.cuh"
