@@ -175,9 +175,11 @@ struct ScratchPtrs {
   int32_t *keyA, *rowA, *keyB, *rowB;
   float *valA, *valB;
   int32_t *tile_hist;
+  int32_t *scan_sums;      // block totals of the multi-CTA scan
   int32_t *flags;
 };
 constexpr int kRadixThreads = 256, kRadixItems = 16, kRadixTile = kRadixThreads * kRadixItems;
+constexpr int kScanChunk = 16384;    // elements per CTA of the multi-CTA scan
 
 static void carve_scratch(Carver &cv, const Dims &dm, bool host_inputs, ScratchPtrs *s) {
   const size_t nz = (size_t)dm.nnz + 64;
@@ -199,6 +201,7 @@ static void carve_scratch(Carver &cv, const Dims &dm, bool host_inputs, ScratchP
   s->valB = cv.take<float>(nz);
   const size_t n_tiles = ((size_t)dm.nnz + kRadixTile - 1) / kRadixTile;
   s->tile_hist = cv.take<int32_t>(256 * n_tiles + 1024);
+  s->scan_sums = cv.take<int32_t>((256 * n_tiles) / kScanChunk + 1024);
   s->flags = cv.take<int32_t>(260);
 }
 
@@ -306,8 +309,21 @@ dao_status setup_sizes(const dao_csr *D, const dao_mlc *mlc, const dao_structs *
   st = fetch_row_ptr(D, &rp, err);
   if (st != DAO_OK) return st;
   HostLayout L;
-  st = make_layout(rp.data(), D->n_vox, effective_sigma(opt, D->n_vox), &L, err);
-  if (st != DAO_OK) return st;
+  const int sigma = effective_sigma(opt, D->n_vox);
+  if (sigma >= D->n_vox && D->n_vox > 1) {
+    // Sizes only: with ONE window sorted by descending length l_0 >= l_1 >= ..., slice s stores 32 l_{32 s} <= the sum of
+    // the 32 lengths of slice s - 1, so the padded copy holds at most nnz + 32 l_0 elements -- no sort needed here
+    // (dao_create computes the exact layout while the matrix uploads).
+    int32_t max_len = 0;
+    for (int32_t j = 0; j < D->n_vox; ++j) max_len = std::max(max_len, rp[j + 1] - rp[j]);
+    L.n_vox_pad = (int32_t)align_up((size_t)std::max(D->n_vox, 1), 128);
+    L.n_slices = L.n_vox_pad / kSellC;
+    L.sell_elems = D->nnz + (int64_t)kSellC * max_len;
+    if (L.sell_elems >= ((int64_t)1 << 32) - 64) { *err = "sliced-ELL copy of D would exceed 2^32 elements"; return DAO_E_UNSUPPORTED; }
+  } else {
+    st = make_layout(rp.data(), D->n_vox, sigma, &L, err);
+    if (st != DAO_OK) return st;
+  }
   Carver cw{nullptr};
   DevPtrs dp{};
   carve_workspace(cw, dm, L, &dp, n_sm);
@@ -455,6 +471,63 @@ __global__ void __launch_bounds__(1024) k_scan_inclusive(int32_t *data, int64_t 
   }
 }
 
+// Multi-CTA in-place inclusive scan (the radix sort's tile histograms: 256 x n_tiles counters, 3M on configs[1]; one
+// CTA took 1.4 ms per pass): CTA b scans its chunk of kScanChunk elements and writes the chunk total, one CTA scans
+// the totals (k_scan_inclusive), every chunk adds the total of the chunks before it.
+__global__ void __launch_bounds__(1024) k_scan_chunks(int32_t *data, int64_t n, int32_t *sums) {
+  __shared__ int32_t warp_tot[32];
+  __shared__ int32_t carry_s;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int64_t lo = (int64_t)blockIdx.x * kScanChunk, hi = lo + kScanChunk < n ? lo + kScanChunk : n;
+  if (tid == 0) carry_s = 0;
+  __syncthreads();
+  for (int64_t base = lo; base < hi; base += 4096) {
+    int32_t v[4];
+    int32_t sm = 0;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int64_t idx = base + (int64_t)tid * 4 + u;
+      v[u] = idx < hi ? data[idx] : 0;
+      sm += v[u];
+    }
+    int32_t inc = sm;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += t;
+    }
+    if (lane == 31) warp_tot[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+      int32_t wt = warp_tot[lane];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int32_t t = __shfl_up_sync(0xffffffffu, wt, o);
+        if (lane >= o) wt += t;
+      }
+      warp_tot[lane] = wt;
+    }
+    __syncthreads();
+    int32_t run = carry_s + (warp > 0 ? warp_tot[warp - 1] : 0) + (inc - sm);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int64_t idx = base + (int64_t)tid * 4 + u;
+      run += v[u];
+      if (idx < hi) data[idx] = run;
+    }
+    __syncthreads();
+    if (tid == 1023) carry_s = run;
+    __syncthreads();
+  }
+  if (tid == 0) sums[blockIdx.x] = carry_s;
+}
+__global__ void __launch_bounds__(1024) k_scan_add(int32_t *data, int64_t n, const int32_t *__restrict__ sums) {
+  if (blockIdx.x == 0) return;
+  const int32_t add = sums[blockIdx.x - 1];
+  const int64_t lo = (int64_t)blockIdx.x * kScanChunk, hi = lo + kScanChunk < n ? lo + kScanChunk : n;
+  for (int64_t i = lo + threadIdx.x; i < hi; i += 1024) data[i] += add;
+}
+
 // LSD radix pass, 8 bits: (1) per-tile digit histogram, (2) scan of [digit][tile] counts,
 // (3) stable scatter.  Elements are taken warp-blocked (warp w of a tile owns 32*kRadixItems
 // consecutive elements, visited 32 at a time), so index order = visiting order.
@@ -568,6 +641,24 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   std::vector<int32_t> rp;
   st = fetch_row_ptr(D, &rp, &c->err);
   if (st != DAO_OK) return st;
+  Carver cs{reinterpret_cast<unsigned char *>(scratch)};
+  ScratchPtrs sp{};
+  const bool host_in = D->mem == DAO_MEM_HOST;
+  carve_scratch(cs, dm, host_in, &sp);
+  if (cs.off > scratch_bytes) {
+    c->err = "workspace or scratch smaller than dao_workspace_bytes reported";
+    return DAO_E_ALLOC;
+  }
+  // the large uploads go out first: the host computes the sliced-ELL layout (a sort of the rows by length) while
+  // they are in flight
+  if (host_in) {
+    SETUP_CUDA(cudaMemcpyAsync(sp.row_ptr, D->row_ptr, ((size_t)dm.n_vox + 1) * 4, cudaMemcpyHostToDevice, c->stream));
+    if (dm.nnz > 0) {
+      SETUP_CUDA(cudaMemcpyAsync(sp.col, D->col_idx, (size_t)dm.nnz * 4, cudaMemcpyHostToDevice, c->stream));
+      SETUP_CUDA(cudaMemcpyAsync(sp.val, D->val, (size_t)dm.nnz * 4, cudaMemcpyHostToDevice, c->stream));
+    }
+    SETUP_CUDA(cudaMemcpyAsync(sp.vs, s->vox_struct, (size_t)dm.n_vox * 4, cudaMemcpyHostToDevice, c->stream));
+  }
   HostLayout L;
   c->opt.sell_sigma = effective_sigma(&c->opt, D->n_vox);
   st = make_layout(rp.data(), D->n_vox, c->opt.sell_sigma, &L, &c->err);
@@ -575,11 +666,7 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
 
   Carver cw{reinterpret_cast<unsigned char *>(workspace)};
   carve_workspace(cw, dm, L, &c->d, c->n_sm);
-  Carver cs{reinterpret_cast<unsigned char *>(scratch)};
-  ScratchPtrs sp{};
-  const bool host_in = D->mem == DAO_MEM_HOST;
-  carve_scratch(cs, dm, host_in, &sp);
-  if (cw.off > workspace_bytes || cs.off > scratch_bytes) {
+  if (cw.off > workspace_bytes) {
     c->err = "workspace or scratch smaller than dao_workspace_bytes reported";
     return DAO_E_ALLOC;
   }
@@ -612,13 +699,7 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
   // ---- inputs on the device ----
   const int32_t *d_row_ptr, *d_col, *d_vs;
   const float *d_val;
-  if (host_in) {
-    SETUP_CUDA(cudaMemcpyAsync(sp.row_ptr, D->row_ptr, ((size_t)dm.n_vox + 1) * 4, cudaMemcpyHostToDevice, q));
-    if (dm.nnz > 0) {
-      SETUP_CUDA(cudaMemcpyAsync(sp.col, D->col_idx, (size_t)dm.nnz * 4, cudaMemcpyHostToDevice, q));
-      SETUP_CUDA(cudaMemcpyAsync(sp.val, D->val, (size_t)dm.nnz * 4, cudaMemcpyHostToDevice, q));
-    }
-    SETUP_CUDA(cudaMemcpyAsync(sp.vs, s->vox_struct, (size_t)dm.n_vox * 4, cudaMemcpyHostToDevice, q));
+  if (host_in) {                 // uploaded above, before the host computed the layout
     d_row_ptr = sp.row_ptr; d_col = sp.col; d_val = sp.val; d_vs = sp.vs;
   } else {
     d_row_ptr = D->row_ptr; d_col = D->col_idx; d_val = D->val; d_vs = s->vox_struct;
@@ -705,7 +786,13 @@ dao_status setup_build(Ctx *c, const dao_csr *D, const dao_mlc *mlc, const dao_s
       float *dst_val = last ? d.t_val : ov;
       k_radix_hist<<<n_tiles, kRadixThreads, 0, q>>>(ik, dm.nnz, pass * 8, n_tiles, sp.tile_hist);
       SETUP_CUDA(cudaGetLastError());
-      k_scan_inclusive<<<1, 1024, 0, q>>>(sp.tile_hist, (int64_t)256 * n_tiles);
+      {
+        const int64_t n_scan = (int64_t)256 * n_tiles;
+        const int n_chunks = (int)((n_scan + kScanChunk - 1) / kScanChunk);
+        k_scan_chunks<<<n_chunks, 1024, 0, q>>>(sp.tile_hist, n_scan, sp.scan_sums);
+        k_scan_inclusive<<<1, 1024, 0, q>>>(sp.scan_sums, (int64_t)n_chunks);
+        k_scan_add<<<n_chunks, 1024, 0, q>>>(sp.tile_hist, n_scan, sp.scan_sums);
+      }
       SETUP_CUDA(cudaGetLastError());
       k_radix_scatter<<<n_tiles, kRadixThreads, 0, q>>>(ik, ir, iv, dm.nnz, pass * 8, n_tiles, sp.tile_hist, ok, dst_row,
                                                        dst_val);
