@@ -49,16 +49,17 @@ constexpr int kMaxStruct = 255;
 constexpr int kNoStruct = 255;         // sid value of a voxel without penalty
 constexpr int kMaxRedux = DAO_MAX_APERTURES + 8;   // doubles per grid reduction in the master (methods 0, 1)
 
-// ---- master_method = 2 (projected Newton, dao_newton.cu) ----
-constexpr int kNewtonMaxK = 103;   // largest pool method 2 handles (13 block rows of the Hessian); larger k_max: method 1
-// The aperture-dose block is stored TILED: tile t (T internal voxels) holds its k_max columns back to
-// back, each padded to TP = T + 4 floats (TP = 4 mod 32: conflict-free tensor-core fragment loads), so
-// the K live columns of a tile are ONE contiguous range = one bulk copy.
+// ---- master_method = 2, 3 (projected Newton, dao_newton.cu) ----
+constexpr int kNewtonMaxK = 103;   // largest pool methods 2, 3 handle (13 block rows of the Hessian); larger k_max: method 1
+// The aperture-dose block is stored TILED: tile t holds T voxels (voxel i sits in tile i mod n_tiles at slot
+// i / n_tiles, a_index) as rows of TP = T + 4 floats: `meta_rows` rows with the structure ids and per-voxel
+// thresholds of its voxels, then its k_max columns back to back, so that the meta rows and the K live columns of
+// a tile are ONE contiguous range = one bulk copy.
 struct NewtonLayout {
   int32_t T = 0;            // voxels per tile (0: plain aperture-major layout, methods 0 and 1)
   int32_t TP = 0;           // floats per column inside a tile
   int32_t n_tiles = 0;      // ceil(n_vox_pad / T)
-  int64_t tile_stride = 0;  // floats between consecutive tiles = k_max * TP
+  int64_t tile_stride = 0;  // floats between consecutive tiles = (meta_rows + k_max) * TP
   int32_t n_stages = 0;     // ring stages of stage_bytes
   int32_t stage_bytes = 0;  // k_max * TP * 4 rounded to 128
   int32_t nb_max = 0;       // 8x8 block rows of the augmented Hessian at K = k_max: ceil((k_max + 1) / 8)
@@ -163,7 +164,7 @@ struct DevPtrs {
   uint8_t *sid;            // [n_vox_pad] structure id or kNoStruct
   StructEntry *stab;       // [256]
   float *vt;               // [n_vox_pad] per-voxel threshold T_j (re-optimisation mode), internal order
-  // CSR of D^T (rows = beamlets, entries = internal voxel ids)
+  // CSR of D^T (rows = beamlets, entries = the CALLER's voxel ids: pi is kept in the caller's order)
   int32_t *t_ptr;          // [n_bl+1]
   int32_t *t_row;          // [nnz padded to kTChunk] caller voxel ids, ascending inside a row
   float *t_val;
@@ -195,10 +196,10 @@ struct DevPtrs {
   unsigned long long *ap_hash;   // [k_max] aperture_hash of every pool aperture (duplicate test: compare, then verify)
   int32_t *ap_left;        // [k_max * max_rows_per_beam]
   int32_t *ap_right;
-  float *A;                // [k_max][n_vox_pad] aperture-major dose block
+  float *A;                // dose block: [k_max][n_vox_pad] aperture-major (methods 0, 1) or tiled (methods 2, 3: NewtonLayout, a_index)
   double *y;               // [k_max]
   // master
-  double *mz;              // [n_vox_pad] z = A y
+  double *mz;              // z = A y: [n_vox_pad] internal order (methods 0, 1) or [n_tiles * T] in the tiled order (methods 2, 3)
   double *mdz;             // [n_vox_pad] dz = A p
   uint4 *ll_part;          // [2][n_cta][kMaxRedux] flagged slots {lo32, epoch, hi32, epoch} of the grid reductions
   uint4 *ll_result;        // [2][kMaxRedux]
@@ -236,7 +237,7 @@ struct Ctx {
   int device = 0, n_sm = 0;
   int spmv_grid = 0, master_grid = 0;
   int red_stride = kMaxRedux;   // slots per CTA of the grid reductions (ll_part)
-  NewtonLayout nwt{};           // master_method = 2
+  NewtonLayout nwt{};           // master_method = 2, 3
   size_t master_smem = 0;
   int master_slab = 0, master_stages = 0, master_z_in_smem = 0;
   bool x_in_smem = true;
@@ -313,11 +314,11 @@ size_t chain_pricing_smem(int32_t max_rows, int32_t width);   // shared memory o
 // dao_fmo.cu
 dao_status fmo_solve(Ctx *c, int32_t max_iter, double tol, bool warm_start, dao_fmo_info *out);
 
-// dao_master.cu (methods 0, 1) -- both dispatch to dao_newton.cu when master_method = 2
+// dao_master.cu (methods 0, 1) -- both dispatch to dao_newton.cu when master_method >= 2
 cudaError_t master_configure(Ctx *c);
 cudaError_t launch_master(Ctx *c, bool add_candidate);
 
-// dao_newton.cu (method 2)
+// dao_newton.cu (methods 2, 3)
 NewtonLayout newton_layout(int32_t k_max, int32_t n_vox_pad, int32_t n_struct, bool tc);   // host only, no device query
 cudaError_t newton_configure(Ctx *c);
 cudaError_t launch_newton(Ctx *c, bool add_candidate);
