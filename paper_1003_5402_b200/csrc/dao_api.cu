@@ -70,6 +70,18 @@ static dao_status read_state(Ctx *c) {
   c->K = c->h_state->K;
   return DAO_OK;
 }
+// The same read-back in two halves: the copy is enqueued (and marked by an event) BEFORE further work goes into the
+// stream, the host then waits for the event only -- the GPU keeps running what was enqueued behind the copy.
+static dao_status enqueue_state_copy(Ctx *c) {
+  API_CUDA(cudaMemcpyAsync(c->h_state, c->d.state, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
+  API_CUDA(cudaEventRecord(c->ev_state, c->stream));
+  return DAO_OK;
+}
+static dao_status wait_state_copy(Ctx *c) {
+  API_CUDA(cudaEventSynchronize(c->ev_state));
+  c->K = c->h_state->K;
+  return DAO_OK;
+}
 
 // steps 1-3 at the current intensities
 static dao_status enqueue_dose(Ctx *c) {
@@ -130,6 +142,7 @@ dao_status dao_create(const dao_csr *D, const dao_mlc *mlc, const dao_structs *s
   if (st == DAO_OK) {
     cudaError_t e = cudaMallocHost(reinterpret_cast<void **>(&c->h_state), sizeof(DevState));
     for (int i = 0; i < 8 && e == cudaSuccess; ++i) e = cudaEventCreate(&c->ev[i]);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_state, cudaEventDisableTiming);
     if (e != cudaSuccess) {
       c->err = std::string("host-side CUDA resources: ") + cudaGetErrorString(e);
       st = DAO_E_CUDA;
@@ -141,6 +154,7 @@ dao_status dao_create(const dao_csr *D, const dao_mlc *mlc, const dao_structs *s
     g_last_error = c->err;
     if (c->h_state) cudaFreeHost(c->h_state);
     for (int i = 0; i < 8; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    if (c->ev_state) cudaEventDestroy(c->ev_state);
     delete c;
     return st;
   }
@@ -154,6 +168,7 @@ dao_status dao_destroy(dao_ctx *ctx) {
   cudaStreamSynchronize(c->stream);
   if (c->h_state) cudaFreeHost(c->h_state);
   for (int i = 0; i < 8; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+  if (c->ev_state) cudaEventDestroy(c->ev_state);
   delete c;
   return DAO_OK;
 }
@@ -270,11 +285,16 @@ dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out) {
   double acc[6] = {0, 0, 0, 0, 0, 0};
   int n_resolve = 0;
   c->iter_seconds.clear();
+  // Without timers the dose SpMV of the NEXT iteration (= the final dose evaluation when the loop ends) is enqueued
+  // right behind the master, after the copy of the state block: the host reads the state while that SpMV runs, so
+  // the GPU does not idle through the host round trip of the one synchronisation per iteration.
+  bool dose_pending = false;
   while (c->K < max_apertures) {
     if (timers) API_CUDA(cudaEventRecord(c->ev[0], c->stream));
-    API_CUDA(launch_intensity(c));
+    if (!dose_pending) API_CUDA(launch_intensity(c));
     if (timers) API_CUDA(cudaEventRecord(c->ev[1], c->stream));
-    API_CUDA(launch_spmv(c, kSpmvObjective, c->d.x, c->d.z));
+    if (!dose_pending) API_CUDA(launch_spmv(c, kSpmvObjective, c->d.x, c->d.z));
+    dose_pending = false;
     if (timers) API_CUDA(cudaEventRecord(c->ev[2], c->stream));
     API_CUDA(launch_spmv_t(c, c->d.g, c->d.w));
     if (timers) API_CUDA(cudaEventRecord(c->ev[3], c->stream));
@@ -288,7 +308,16 @@ dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out) {
     API_CUDA(launch_master(c, true));
     if (timers) API_CUDA(cudaEventRecord(c->ev[6], c->stream));
     const int32_t k_before = c->K;
-    st = read_state(c);                 // the one host synchronisation of this iteration
+    if (timers) {
+      st = read_state(c);               // the one host synchronisation of this iteration
+    } else {
+      st = enqueue_state_copy(c);
+      if (st != DAO_OK) return st;
+      st = enqueue_dose(c);             // x is the one the master just wrote (or left unchanged)
+      if (st != DAO_OK) return st;
+      dose_pending = true;
+      st = wait_state_copy(c);          // the one host synchronisation of this iteration
+    }
     if (st != DAO_OK) return st;
     ++info.n_iterations;
     if (timers) {
@@ -302,6 +331,7 @@ dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out) {
     if (c->h_state->done == 2 && n_resolve < 2 && c->K > 0) {
       // stalled on a duplicate after an unconverged master (S6): solve the master further, then price again
       ++n_resolve;
+      dose_pending = false;             // the re-solve changes x: the dose enqueued above is stale
       API_CUDA(launch_master(c, false));
       st = read_state(c);
       if (st != DAO_OK) return st;
@@ -310,9 +340,11 @@ dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out) {
     if (c->h_state->done) { info.converged = c->h_state->done == 1 ? 1 : 0; info.stalled = c->h_state->done == 2 ? 1 : 0; break; }
     if (c->K == k_before) break;        // nothing was added (pool full)
   }
-  // final dose evaluation of the returned plan (steps 1-3)
-  st = enqueue_dose(c);
-  if (st != DAO_OK) return st;
+  // final dose evaluation of the returned plan (steps 1-3), unless it is already in the stream
+  if (!dose_pending) {
+    st = enqueue_dose(c);
+    if (st != DAO_OK) return st;
+  }
   API_CUDA(cudaEventRecord(c->ev[6], c->stream));
   st = read_state(c);
   if (st != DAO_OK) return st;

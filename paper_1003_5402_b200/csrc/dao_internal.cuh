@@ -252,6 +252,7 @@ struct Ctx {
   bool cand_appended = false;   // the last pricing launch already wrote the candidate into the pool tables
   double objective = 0.0;
   cudaEvent_t ev[8] = {};
+  cudaEvent_t ev_state = nullptr;   // marks the copy of the state block (dao_run reads it while later work runs)
   int64_t n_launches = 0;       // kernels launched on the hot path since dao_create (dao_run reports the difference)
   std::vector<double> iter_seconds;   // [iterations of the last dao_run][6]: per kernel class, when options.timers != 0
   std::string err;
