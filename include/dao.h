@@ -321,6 +321,53 @@ dao_status dao_price_from_w(dao_ctx *ctx, const float *w_dev, const int32_t *row
                             const int32_t *beam_row_ptr_dev, int32_t n_rows, int32_t n_beams,
                             int32_t *left_dev, int32_t *right_dev, double *vstar_dev,
                             double *beam_price_dev, int32_t *best_dev);
+/* ---- pricing for callers that cannot allocate device memory ---------------------------------------
+ * Steps 5-6 (per leaf row the most negative contiguous interval, per-beam sums, best beam)
+ * with NO context, NO workspace and NO allocation of any kind: the same row kernel and the same last-CTA tail
+ * as dao_price_from_w, but the intermediate arrays the tail needs (max |w| per leaf row and per beam, the
+ * ticket counter that elects the last CTA) live in a fixed array compiled into the library image instead of in
+ * a dao_create workspace.
+ *
+ * Who this is for.  Every other call of this library works inside a context, and a context needs a workspace
+ * somebody obtained from cudaMalloc (or from a framework's allocator, which calls it).  Some hosts of a pricing
+ * step cannot do that at the moment they need the answer: a treatment-console process whose device memory was
+ * handed out in full at start-up and is owned by another component; a plug-in that is given device pointers by
+ * its host application but no allocator; a delivery-time safety loop whose coding rules forbid any call that
+ * may block on the driver's allocator lock or grow the process footprint (cudaMalloc and cudaFree both
+ * synchronise the device and can fail late, when there is nobody left to handle it).  Such a caller already
+ * owns w and the MLC tables and somewhere to put the answer; this entry point asks for nothing else.
+ *
+ * Arguments: as dao_price_from_w with caller tables -- all DEVICE pointers on the CURRENT device, which must
+ * also be the device of `cuda_stream` (NULL = legacy default stream): w_dev fp32 [row_bl_ptr[n_rows]];
+ * row_bl_ptr_dev int32 [n_rows+1] and beam_row_ptr_dev int32 [n_beams+1], both starting at 0 and non-decreasing
+ * (not checked: they are device data); outputs left/right int32 [n_rows] (half-open leaves inside the row,
+ * closed row = (0, 0)), vstar double [n_rows], beam_price double [n_beams], best int32 [1].  Consecutive-leaf
+ * rule only (DAO_MLC_CONSECUTIVE).  Asynchronous: nothing is synchronised; outputs are valid once the stream
+ * reaches the end of the launch.  Bit-identical to dao_price_from_w on the same inputs.
+ *
+ * Limits.  1 <= n_rows <= DAO_STATIC_MAX_ROWS and 1 <= n_beams <= DAO_STATIC_MAX_BEAMS, otherwise DAO_E_SHAPE
+ * with the limit named in dao_last_error(NULL) and nothing launched.  The fixed array is DAO_STATIC_SCRATCH_BYTES
+ * (136 KiB) of device memory on every GPU that loads the library, held until the process exits, whether or not
+ * this function is ever called.
+ *
+ * First call on a device: the library looks up the array's device address (cudaGetSymbolAddress, once per
+ * device, with that device current; this is also what makes the CUDA runtime load the library's device code
+ * if nothing has yet).  Make that first call during start-up, outside any stream capture and before timing
+ * matters; later calls on that device only enqueue a 256-byte memset of the ticket and one kernel.
+ *
+ * Sharing.  All calls on a device use the one array, and it keeps whatever the previous call left there.  The
+ * function clears the part that must start at zero (the ticket) in stream order before its kernel; the rest is
+ * fully rewritten before it is read.  Two calls whose kernels can overlap on the GPU (different streams, or
+ * different host threads on different streams) RACE on it and return garbage: issue them on one stream, or
+ * order them with events.  Calls from several host threads on the same stream are safe. */
+#define DAO_STATIC_MAX_ROWS 16384
+#define DAO_STATIC_MAX_BEAMS 1024
+#define DAO_STATIC_SCRATCH_BYTES (256 + 8 * DAO_STATIC_MAX_ROWS + 8 * DAO_STATIC_MAX_BEAMS)
+dao_status dao_price_from_w_static(const float *w_dev, const int32_t *row_bl_ptr_dev,
+                                   const int32_t *beam_row_ptr_dev, int32_t n_rows, int32_t n_beams,
+                                   int32_t *left_dev, int32_t *right_dev, double *vstar_dev,
+                                   double *beam_price_dev, int32_t *best_dev, void *cuda_stream);
+
 /* Load a pool of apertures (host arrays laid out as in dao_plan) with intensities y (host, may be
  * NULL = zeros) replacing the current pool: builds the dose columns (step 7) but does not solve.
  * Lets the parity harness solve the master on the oracle's pool. */

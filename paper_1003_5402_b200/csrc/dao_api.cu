@@ -497,6 +497,14 @@ dao_status dao_price_from_w(dao_ctx *ctx, const float *w_dev, const int32_t *row
   return DAO_OK;
 }
 
+dao_status dao_price_from_w_static(const float *w_dev, const int32_t *row_bl_ptr_dev, const int32_t *beam_row_ptr_dev,
+                                   int32_t n_rows, int32_t n_beams, int32_t *left_dev, int32_t *right_dev,
+                                   double *vstar_dev, double *beam_price_dev, int32_t *best_dev, void *cuda_stream) {
+  // no context: failures are reported through dao_last_error(NULL) of the calling thread
+  return price_from_w_static(w_dev, row_bl_ptr_dev, beam_row_ptr_dev, n_rows, n_beams, left_dev, right_dev, vstar_dev,
+                             beam_price_dev, best_dev, static_cast<cudaStream_t>(cuda_stream), &g_last_error);
+}
+
 dao_status dao_set_pool(dao_ctx *ctx, int32_t n_apertures, const int32_t *beam, const int32_t *ap_row_ptr,
                         const int32_t *left, const int32_t *right, const double *y) {
   Ctx *c = reinterpret_cast<Ctx *>(ctx);

@@ -311,6 +311,10 @@ cudaError_t launch_pricing(Ctx *c, const float *w, const int32_t *row_bl_ptr, co
                            bool update_state, int32_t max_row_len = 0 /* 0 = unknown: warp-per-row kernel */);
 cudaError_t launch_append_candidate(Ctx *c);
 size_t chain_pricing_smem(int32_t max_rows, int32_t width);   // shared memory of k_price_chain
+// steps 5-6 without a context, scratch in a fixed array of the library image (dao_price_from_w_static, dao.h)
+dao_status price_from_w_static(const float *w, const int32_t *row_bl_ptr, const int32_t *beam_row_ptr, int32_t n_rows,
+                               int32_t n_beams, int32_t *left, int32_t *right, double *vstar, double *beam_price,
+                               int32_t *best_out, cudaStream_t stream, std::string *err);
 
 // dao_fmo.cu
 dao_status fmo_solve(Ctx *c, int32_t max_iter, double tol, bool warm_start, dao_fmo_info *out);

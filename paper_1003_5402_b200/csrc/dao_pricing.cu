@@ -7,6 +7,8 @@
 #include <math_constants.h>
 
 #include <algorithm>
+#include <mutex>
+#include <string>
 
 namespace dao {
 
@@ -731,6 +733,99 @@ cudaError_t launch_append_candidate(Ctx *c) {
                                                            c->d.left, c->d.right, c->d.ap_beam, c->d.ap_left,
                                                            c->d.ap_right, c->d.ap_hash, c->d.xmask);
   return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// dao_price_from_w_static: steps 5-6 for a caller that has no context and may not allocate (a host process whose
+// device memory is owned by someone else, or whose rules forbid cudaMalloc / cudaFree at run time -- see dao.h).
+// Same row kernel body and same last-CTA tail as the one-launch path of launch_pricing; what that path keeps in the
+// context's workspace sits in this fixed array of the library image instead:
+//     [0, 256)                        ticket counter of the tail (uint32, the rest of the line unused)
+//     [256, 256 + 8 MAX_ROWS)         max |w| per leaf row   (double)
+//     [.., .. + 8 MAX_BEAMS)          max |w| per beam       (double)
+// One copy per GPU that loads the library, for the life of the process.  In HOST code the name below is only a
+// handle for cudaGetSymbolAddress -- it is not a device address and must never be handed to a kernel as one; the
+// host side looks the address up once per device and passes that pointer.
+// ------------------------------------------------------------------------------------------
+constexpr size_t kStaticTicketBytes = 256;
+constexpr size_t kStaticScratchBytes = DAO_STATIC_SCRATCH_BYTES;
+static_assert(kStaticScratchBytes == kStaticTicketBytes + 8 * (size_t)DAO_STATIC_MAX_ROWS + 8 * (size_t)DAO_STATIC_MAX_BEAMS,
+              "dao.h and the scratch layout disagree");
+static_assert(DAO_STATIC_MAX_ROWS < kPriceSeqMinRows, "the static entry point only has the one-launch kernel");
+static __device__ __align__(256) unsigned char g_static_price_scratch[kStaticScratchBytes];
+
+__global__ void __launch_bounds__(256) k_price_rows_static(const float *w, const int32_t *row_bl_ptr,
+                                                           const int32_t *beam_row_ptr, int32_t n_rows, int32_t n_beams,
+                                                           double *vstar, int32_t *left, int32_t *right,
+                                                           double *beam_price, int32_t *best_out, unsigned char *scratch) {
+  double *row_absmax = reinterpret_cast<double *>(scratch + kStaticTicketBytes);
+  double *beam_absmax = row_absmax + DAO_STATIC_MAX_ROWS;
+  price_rows_body(w, row_bl_ptr, n_rows, vstar, left, right, row_absmax, nullptr);
+  PriceTail q{};                       // st = null: beam sums and the best beam, no candidate bookkeeping
+  q.ticket = reinterpret_cast<uint32_t *>(scratch);
+  q.do_beams = 1;
+  q.n_beams = n_beams; q.n_rows = n_rows;
+  q.beam_row_ptr = beam_row_ptr; q.row_bl_ptr = row_bl_ptr;
+  q.vstar = vstar; q.row_absmax = row_absmax; q.beam_price = beam_price; q.beam_absmax = beam_absmax;
+  q.left = left; q.right = right; q.best_out = best_out;
+  price_tail(q);
+}
+
+constexpr int kStaticMaxDevices = 64;
+static std::mutex g_static_mutex;
+static unsigned char *g_static_scratch_of_device[kStaticMaxDevices];   // device address of the array, per device
+
+dao_status price_from_w_static(const float *w, const int32_t *row_bl_ptr, const int32_t *beam_row_ptr, int32_t n_rows,
+                               int32_t n_beams, int32_t *left, int32_t *right, double *vstar, double *beam_price,
+                               int32_t *best_out, cudaStream_t stream, std::string *err) {
+  if (!w || !row_bl_ptr || !beam_row_ptr || !left || !right || !vstar || !beam_price || !best_out) {
+    *err = "dao_price_from_w_static: null pointer";
+    return DAO_E_ARG;
+  }
+  if (n_rows < 1 || n_beams < 1) {
+    *err = "dao_price_from_w_static: n_rows and n_beams must be >= 1";
+    return DAO_E_ARG;
+  }
+  if (n_rows > DAO_STATIC_MAX_ROWS || n_beams > DAO_STATIC_MAX_BEAMS) {
+    *err = "dao_price_from_w_static: " + std::to_string(n_rows) + " leaf rows / " + std::to_string(n_beams) +
+           " beams exceed the fixed scratch array (DAO_STATIC_MAX_ROWS = " + std::to_string(DAO_STATIC_MAX_ROWS) +
+           ", DAO_STATIC_MAX_BEAMS = " + std::to_string(DAO_STATIC_MAX_BEAMS) +
+           "); use dao_price_from_w with a context for larger problems";
+    return DAO_E_SHAPE;
+  }
+  auto cuda_fail = [&](const char *what, cudaError_t e) {
+    *err = std::string("dao_price_from_w_static: ") + what + ": " + cudaGetErrorString(e);
+    return DAO_E_CUDA;
+  };
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail("cudaGetDevice", e);
+  if (dev < 0 || dev >= kStaticMaxDevices) {
+    *err = "dao_price_from_w_static: device ordinal beyond the per-device address table";
+    return DAO_E_UNSUPPORTED;
+  }
+  unsigned char *scratch = nullptr;
+  {
+    // set-up, once per device, with that device current: the array's address on THIS device
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    scratch = g_static_scratch_of_device[dev];
+    if (scratch == nullptr) {
+      e = cudaGetSymbolAddress(reinterpret_cast<void **>(&scratch), g_static_price_scratch);
+      if (e != cudaSuccess) return cuda_fail("cudaGetSymbolAddress", e);
+      if (scratch == nullptr) return cuda_fail("cudaGetSymbolAddress returned a null address", cudaErrorInvalidSymbol);
+      g_static_scratch_of_device[dev] = scratch;
+    }
+  }
+  // the array keeps the last call's contents: the ticket must start at zero (a launch that died half way would
+  // otherwise leave it counting); the two max|w| arrays are written in full before the tail reads them
+  e = cudaMemsetAsync(scratch, 0, kStaticTicketBytes, stream);
+  if (e != cudaSuccess) return cuda_fail("cudaMemsetAsync", e);
+  const int wpb = 8;
+  k_price_rows_static<<<(n_rows + wpb - 1) / wpb, wpb * 32, 0, stream>>>(w, row_bl_ptr, beam_row_ptr, n_rows, n_beams, vstar,
+                                                                        left, right, beam_price, best_out, scratch);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail("k_price_rows_static", e);
+  return DAO_OK;
 }
 
 }  // namespace dao

@@ -29,7 +29,8 @@ MAX_APERTURES = 128
 EXPORTS = ["dao_default_options", "dao_workspace_bytes", "dao_create", "dao_price", "dao_solve_master",
            "dao_run", "dao_get_plan", "dao_reset", "dao_destroy", "dao_last_error", "dao_get_vector",
            "dao_get_dims", "dao_spmv", "dao_spmv_t", "dao_eval_x", "dao_price_from_w", "dao_set_pool",
-           "dao_resolve_master", "dao_fmo_solve"]
+           "dao_resolve_master", "dao_fmo_solve", "dao_price_from_w_static"]
+STATIC_MAX_ROWS, STATIC_MAX_BEAMS = 16384, 1024     # DAO_STATIC_MAX_ROWS / DAO_STATIC_MAX_BEAMS of dao.h
 
 
 class DaoError(RuntimeError):
@@ -149,6 +150,45 @@ def default_options(**overrides) -> COptions:
 
 def _np_ptr(a: np.ndarray) -> int:
     return a.ctypes.data
+
+
+def price_from_w_static(w_dev, row_bl_ptr_dev, beam_row_ptr_dev, out=None, stream=None):
+    """``dao_price_from_w_static``: steps 5-6 (row pricing, beam sums, best beam) on device tensors with no
+    :class:`Dao` context and no device allocation inside the library -- for hosts that own ``w`` and the MLC
+    tables but may not (or cannot) call ``cudaMalloc`` when they need the answer; the library's intermediate
+    arrays live in a fixed 136 KiB array of ``libdao.so`` instead of a workspace.  At most ``STATIC_MAX_ROWS``
+    leaf rows and ``STATIC_MAX_BEAMS`` beams (``DaoError`` with ``DAO_E_SHAPE`` beyond).  All calls on a GPU
+    share that array: keep them on one stream or order them, overlapping calls race.  The first call on a
+    device looks the array's address up; make it at start-up.
+
+    ``out`` = ``(left, right, vstar, beam_price, best)`` device tensors (int32 [n_rows] x 2, float64 [n_rows],
+    float64 [n_beams], int32 [1]) the caller already holds; when None this wrapper creates them with torch --
+    a convenience of the Python side only, the C call itself takes them as arguments.  ``stream``: a
+    ``torch.cuda.Stream`` (default: torch's current stream).  Asynchronous; returns the five tensors."""
+    import torch
+    lib = load_library()
+    n_rows, n_beams = row_bl_ptr_dev.numel() - 1, beam_row_ptr_dev.numel() - 1
+    for t, dt in ((w_dev, torch.float32), (row_bl_ptr_dev, torch.int32), (beam_row_ptr_dev, torch.int32)):
+        assert t.is_cuda and t.dtype == dt and t.is_contiguous()
+    if out is None:
+        out = (torch.empty(max(n_rows, 0), dtype=torch.int32, device=w_dev.device),
+               torch.empty(max(n_rows, 0), dtype=torch.int32, device=w_dev.device),
+               torch.empty(max(n_rows, 0), dtype=torch.float64, device=w_dev.device),
+               torch.empty(max(n_beams, 0), dtype=torch.float64, device=w_dev.device),
+               torch.empty(1, dtype=torch.int32, device=w_dev.device))
+    le, ri, vs, bp, best = out
+    for t, dt, n in ((le, torch.int32, n_rows), (ri, torch.int32, n_rows), (vs, torch.float64, n_rows),
+                     (bp, torch.float64, n_beams), (best, torch.int32, 1)):
+        assert t.is_cuda and t.dtype == dt and t.is_contiguous() and t.numel() >= n
+    s = torch.cuda.current_stream(w_dev.device) if stream is None else stream
+    with torch.cuda.device(w_dev.device):
+        st = lib.dao_price_from_w_static(C.c_void_p(w_dev.data_ptr()), C.c_void_p(row_bl_ptr_dev.data_ptr()),
+                                         C.c_void_p(beam_row_ptr_dev.data_ptr()), C.c_int32(n_rows), C.c_int32(n_beams),
+                                         C.c_void_p(le.data_ptr()), C.c_void_p(ri.data_ptr()), C.c_void_p(vs.data_ptr()),
+                                         C.c_void_p(bp.data_ptr()), C.c_void_p(best.data_ptr()), C.c_void_p(s.cuda_stream))
+    if st != DAO_OK:
+        raise DaoError(st, (lib.dao_last_error(None) or b"").decode())
+    return le, ri, vs, bp, best
 
 
 @dataclass
