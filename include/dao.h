@@ -14,7 +14,9 @@
  *   6. beam selection        price_b = sum of the row minima of beam b; b* = argmin_b (ties: smallest b)
  *                                                                           PAPER.md:169
  *   7. aperture dose column  a_K = sum_{i in A_K} D_i.                      PAPER.md:69 (eq. 2)
- *   8. restricted master     min_{y >= 0} F(A y) by gradient projection
+ *   8. restricted master     min_{y >= 0} F(A y): gradient projection as the paper names it (methods 0, 1) or
+ *                            projected Newton to the same unique optimum (methods 2, 3; 2 is the default)
+ *                                                                           PAPER.md:114, 134
  *   9. the column-generation loop over 1-8
  *
  * Conventions
@@ -142,8 +144,9 @@ typedef struct {
                                 tensor cores, one pass over A per iteration), 3 = the same projected Newton method
                                 with the Hessian on the 5th-generation tensor cores (tcgen05, TF32 hi/lo split,
                                 TMEM accumulators: H to ~2^-21 relative; dose, objective and gradient -- all
-                                that enters the stopping test -- stay fp64); pools of more than 103 apertures
-                                use method 1.  Same stopping test and the same (unique) optimal value for all
+                                that enters the stopping test -- stay fp64; k_max <= 56 only: with a larger
+                                pool capacity method 3 runs as method 2); pools of more than 103 apertures
+                                use method 1.  dao_get_dims reports the method in effect.  Same stopping test and the same (unique) optimal value for all
                                 four; reading S2 */
   int32_t sell_sigma;        /* sorting window (rows) of the internal sliced-ELL layout of D; 1 = keep the
                                 caller's voxel order; 0 = library default */
@@ -177,7 +180,7 @@ typedef struct {
 
 typedef struct {
   int32_t n_apertures;       /* pool size after the call */
-  int32_t n_pg_iter;         /* projected-gradient (methods 0, 1) or Newton (method 2) iterations taken */
+  int32_t n_pg_iter;         /* projected-gradient (methods 0, 1) or Newton (methods 2, 3) iterations taken */
   int32_t hit_max_iter;      /* 1: stopped by master_max_iter */
   int32_t n_restarts;        /* conjugate-direction restarts (method 1) */
   double objective;          /* F(A y) at return */
@@ -240,9 +243,13 @@ typedef enum {               /* dao_get_vector selectors; lengths in elements */
   DAO_VEC_BEAM_PRICE = 8,    /* double [n_beams] */
   DAO_VEC_HISTORY = 9,       /* dao_iter_record [k_max] (first n_apertures valid) */
   DAO_VEC_MASTER_Z = 10,     /* double [n_vox]  z = A y as the master holds it, caller's voxel order */
-  DAO_VEC_ITER_SECONDS = 12, /* double [k_max][6]  HOST only: device seconds of every column-generation iteration of the last
-                                dao_run per kernel class {intensity, dose SpMV, SpMV^T, pricing, column, master}
-                                (CUDA events; zeros when options.timers == 0 and beyond the iterations run) */
+  DAO_VEC_ITER_SECONDS = 12, /* double [k_max][6]  HOST only: one row per aperture the last dao_run ADDED, in order (row i
+                                belongs to the i-th history record that call wrote): device seconds per kernel class
+                                {intensity, dose SpMV, SpMV^T, pricing, column, master} of the iteration that added it,
+                                plus those of preceding iterations that added nothing (a stalled pricing and its master
+                                re-solve, S6).  The last pricing of a run that ends converged or stalled adds no row; its
+                                time is in dao_run_info.seconds_*.  CUDA events; zeros when options.timers == 0 and
+                                beyond the rows written */
   DAO_VEC_MASTER_PHASES = 11 /* uint64 [16]     phase timers of the master kernel, accumulated since dao_create when
                                 dao_options.reserved has bit 1 (value 2) set, else zeros.  Nanoseconds of CTA 0 in:
                                 0 set-up and z = A y, 1 gradient pass over A, 2 gradient reduction, 3 direction,
@@ -303,7 +310,8 @@ typedef struct {
   int64_t nnz;               /* of D as given */
   int64_t sell_elems;        /* stored elements of the sliced-ELL copy (>= nnz: padding) */
   int32_t sell_slice_rows, sell_sigma;
-  int32_t n_sm, reserved;
+  int32_t n_sm;
+  int32_t master_method;     /* the master method in effect (dao_options.master_method after the capacity fallbacks) */
 } dao_dims;
 dao_status dao_get_dims(const dao_ctx *ctx, dao_dims *out);
 

@@ -3,6 +3,8 @@
 // Every arithmetic step runs in the kernels of dao_spmv.cu / dao_pricing.cu / dao_master.cu.
 #include "dao_internal.cuh"
 
+#include <math_constants.h>
+
 #include <cstring>
 #include <new>
 
@@ -62,6 +64,10 @@ __global__ void k_set_pool_state(DevState *st, int32_t K) {
   st->K = K;
   st->cand_valid = 0;
   st->done = 0;
+  // no master solve has been made for THIS pool: a duplicate candidate priced before one is reported as stalled,
+  // never as a proof of optimality (reading S6 uses m_hit_max / m_kkt of the last solve)
+  st->m_hit_max = 1;
+  st->m_kkt = CUDART_INF;
 }
 
 static dao_status read_state(Ctx *c) {
@@ -183,7 +189,7 @@ dao_status dao_get_dims(const dao_ctx *ctx, dao_dims *out) {
   if (!c || !out) return DAO_E_ARG;
   out->n_vox = c->n_vox; out->n_bl = c->n_bl; out->n_beams = c->n_beams; out->n_rows = c->n_rows;
   out->n_struct = c->n_struct; out->k_max = c->opt.k_max; out->nnz = c->nnz; out->sell_elems = c->sell_elems;
-  out->sell_slice_rows = kSellC; out->sell_sigma = c->opt.sell_sigma; out->n_sm = c->n_sm; out->reserved = 0;
+  out->sell_slice_rows = kSellC; out->sell_sigma = c->opt.sell_sigma; out->n_sm = c->n_sm; out->master_method = c->opt.master_method;
   return DAO_OK;
 }
 
@@ -283,6 +289,7 @@ dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out) {
   const int32_t hit0 = c->h_state->n_hit_max;
   const int64_t launches0 = c->n_launches;
   double acc[6] = {0, 0, 0, 0, 0, 0};
+  double pending[6] = {0, 0, 0, 0, 0, 0};   // times not yet written to a DAO_VEC_ITER_SECONDS row
   int n_resolve = 0;
   c->iter_seconds.clear();
   // Without timers the dose SpMV of the NEXT iteration (= the final dose evaluation when the loop ends) is enqueued
@@ -325,17 +332,30 @@ dao_status dao_run(dao_ctx *ctx, int32_t max_apertures, dao_run_info *out) {
         float ms = 0.f;
         API_CUDA(cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]));
         acc[i] += ms * 1e-3;
-        c->iter_seconds.push_back(ms * 1e-3);
+        pending[i] += ms * 1e-3;
       }
     }
     if (c->h_state->done == 2 && n_resolve < 2 && c->K > 0) {
       // stalled on a duplicate after an unconverged master (S6): solve the master further, then price again
       ++n_resolve;
       dose_pending = false;             // the re-solve changes x: the dose enqueued above is stale
+      if (timers) API_CUDA(cudaEventRecord(c->ev[5], c->stream));
       API_CUDA(launch_master(c, false));
+      if (timers) API_CUDA(cudaEventRecord(c->ev[6], c->stream));
       st = read_state(c);
       if (st != DAO_OK) return st;
+      if (timers) {                     // the re-solve is master time of this call
+        float ms = 0.f;
+        API_CUDA(cudaEventElapsedTime(&ms, c->ev[5], c->ev[6]));
+        acc[5] += ms * 1e-3;
+        pending[5] += ms * 1e-3;
+      }
       continue;
+    }
+    if (timers && c->K > k_before) {
+      // one row per aperture ADDED, so that row i pairs with history record i of this call; an iteration that added
+      // nothing (a stalled pricing and its re-solve) is charged to the next aperture's row
+      for (int i = 0; i < 6; ++i) { c->iter_seconds.push_back(pending[i]); pending[i] = 0.0; }
     }
     if (c->h_state->done) { info.converged = c->h_state->done == 1 ? 1 : 0; info.stalled = c->h_state->done == 2 ? 1 : 0; break; }
     if (c->K == k_before) break;        // nothing was added (pool full)

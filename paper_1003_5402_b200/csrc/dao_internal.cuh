@@ -50,6 +50,7 @@ constexpr int kNoStruct = 255;         // sid value of a voxel without penalty
 constexpr int kMaxRedux = DAO_MAX_APERTURES + 8;   // doubles per grid reduction in the master (methods 0, 1)
 
 // ---- master_method = 2, 3 (projected Newton, dao_newton.cu) ----
+constexpr int kNewtonTcMaxK = 56;  // largest pool method 3 handles (8 block rows of the augmented Hessian = the 64 rows of one operand half); larger k_max: method 2
 constexpr int kNewtonMaxK = 103;   // largest pool methods 2, 3 handle (13 block rows of the Hessian); larger k_max: method 1
 // The aperture-dose block is stored TILED: tile t holds T voxels (voxel i sits in tile i mod n_tiles at slot
 // i / n_tiles, a_index) as rows of TP = T + 4 floats: `meta_rows` rows with the structure ids and per-voxel
@@ -69,7 +70,7 @@ struct NewtonLayout {
   size_t smem = 0;          // dynamic shared memory of k_master_newton
   // master_method = 3: the Hessian on the 5th-generation tensor cores (tcgen05, TF32 hi/lo split, TMEM accumulators)
   int32_t tc = 0;           // 1: k_master_newton<true>
-  int32_t kp = 0;           // rows of one half (hi or lo) of the operand tile: 64 (k_max <= 56) or 128
+  int32_t kp = 0;           // rows of one half (hi or lo) of the operand tile: 64 (method 3 exists for k_max <= kNewtonTcMaxK = 56 only)
   int32_t lbo = 0;          // bytes between the two 16-byte K-halves of an MMA k-step (core matrices adjacent along the voxels)
   int32_t sbo = 0;          // bytes between groups of 8 operand rows
   int32_t w_bytes = 0;      // bytes of one operand tile: (2 kp / 8) sbo
@@ -254,7 +255,7 @@ struct Ctx {
   cudaEvent_t ev[8] = {};
   cudaEvent_t ev_state = nullptr;   // marks the copy of the state block (dao_run reads it while later work runs)
   int64_t n_launches = 0;       // kernels launched on the hot path since dao_create (dao_run reports the difference)
-  std::vector<double> iter_seconds;   // [iterations of the last dao_run][6]: per kernel class, when options.timers != 0
+  std::vector<double> iter_seconds;   // [apertures added by the last dao_run][6]: per kernel class, when options.timers != 0
   std::string err;
 };
 

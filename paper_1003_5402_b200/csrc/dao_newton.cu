@@ -62,7 +62,7 @@ constexpr int kTcGroups = kNW / kTcGroupWarps;
 constexpr int kTcHV = 16;                // voxels per half = two MMA k-steps
 constexpr uint32_t kTcLbo = 128, kTcSbo = (kTcHV / 4) * kTcLbo, kTcHalfBytes = 16 * kTcSbo;
 constexpr uint32_t kTcCols = 64 * kTcGroups;   // TMEM columns: one 128 x 64 fp32 accumulator per group
-constexpr int kTcMaxK = 56;              // 8 block rows of the augmented Hessian fit the 64 rows of one operand half
+constexpr int kTcMaxK = kNewtonTcMaxK;             // 8 block rows of the augmented Hessian fit the 64 rows of one operand half
 constexpr int kTcMaxStages = 12;
 constexpr int kNwtMetaRows = 2;
 constexpr int kNwtAcc = 7;               // gradient accumulators per thread: rows r, r + 8, ... < 56

@@ -541,7 +541,7 @@ __device__ void price_select_body(const double *beam_price, const double *beam_a
     const bool improving = price < -tol_abs;
     int done = improving ? 0 : 1;
     if (improving && s_dup) done = (!st->m_hit_max && -price <= 10.0 * fmax(st->m_kkt, tol_abs)) ? 1 : 2;
-    if (s_dup) st->n_duplicates += 1;
+    if (improving && s_dup) st->n_duplicates += 1;   // as the oracle's driver: the ordinary converged stop is not a duplicate event
     st->cand_beam = best;
     st->cand_hash = cand_hash;
     st->cand_price = price;

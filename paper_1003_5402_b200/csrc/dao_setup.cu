@@ -260,6 +260,9 @@ static dao_status check_args(const dao_csr *D, const dao_mlc *mlc, const dao_str
   dm->max_rows = std::max(max_rows, 1);
   // the projected-Newton master handles pools up to kNewtonMaxK apertures; larger pools use method 1
   dm->master_method = (opt->master_method >= 2 && opt->k_max > kNewtonMaxK) ? 1 : opt->master_method;
+  // the tcgen05 variant holds 8 block rows of the Hessian: beyond kNewtonTcMaxK apertures it is method 2, and says so
+  // (dao_get_dims reports the method in effect)
+  if (dm->master_method == 3 && opt->k_max > kNewtonTcMaxK) dm->master_method = 2;
   dm->n_struct = s->n_struct;
   dm->chain_states = 0;
   if (opt->mlc_mode == DAO_MLC_INTERDIGITATION || opt->mlc_mode == DAO_MLC_CONNECTED) {

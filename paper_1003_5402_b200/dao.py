@@ -108,7 +108,7 @@ class CPlan(C.Structure):
 class CDims(C.Structure):
     _fields_ = [("n_vox", C.c_int32), ("n_bl", C.c_int32), ("n_beams", C.c_int32), ("n_rows", C.c_int32),
                 ("n_struct", C.c_int32), ("k_max", C.c_int32), ("nnz", C.c_int64), ("sell_elems", C.c_int64),
-                ("sell_slice_rows", C.c_int32), ("sell_sigma", C.c_int32), ("n_sm", C.c_int32), ("reserved", C.c_int32)]
+                ("sell_slice_rows", C.c_int32), ("sell_sigma", C.c_int32), ("n_sm", C.c_int32), ("master_method", C.c_int32)]
 
 
 ITER_RECORD_DTYPE = np.dtype([("k", "<i4"), ("beam", "<i4"), ("n_pg_iter", "<i4"), ("duplicate", "<i4"),

@@ -104,5 +104,6 @@ def test_method3_master_on_oracle_pool(D, mini):
 def test_method3_falls_back_above_56_apertures(D, mini):
     """Pools of more than 56 apertures do not fit one 64-row operand half: method 3 then runs as method 2."""
     with D.Dao(mini, k_max=60, master_method=3) as d3, D.Dao(mini, k_max=60, master_method=2) as d2:
+        assert d3.dims().master_method == 2 and d2.dims().master_method == 2     # reported, not silent
         a = d3.run(60); b = d2.run(60)
     assert a.objective == b.objective and a.n_passes_total == b.n_passes_total
