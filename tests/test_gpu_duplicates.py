@@ -18,7 +18,7 @@ def D():
     return dao
 
 
-@pytest.mark.parametrize("method", [1, 2, 3])
+@pytest.mark.parametrize("method", [0, 1, 2, 3])
 @pytest.mark.parametrize("tol", [0.1, 0.03])
 def test_duplicate_ends_the_run_as_in_the_oracle(D, tiny, tol, method):
     ref = orc.run(tiny, 30, master_tol=tol)
@@ -34,7 +34,7 @@ def test_duplicate_ends_the_run_as_in_the_oracle(D, tiny, tol, method):
     assert not hist["hit_max_iter"].any()
 
 
-@pytest.mark.parametrize("method", [1, 2, 3])
+@pytest.mark.parametrize("method", [0, 1, 2, 3])
 def test_duplicate_after_an_unconverged_master_is_reported_as_stalled(D, tiny, method):
     with D.Dao(tiny, k_max=30, master_max_iter=0, master_method=method) as d:
         info = d.run(30)

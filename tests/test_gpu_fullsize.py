@@ -107,17 +107,19 @@ def test_cfg1_lockstep_first_iterations(D, cfg1):
             assert -1e-5 <= rel <= REL_OBJ, (it, m.objective, res.objective)
 
 
-@pytest.mark.parametrize("method", [2, 3])
-def test_cfg1_plan_50_apertures(D, cfg1, method):
+@pytest.mark.parametrize("method,timers", [(2, 1), (3, 1), (1, 1), (2, 0), (1, 0)])
+def test_cfg1_plan_50_apertures(D, cfg1, method, timers):
     """The north-star target: a free-running 50-aperture plan of configs[1], run exactly as bench.py
     runs it, against (i) the oracle's own free-running plan (stored fixture), (ii) the oracle's
     recomputation of dose / objective / reduced costs from the GPU's plan.  Method 2 (the default; exact Hessian on
-    the fp64 tensor cores) and method 3 (Hessian on tcgen05 in split TF32)."""
+    the fp64 tensor cores), method 3 (Hessian on tcgen05 in split TF32) and method 1 (gradient projection with conjugated
+    directions, the family PAPER.md:134 names: its HBM-regime ring streams A from DRAM at this size); timers = 0 is the
+    branch of dao_run that bench.py times (speculative dose SpMV behind the state copy)."""
     ph = cfg1
     with open(os.path.join(GOLDEN, "oracle_plan_cfg1.json")) as f:
         gold = json.load(f)
     assert (gold["n_vox"], gold["n_bl"], gold["nnz"]) == (ph.n_vox, ph.n_bl, ph.nnz)
-    with D.Dao(ph, k_max=50, master_method=method) as d:
+    with D.Dao(ph, k_max=50, master_method=method, timers=timers) as d:
         info = d.run(50)
         plan = d.get_plan()
         hist = d.get_vector(D.VEC_HISTORY)[:info.n_apertures]

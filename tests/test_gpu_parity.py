@@ -16,6 +16,7 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 REL_DOSE = 1e-4
 REL_OBJ = 1e-3
+GP_MAX_ITER = 200000   # iteration cap for master_method 0 (plain gradient projection converges linearly)
 
 
 @pytest.fixture(scope="module")
@@ -155,12 +156,14 @@ def test_pricing_on_own_tables(D, mini):
 
 
 # ----------------------------------------------------------------------------- lock-step protocol
-@pytest.mark.parametrize("case,n_ap", [("cfg0", 12), ("mini", 20), ("mini_reopt", 12)])
-def test_lockstep_against_oracle(D, case, n_ap, cfg0, mini, mini_reopt):
+@pytest.mark.parametrize("case,n_ap,method", [("cfg0", 12, 2), ("mini", 20, 2), ("mini_reopt", 12, 2),
+                                               ("mini", 10, 0), ("mini", 20, 1), ("mini", 20, 3)])
+def test_lockstep_against_oracle(D, case, n_ap, method, cfg0, mini, mini_reopt):
     """SURVEY 8(c) lock-step: at every column-generation iteration the oracle recomputes each step
     from the GPU's own state; isolates every step's error from trajectory divergence."""
     ph = {"cfg0": cfg0, "mini": mini, "mini_reopt": mini_reopt}[case]
-    with D.Dao(ph, k_max=n_ap) as d:
+    # method 0 is the plain gradient projection PAPER.md:134 names: same stopping test, many more iterations
+    with D.Dao(ph, k_max=n_ap, master_method=method, master_max_iter=GP_MAX_ITER if method == 0 else 2000) as d:
         for it in range(n_ap):
             info = d.price()
             plan = d.get_plan()
@@ -195,11 +198,13 @@ def test_lockstep_against_oracle(D, case, n_ap, cfg0, mini, mini_reopt):
             assert np.abs(mz - yk @ A).max() <= 1e-6 * max(1.0, np.abs(mz).max())
 
 
-def test_master_on_oracle_pool(D, mini):
-    """dao_set_pool + dao_resolve_master on the oracle's 15-aperture pool: same optimum value."""
+@pytest.mark.parametrize("method", [0, 1, 2, 3])
+def test_master_on_oracle_pool(D, mini, method):
+    """dao_set_pool + dao_resolve_master on the oracle's 15-aperture pool: same optimum value (the optimum is unique,
+    PAPER.md:114, whichever of the four methods reaches it; 0 = the gradient projection PAPER.md:134 names)."""
     plan = orc.run(mini, 15, keep_A=True)
     vp = orc.voxel_params(mini.vox_struct, mini.t_under, mini.w_under, mini.t_over, mini.w_over)
-    with D.Dao(mini) as d:
+    with D.Dao(mini, master_method=method, master_max_iter=GP_MAX_ITER if method == 0 else 2000) as d:
         d.set_pool(plan.beams, plan.lefts, plan.rights)
         m = d.resolve_master()
         y = d.get_vector(D.VEC_Y)[:15]
@@ -212,14 +217,17 @@ def test_master_on_oracle_pool(D, mini):
 
 
 # ----------------------------------------------------------------------------- free-running plans
-@pytest.mark.parametrize("case", ["cfg0", "mini", "mini_reopt"])
-def test_free_running_50_apertures(D, case, cfg0, mini, mini_reopt):
+@pytest.mark.parametrize("case,method,n_ap", [("cfg0", 2, 50), ("mini", 2, 50), ("mini_reopt", 2, 50), ("mini", 0, 15),
+                                               ("mini", 1, 50), ("mini", 3, 50)])
+def test_free_running_50_apertures(D, case, method, n_ap, cfg0, mini, mini_reopt):
+    """(15 apertures for method 0: plain gradient projection needs ~1e4-1e5 iterations per solve as the pool grows)"""
     ph = {"cfg0": cfg0, "mini": mini, "mini_reopt": mini_reopt}[case]
-    with D.Dao(ph) as d:
-        info = d.run(50)
+    with D.Dao(ph, k_max=n_ap, master_method=method, master_max_iter=GP_MAX_ITER if method == 0 else 2000) as d:
+        info = d.run(n_ap)
         plan = d.get_plan()
         hist = d.get_vector(D.VEC_HISTORY)[:info.n_apertures]
-    ref = orc.run(ph, 50)
+    ref = orc.run(ph, n_ap)
+    assert info.n_hit_max_iter == 0
     assert abs(info.objective - ref.objective) <= REL_OBJ * ref.objective
     assert abs(plan.objective - info.objective) <= 1e-12 * info.objective
     # monotone decrease of the master optimum (convexity + warm start)
