@@ -9,8 +9,8 @@ path does not shard at these sizes: DESIGN.md "Multi-GPU"), one process per GPU 
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg1] [--impl reference]
 
-Prints ONE JSON line (rank 0).  `--impl reference` times the fp64 CPU oracle instead (a bounded
-sample of the same workload on the host cores).
+Prints ONE JSON line (rank 0).  `--impl reference` times the fp64 CPU oracle instead: one full plan of the
+same workload on one host core (minutes; --ref-apertures times a prefix and says so).
 """
 from __future__ import annotations
 
@@ -112,6 +112,27 @@ def ncu_traffic(kernel: str):
     except Exception:
         pass
     return None
+
+
+def measure_l2_bandwidth(torch, l2_bytes: int, reps: int = 400):
+    """A denominator for the L2-resident regime of the master ("below that, L2 bandwidth -- say so"):
+    read + write GB/s of a device-to-device copy whose source and destination together take a third of the L2, repeated
+    back to back so that every pass after the first hits the L2.  torch's copy kernel is the measuring tool here, like
+    the copy behind MEASURED_PEAKS.json; it is not on the product path and not counted in gpu_launches."""
+    n = max(1 << 20, (l2_bytes // 6) // 4096 * 4096)
+    src = torch.empty(n, dtype=torch.uint8, device="cuda").random_(0, 255)
+    dst = torch.empty_like(src)
+    for _ in range(20):
+        dst.copy_(src)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        dst.copy_(src)
+    e1.record()
+    torch.cuda.synchronize()
+    s = e0.elapsed_time(e1) * 1e-3
+    return {"GBps": 2.0 * n * reps / s * 1e-9, "bytes_per_buffer": int(n), "reps": reps,
+            "how": "torch device-to-device copy, source + destination = L2/3, back to back (read + write bytes / time)"}
 
 
 def master_alg_bytes(method: int, V: int, K: int, n_iter: int, n_passes: int) -> float:
@@ -377,7 +398,7 @@ def main():
     opts = dict(k_max=N_APERTURES, master_method=args.master_method)
     d = dao.Dao(ph, timers=0, **opts)
     dims = d.dims()
-    method = int(d.opt.master_method)
+    method = int(d.dims().master_method)          # the method in effect (capacity fallbacks applied)
     infos = []
     for _ in range(args.warmup):
         d.reset()
@@ -399,6 +420,7 @@ def main():
     last = infos[-1]
     n_it = sum(i.n_iterations for i in infos)
     launches = sum(i.n_kernel_launches for i in infos)
+    timed_plan = d.get_plan()
     d.close()
 
     # ---- per-kernel-class split: a separate pass with the library's CUDA-event timers on (same kernels, same plan;
@@ -410,7 +432,16 @@ def main():
         dt_.reset()
         tinfos.append(dt_.run(N_APERTURES))
     hist = dt_.get_vector(dao.VEC_HISTORY)[:tinfos[-1].n_apertures]
-    it_sec = dt_.get_vector(dao.VEC_ITER_SECONDS).reshape(-1, 6)[:tinfos[-1].n_iterations]
+    # the timed pass (timers = 0: speculative dose SpMV behind the state copy) and this pass (timers = 1, the branch the
+    # parity tests run against the oracle) must have produced the SAME plan, bit for bit -- a stale-dose or ordering bug
+    # in the untimed branch would show here
+    split_plan = dt_.get_plan()
+    assert (tinfos[-1].objective == last.objective and tinfos[-1].n_apertures == last.n_apertures and
+            tinfos[-1].n_iterations == last.n_iterations and tinfos[-1].n_passes_total == last.n_passes_total), \
+        ("timed (timers=0) and split (timers=1) passes disagree", last.objective, tinfos[-1].objective)
+    for f in ("beams", "intensity", "ap_row_ptr", "left", "right"):
+        assert np.array_equal(getattr(timed_plan, f), getattr(split_plan, f)), f"timers=0 / timers=1 plans differ in {f}"
+    it_sec = dt_.get_vector(dao.VEC_ITER_SECONDS).reshape(-1, 6)[:tinfos[-1].n_apertures]   # one row per aperture added: pairs with hist
     dt_.close()
     n_it_t = sum(i.n_iterations for i in tinfos)
     ab = algorithmic_bytes(ph)
@@ -446,8 +477,11 @@ def main():
             regimes[r] = {"solves": len(sel), "K_range": [min(x["K"] for x in sel), max(x["K"] for x in sel)],
                           "alg_bytes": bsum, "seconds": ssum, "achieved_GBps": bsum / ssum * 1e-9 if ssum > 0 else None,
                           "share_of_master_time": ssum / master_s_plan if master_s_plan > 0 else None}
+    l2_bw = measure_l2_bandwidth(torch, l2_bytes) if "l2" in regimes else None
     if "l2" in regimes:
-        regimes["l2"].update({"peak": None, "note": "4*V*K fits the L2: L2-bandwidth regime, no measured L2 peak on this pool"})
+        regimes["l2"].update({"peak": l2_bw["GBps"], "frac": regimes["l2"]["achieved_GBps"] / l2_bw["GBps"],
+                              "peak_source": l2_bw,
+                              "note": "4*V*K fits the L2: the peak is an L2-resident copy bandwidth measured in this run"})
     if "hbm" in regimes:
         regimes["hbm"].update({"peak": peak, "frac": regimes["hbm"]["achieved_GBps"] / peak})
     kernels["master"].update({
@@ -494,6 +528,16 @@ def main():
         "frac": hb["frac"] if hb else None, "traffic": mtr, "traffic_detail": mtrd, "peak_source": peak_src,
         "alg_bytes_per_launch": head.get("alg_bytes", 0.0) / n_head, "avg_launch_us": 1e6 * head.get("seconds", 0.0) / n_head,
         "alg_bytes_model": master_model, "share_of_step": kernels["master"]["share"],
+        # the same quotient over ALL launches of the plan (every pool size, L2-resident solves included) against the HBM
+        # peak: `frac` above describes the HBM-regime solves only
+        "frac_all_launches": (master_bytes_plan / master_s_plan * 1e-9 / peak) if master_s_plan > 0 else None,
+        "achieved_all_launches": (master_bytes_plan / master_s_plan * 1e-9) if master_s_plan > 0 else None,
+        "alg_bytes_per_launch_all": master_bytes_plan / max(1, len(solves)),
+        "avg_launch_us_all": 1e6 * master_s_plan / max(1, len(solves)),
+        # `traffic` is the ncu DRAM count of ONE captured launch; these are the algorithmic bytes of that same launch
+        "traffic_launch_alg_bytes": (mtrd or {}).get("alg_bytes_of_that_launch"),
+        "traffic_over_alg_same_launch": (mtrd or {}).get("dram_over_alg"),
+        "traffic_source": TRAFFIC_CSV + " (committed ncu capture of an earlier build of this kernel; re-capture after kernel changes)",
         "regime": (f"solves with 4*V_pad*K >= 0.8 x L2 ({l2_bytes >> 20} MB): K = {hb['K_range'][0]}..{hb['K_range'][1]}, "
                    f"{100 * hb['share_of_master_time']:.0f} % of the master's time; the other solves are L2-resident (see regimes)"
                    if hb else "every solve is L2-resident: no HBM figure, no measured L2 peak"),
@@ -531,7 +575,7 @@ def main():
     if rank == 0 and world == 1 and args.config == "cfg1" and not args.no_other_configs:
         others = {}
 
-        def plan_time(ph_o, n_ap, **o):
+        def plan_time(ph_o, n_ap, split=False, **o):
             with dao.Dao(ph_o, timers=0, k_max=n_ap, **o) as d3:
                 for _ in range(3):
                     d3.reset()
@@ -544,17 +588,33 @@ def main():
                     inf3 = d3.run(n_ap)
                 e1.record()
                 torch.cuda.synchronize()
-                return {"seconds_per_plan": e0.elapsed_time(e1) * 1e-3 / 3, "apertures": int(inf3.n_apertures),
-                        "objective": inf3.objective, "master_passes_over_A": int(inf3.n_passes_total),
-                        "master_method": int(d3.opt.master_method), "n_vox": int(ph_o.n_vox), "n_bl": int(ph_o.n_bl),
-                        "nnz": int(ph_o.nnz)}
+                res = {"seconds_per_plan": e0.elapsed_time(e1) * 1e-3 / 3, "apertures": int(inf3.n_apertures),
+                       "objective": inf3.objective, "master_passes_over_A": int(inf3.n_passes_total),
+                       "master_method": int(d3.dims().master_method), "n_vox": int(ph_o.n_vox), "n_bl": int(ph_o.n_bl),
+                       "nnz": int(ph_o.nnz)}
+            if split:
+                # BASELINE.json configs[4]: "per-iteration time split across SpMV, gradient, pricing and master solve"
+                # (the gradient is fused into the dose SpMV's epilogue): one more plan with the library's event timers on
+                with dao.Dao(ph_o, timers=1, k_max=n_ap, **o) as d4:
+                    d4.run(n_ap); d4.reset()
+                    i4 = d4.run(n_ap)
+                cls = {"intensity": i4.seconds_intensity, "spmv_dose_objective_gradient": i4.seconds_spmv,
+                       "spmv_t": i4.seconds_spmv_t, "pricing": i4.seconds_price, "column": i4.seconds_column,
+                       "master": i4.seconds_master}
+                tot4 = sum(cls.values())
+                res["per_iteration_split_us"] = {k: 1e6 * v / max(1, i4.n_iterations) for k, v in cls.items()}
+                res["split_share"] = {k: v / tot4 for k, v in cls.items()} if tot4 > 0 else None
+                res["split_same_plan"] = bool(i4.objective == res["objective"])
+            return res
 
         others["cfg1_master_method_3"] = plan_time(ph, N_APERTURES, master_method=3)
+        # the gradient projection PAPER.md:134 names (conjugated directions on the free face), same plan, same optimum
+        others["cfg1_master_method_1"] = plan_time(ph, N_APERTURES, master_method=1)
         for name, n_ap in (("paper_p1", 50), ("cfg2", 50), ("cfg4", 100)):
             if time.perf_counter() - T_PROCESS_START > (90.0 if name == "cfg4" else 150.0):
                 others[name] = {"skipped": "time budget of the default run (the whole run must end within minutes)"}
                 continue
-            others[name] = plan_time(phantom.make(name, 0), n_ap, master_method=args.master_method)
+            others[name] = plan_time(phantom.make(name, 0), n_ap, master_method=args.master_method, split=(name == "cfg4"))
 
     # ---- CPU baseline: the oracle as it stands, one full plan, rank 0, N = 1 only ----
     cpu = None
