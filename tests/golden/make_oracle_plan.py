@@ -1,6 +1,6 @@
 """Writes tests/golden/oracle_plan_<config>.json: the fp64 CPU oracle's free-running column-generation
 plan (O9) on a BASELINE.json phantom -- per-iteration beam, reduced
-cost and master optimum, and the final objective.  Calls ONLY the seeded input generator and
+cost and master optimum, the leaves of every aperture, and the final objective.  Calls ONLY the seeded input generator and
 oracle/ (never the CUDA path).  The GPU parity test compares its own free-running plan against the
 stored final objective within the north star's 1e-3.
 
@@ -39,6 +39,10 @@ def main():
         "kkt": [float(h.kkt) for h in plan.history],
         "n_duplicates": int(plan.n_duplicates), "stalled": bool(plan.stalled),
         "n_open_beamlets": [int(sum(int(r) - int(l) for l, r in zip(h.left, h.right))) for h in plan.history],
+        # the apertures themselves (half-open leaves of the rows of aperture k's beam, in row order), so that a test can
+        # load the ORACLE's pool at any size K with dao_set_pool and solve the master on it (lock-step at large K)
+        "left": [[int(v) for v in plan.lefts[k]] for k in range(len(plan.beams))],
+        "right": [[int(v) for v in plan.rights[k]] for k in range(len(plan.beams))],
     }
     path = os.path.join(HERE, f"oracle_plan_{config}.json")
     with open(path, "w") as f:

@@ -153,6 +153,44 @@ def test_cfg1_plan_50_apertures(D, cfg1, method, timers):
           f"pg iterations {info.n_pg_iter_total} kkt gap {gap:.2e}")
 
 
+@pytest.mark.parametrize("method", [1, 2, 3])
+def test_cfg1_master_on_the_oracles_large_pools(D, cfg1, method):
+    """Lock-step on the master where the dose block A has left the L2 (4 V K = 109 / 121 MB at K = 45 / 50): the pool
+    is the ORACLE's own (its first K apertures, leaves stored in the fixture), loaded with dao_set_pool; the GPU solves
+    the restricted master on it from y = 0 and must reach the oracle's optimum of that pool (unique: the model is
+    convex) -- (F_gpu - F*) / F* in [-1e-5, 1e-3] against the stored master_objective[K - 1] -- and its y
+    must satisfy the KKT conditions when the ORACLE recomputes dose, gradient and reduced costs (eq. 1, 8) from it."""
+    ph = cfg1
+    with open(os.path.join(GOLDEN, "oracle_plan_cfg1.json")) as f:
+        gold = json.load(f)
+    assert (gold["n_vox"], gold["n_bl"], gold["nnz"]) == (ph.n_vox, ph.n_bl, ph.nnz) and len(gold["left"]) == 50
+    # from y = 0 the conjugated gradient projection needs more than the default 2,000 iterations (dao_run warm-starts)
+    with D.Dao(ph, k_max=50, master_method=method, master_max_iter=50000 if method == 1 else 2000) as d:
+        for K in (45, 50):
+            beams = gold["beams"][:K]
+            lefts = [np.asarray(a, np.int32) for a in gold["left"][:K]]
+            rights = [np.asarray(a, np.int32) for a in gold["right"][:K]]
+            d.set_pool(beams, lefts, rights)
+            m = d.resolve_master()
+            y = d.get_vector(D.VEC_Y)[:K].copy()
+            f_star = gold["master_objective"][K - 1]
+            rel = (m.objective - f_star) / f_star
+            assert m.n_apertures == K and not m.hit_max_iter
+            assert -1e-5 <= rel <= REL_OBJ, (method, K, m.objective, f_star)
+            if K == 50:
+                _, _, _, _, w_o, F_o = pu.oracle_state_from_plan(ph, beams, lefts, rights, y)
+                assert abs(F_o - m.objective) <= 1e-6 * F_o            # A is stored in fp32 on the GPU
+                grad = np.zeros(K)
+                for k, b in enumerate(beams):
+                    msk = orc.aperture_open_mask(ph.n_bl, int(b), lefts[k], rights[k], ph.beam_row_ptr, ph.row_bl_ptr)
+                    grad[k] = w_o[msk.astype(bool)].sum()
+                # convexity: F(y) - F* <= grad.y - min(0, min grad) |y*|_1, |y*|_1 taken as 2 |y|_1
+                gap = float(grad @ y) + max(0.0, -grad.min()) * 2.0 * y.sum()
+                assert (y >= 0).all() and gap <= REL_OBJ * F_o, (method, gap, F_o)
+            print(f"cfg1 oracle pool K={K} method {method}: F_gpu={m.objective:.12g} F*={f_star:.12g} rel={rel:.2e} "
+                  f"iterations {m.n_pg_iter} passes {m.n_passes}")
+
+
 @pytest.mark.parametrize("config,n_ap", [("cfg2", 50), ("cfg4", 100), ("cfg1_reopt", 50)])
 def test_other_full_size_configs(D, config, n_ap):
     """BASELINE.json configs[2] (5-field head-and-neck shape, 50 apertures), configs[4] (7-field stress
